@@ -1,0 +1,130 @@
+// Device CSR builder: validation of the caller's graph and packing into
+// the sliced, relabelled, replica-tile-friendly layout of common.cuh.  The paper leaves the
+// storage of its "generally connected" model unstated (Fig. 2 L61) and only
+// says the graph is copied to the device once (L138); everything here is this library's.
+#pragma once
+#include "common.cuh"
+
+namespace ising {
+
+struct BuildReport {
+    unsigned int err_mask;     // bit k set = ISING_ERR_k seen
+    int max_abs_w;             // max |w|
+    long long w_sum;           // sum over directed entries (= 2 W)
+    long long absw_max;        // max_i sum_j |w_ij|
+};
+
+__device__ __forceinline__ long long load_w(const void* w, int wtype, long long e) {
+    return wtype == 1 ? (long long)reinterpret_cast<const int8_t*>(w)[e]
+                      : (long long)reinterpret_cast<const int32_t*>(w)[e];
+}
+
+// row_ptr[0] == 0, row_ptr[n] == nnz, monotone non-decreasing
+__global__ void k_check_rowptr(const long long* row_ptr, int32_t n, long long nnz, BuildReport* rep) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > n) return;
+    bool bad = false;
+    const long long v = row_ptr[i];
+    if (i == 0 && v != 0) bad = true;
+    if (i == n && v != nnz) bad = true;
+    if (v < 0 || v > nnz) bad = true;
+    if (i < n && row_ptr[i + 1] < v) bad = true;
+    if (bad) atomicOr(&rep->err_mask, 1u << 2);
+}
+
+// One warp per row: column range / order / self loops, symmetry (binary search of the
+// mirrored entry), colouring, sum_j |w_ij|.
+__global__ void k_validate(int32_t n, const long long* row_ptr, const int32_t* col, const void* w, int wtype,
+                           const int32_t* colour, int32_t n_colours, BuildReport* rep) {
+    const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (gw >= n) return;
+    const int32_t i = (int32_t)gw;
+    const long long b = row_ptr[i], e = row_ptr[i + 1];
+    unsigned int err = 0;
+    long long absw = 0, wsum = 0;
+    int maxabs = 0;
+    int ci = 0;
+    if (colour) {
+        ci = colour[i];
+        if (ci < 0 || ci >= n_colours) err |= 1u << 6;
+    }
+    for (long long idx = b + lane; idx < e; idx += 32) {
+        const int32_t j = col[idx];
+        if (j < 0 || j >= n) { err |= 1u << 2; continue; }
+        if (j == i) err |= 1u << 4;
+        if (idx > b && col[idx - 1] >= j) err |= 1u << 3;
+        const long long wv = load_w(w, wtype, idx);
+        long long lo = row_ptr[j], hi = row_ptr[j + 1];   // find i in row j
+        while (lo < hi) {
+            const long long mid = (lo + hi) >> 1;
+            if (col[mid] < i) lo = mid + 1; else hi = mid;
+        }
+        if (lo >= row_ptr[j + 1] || col[lo] != i || load_w(w, wtype, lo) != wv) err |= 1u << 5;
+        if (colour && colour[j] == ci) err |= 1u << 6;
+        const long long aw = wv < 0 ? -wv : wv;
+        absw += aw;
+        wsum += wv;
+        if (aw > maxabs) maxabs = (int)(aw > 0x7fffffffll ? 0x7fffffffll : aw);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        absw += __shfl_xor_sync(0xffffffffu, absw, o);
+        wsum += __shfl_xor_sync(0xffffffffu, wsum, o);
+        maxabs = max(maxabs, __shfl_xor_sync(0xffffffffu, maxabs, o));
+        err |= __shfl_xor_sync(0xffffffffu, err, o);
+    }
+    if (lane == 0) {
+        if (err) atomicOr(&rep->err_mask, err);
+        if (absw >= (1ll << 31)) atomicOr(&rep->err_mask, 1u << 7);
+        atomicMax(&rep->absw_max, absw);
+        atomicMax(&rep->max_abs_w, maxabs);
+        if (wsum != 0) atomicAdd(reinterpret_cast<unsigned long long*>(&rep->w_sum), (unsigned long long)wsum);
+    }
+}
+
+// One warp per slice: fill col4 / w4 (or w4w).  Cell (g, sr) of the slice holds group
+// q = g * SPR + part of row row0 + (sr >> log_spr), part = sr & (SPR - 1); edges 4q .. 4q+3.
+__global__ void k_pack(const SliceDesc* slices, uint32_t n_slices, const int32_t* perm, const int32_t* inv,
+                       const long long* row_ptr, const int32_t* col, const void* w, int wtype, int4* col4,
+                       uint32_t* w4, int4* w4w) {
+    const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (gw >= n_slices) return;
+    const SliceDesc d = slices[gw];
+    const int log_spr = (int)(d.meta & 0xffu), nrows = (int)(d.meta >> 8);
+    const uint32_t spr = 1u << log_spr;
+    const unsigned long long cells = (unsigned long long)d.G * kSubRows;
+    for (unsigned long long cell = lane; cell < cells; cell += 32) {
+        const uint32_t g = (uint32_t)(cell / kSubRows), sr = (uint32_t)(cell % kSubRows);
+        const uint32_t rloc = sr >> log_spr, part = sr & (spr - 1);
+        int cc[4];
+        int ww[4] = {0, 0, 0, 0};
+        if ((int)rloc < nrows) {
+            const uint32_t row = d.row0 + rloc;
+            const int32_t orig = perm[row];
+            const long long b = row_ptr[orig], deg = row_ptr[orig + 1] - b;
+            const long long q = (long long)g * spr + part;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const long long e = 4 * q + j;
+                if (e < deg) {
+                    cc[j] = inv[col[b + e]];
+                    ww[j] = (int)load_w(w, wtype, b + e);
+                } else {
+                    cc[j] = (int)row;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) cc[j] = (int)d.row0;
+        }
+        const size_t at = (size_t)d.off + cell;
+        col4[at] = make_int4(cc[0], cc[1], cc[2], cc[3]);
+        if (w4w) w4w[at] = make_int4(ww[0], ww[1], ww[2], ww[3]);
+        else w4[at] = ((uint32_t)ww[0] & 0xffu) | (((uint32_t)ww[1] & 0xffu) << 8) |
+                      (((uint32_t)ww[2] & 0xffu) << 16) | (((uint32_t)ww[3] & 0xffu) << 24);
+    }
+}
+
+}  // namespace ising

@@ -1,0 +1,753 @@
+// C-ABI entry points of the B200 Ising annealer (include/ising.h).
+//
+// Host side: argument validation, workspace carving, the O(n) slice planning of the
+// device layout, and the per-sweep launch sequence.  Every step of the hot path
+// (field, argmin, flip, write-back, cut reduction, best capture) runs in the kernels of
+// sparse_sweep.cuh / dense_tcgen05.cuh; there is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdint>
+#include <cstring>
+#include <new>
+#include <type_traits>
+#include <vector>
+
+#include "../../include/ising.h"
+#include "builder.cuh"
+#include "common.cuh"
+#include "dense_tcgen05.cuh"
+#include "sparse_sweep.cuh"
+
+using namespace ising;
+
+#define CK(call)                                  \
+    do {                                          \
+        cudaError_t e_ = (call);                  \
+        if (e_ != cudaSuccess) {                  \
+            (void)cudaGetLastError();             \
+            return ISING_ERR_CUDA;                \
+        }                                         \
+    } while (0)
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+struct Bump {
+    uint8_t* base;
+    size_t cap, used;
+    bool overflow;
+    void* take(size_t bytes) {
+        const size_t at = align_up(used);
+        if (at + bytes > cap) { overflow = true; used = at + bytes; return nullptr; }
+        used = at + bytes;
+        return base + at;
+    }
+};
+
+bool is_device_ptr(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+inline int spr_log2_for_degree(int64_t deg) {
+    int l = 0;
+    while (l < 4 && ((deg + (1ll << l) - 1) >> l) > kSubRowEdges) ++l;
+    return l;
+}
+
+// Upper bounds used by ising_workspace_bytes (any degree distribution).
+inline uint64_t bound_slices(int64_t n, int64_t nnz, int64_t C) {
+    return (uint64_t)n / 16 + 4 * ((uint64_t)nnz / 256) + 6 * (uint64_t)(C + 1) + 8;
+}
+inline uint64_t bound_slots(int64_t n, int64_t nnz, int64_t C) {
+    return (uint64_t)nnz + 128 * bound_slices(n, nnz, C) + 2048 * (uint64_t)(C + 1);
+}
+
+struct SmallArrays {
+    long long* accum[2];
+    long long* E[2];
+    long long* bestcut[2];
+    long long* accum_eval;
+    long long* out_tmp;    // 2 * max_replicas
+    int32_t* best_sweep;
+    int* flag;
+};
+
+size_t workspace_need(int64_t n, int64_t nnz, int wtype, int64_t max_replicas, int64_t C, bool wide,
+                      uint64_t n_slices, uint64_t slots, bool with_raw, bool dense) {
+    const uint64_t tiles = (uint64_t)(max_replicas + kTile - 1) / kTile;
+    size_t s = 0;
+    auto add = [&](size_t b) { s = align_up(s) + b; };
+    add(sizeof(BuildReport));
+    if (with_raw) {
+        add(8 * (size_t)(n + 1));
+        add(4 * (size_t)nnz);
+        add((size_t)wtype * (size_t)nnz);
+        add(4 * (size_t)n);
+    }
+    add(4 * (size_t)n);                       // perm
+    add(4 * (size_t)n);                       // inv
+    add(sizeof(SliceDesc) * (size_t)n_slices);
+    add(4 * (size_t)slots);                   // col4
+    add(1 * (size_t)slots);                   // w4
+    if (wide) add(4 * (size_t)slots);         // w4w
+    for (int k = 0; k < 3; ++k) add((size_t)tiles * (size_t)n * kTile);   // state x2, best
+    add((size_t)max_replicas * (size_t)n);    // io staging
+    for (int k = 0; k < 7; ++k) add(8 * (size_t)tiles * kTile);
+    add(16 * (size_t)tiles * kTile);          // out_tmp
+    add(4 * (size_t)tiles * kTile);           // best_sweep
+    add(256);                                 // flag
+    if (dense) add(dense_workspace_bytes(n, max_replicas));
+    return align_up(s) + kAlign;
+}
+
+}  // namespace
+
+struct ising_problem {
+    int32_t n = 0;
+    int64_t nnz = 0;
+    int32_t n_colours = 0;
+    int32_t max_replicas = 0;
+    int32_t tiles_max = 0;
+    int64_t W = 0;
+    int64_t absw_max = 0;
+    bool wide = false;
+    // device (inside the caller's workspace)
+    int32_t* perm = nullptr;
+    int32_t* inv = nullptr;
+    SliceDesc* slices = nullptr;
+    int4* col4 = nullptr;
+    uint32_t* w4 = nullptr;
+    int4* w4w = nullptr;
+    uint8_t* state[2] = {nullptr, nullptr};
+    uint8_t* best = nullptr;
+    int8_t* io_stage = nullptr;
+    SmallArrays sm{};
+    DenseEngine* dense = nullptr;
+    // host bookkeeping
+    std::vector<uint32_t> phase_begin;   // [n_colours + 1] slice ranges per colour (GS)
+    uint32_t n_slices = 0;
+    uint64_t slots = 0;
+    size_t ws_used = 0;
+    int cur = 0;
+    int parity = 0;
+    bool have_state = false;
+    bool have_best = false;
+    bool state_in_dense = false;         // current / best state live in the dense engine's layout
+    int32_t last_R = 0;
+    int64_t launches = 0;
+    int sm_count = 148;
+    int ctas_per_sm[2][3] = {{1, 1, 1}, {1, 1, 1}};
+    uint32_t flush_rows = 1;
+};
+
+namespace {
+
+template <int KIND>
+void launch_sweep_kind(ising_problem* p, const SweepParams& sp, dim3 grid, cudaStream_t st) {
+    if (p->wide) k_sweep<KIND, true><<<grid, kSweepThreads, 0, st>>>(sp);
+    else k_sweep<KIND, false><<<grid, kSweepThreads, 0, st>>>(sp);
+}
+
+void launch_sweep(ising_problem* p, int kind, SweepParams sp, int tiles, cudaStream_t st) {
+    const uint32_t nsl = sp.slice_end - sp.slice_begin;
+    if (nsl == 0) return;
+    const int occ = p->ctas_per_sm[p->wide ? 1 : 0][kind];
+    long long cap = ((long long)p->sm_count * occ + tiles - 1) / tiles;
+    if (cap < 1) cap = 1;
+    long long bx = (nsl + kWarpsPerCta - 1) / kWarpsPerCta;
+    if (bx > cap) bx = cap;
+    dim3 grid((unsigned)bx, (unsigned)tiles, 1);
+    if (kind == kKindGS) launch_sweep_kind<kKindGS>(p, sp, grid, st);
+    else if (kind == kKindJacobi) launch_sweep_kind<kKindJacobi>(p, sp, grid, st);
+    else launch_sweep_kind<kKindEval>(p, sp, grid, st);
+    p->launches++;
+}
+
+SweepParams base_params(const ising_problem* p) {
+    SweepParams sp{};
+    sp.col4 = p->col4;
+    sp.w4 = p->w4;
+    sp.w4w = p->w4w;
+    sp.slices = p->slices;
+    sp.perm = p->perm;
+    sp.tile_stride = (unsigned long long)p->n * kTile;
+    sp.slice_begin = 0;
+    sp.slice_end = p->n_slices;
+    sp.flush_rows = p->flush_rows;
+    return sp;
+}
+
+void launch_sweep_end(ising_problem* p, const uint8_t* src, int energy_mode, int first, int32_t T,
+                      long long* trace_row, int n_replicas, int tiles, cudaStream_t st) {
+    SweepEndParams ep{};
+    const int par = p->parity;
+    ep.src = src;
+    ep.best = p->best;
+    ep.accum_in = p->sm.accum[par];
+    ep.accum_zero = p->sm.accum[par ^ 1];
+    ep.E_in = p->sm.E[par];
+    ep.E_out = p->sm.E[par ^ 1];
+    ep.best_in = p->sm.bestcut[par];
+    ep.best_out = p->sm.bestcut[par ^ 1];
+    ep.best_sweep = p->sm.best_sweep;
+    ep.trace_row = trace_row;
+    ep.tile_stride = (unsigned long long)p->n * kTile;
+    ep.units = (unsigned long long)p->n * 2;
+    ep.W = p->W;
+    ep.n_replicas = n_replicas;
+    ep.energy_mode = energy_mode;
+    ep.first = first;
+    ep.T = T;
+    long long bx = (long long)((ep.units + 255) / 256);
+    long long cap = ((long long)p->sm_count * 8 + tiles - 1) / tiles;
+    if (bx > cap) bx = cap;
+    if (bx < 1) bx = 1;
+    if (energy_mode == 2) bx = 1;
+    k_sweep_end<<<dim3((unsigned)bx, (unsigned)tiles, 1), 256, 0, st>>>(ep);
+    p->launches++;
+    p->parity ^= 1;
+}
+
+ising_status check_device() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return ISING_ERR_UNSUPPORTED_DEVICE; }
+    int major = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return ISING_ERR_UNSUPPORTED_DEVICE;
+    }
+    return major == 10 ? ISING_OK : ISING_ERR_UNSUPPORTED_DEVICE;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ising_status_string(ising_status s) {
+    switch (s) {
+        case ISING_OK: return "ok";
+        case ISING_ERR_NULL_ARG: return "null argument";
+        case ISING_ERR_BAD_SHAPE: return "bad shape / out-of-range index / bad enum";
+        case ISING_ERR_UNSORTED_OR_DUP: return "row columns not strictly ascending";
+        case ISING_ERR_SELF_LOOP: return "self loop";
+        case ISING_ERR_ASYMMETRIC: return "graph or weights not symmetric";
+        case ISING_ERR_BAD_COLOURING: return "colouring out of range or not proper";
+        case ISING_ERR_FIELD_OVERFLOW: return "max_i sum_j |w_ij| >= 2^31";
+        case ISING_ERR_TOO_MANY_REPLICAS: return "too many replicas";
+        case ISING_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+        case ISING_ERR_NO_COLOURING_FOR_GS: return "Gauss-Seidel mode needs a colouring";
+        case ISING_ERR_UNSUPPORTED_DEVICE: return "no sm_100 (B200) device";
+        case ISING_ERR_CUDA: return "CUDA error";
+        case ISING_ERR_BAD_SPINS: return "spin value is neither +1 nor -1";
+        case ISING_ERR_NO_STATE: return "no state yet";
+        default: return "unknown status";
+    }
+}
+
+ising_status ising_workspace_bytes(int32_t n, int64_t nnz, int32_t wtype, int32_t max_replicas,
+                                   int32_t n_colours, size_t* bytes_out) {
+    if (!bytes_out) return ISING_ERR_NULL_ARG;
+    if (n <= 0 || nnz < 0 || n_colours < 0 || (wtype != ISING_W_INT8 && wtype != ISING_W_INT32))
+        return ISING_ERR_BAD_SHAPE;
+    if (max_replicas < 1 || max_replicas > 65536) return ISING_ERR_TOO_MANY_REPLICAS;
+    const bool dense = kDenseEnabled && nnz == (int64_t)n * (n - 1) && n >= 2;
+    *bytes_out = workspace_need(n, nnz, wtype, max_replicas, n_colours, wtype == ISING_W_INT32,
+                                bound_slices(n, nnz, n_colours), bound_slots(n, nnz, n_colours), true, dense);
+    return ISING_OK;
+}
+
+ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
+                            const void* weights, int32_t wtype, const int32_t* colour, int32_t n_colours,
+                            int32_t max_replicas, void* workspace, size_t workspace_bytes, int32_t flags,
+                            void* stream, ising_problem** out) {
+    if (!out || !row_ptr || !workspace || (nnz > 0 && (!col_idx || !weights))) return ISING_ERR_NULL_ARG;
+    if (n <= 0 || nnz < 0 || n_colours < 0 || (wtype != ISING_W_INT8 && wtype != ISING_W_INT32))
+        return ISING_ERR_BAD_SHAPE;
+    if ((colour == nullptr) != (n_colours == 0)) return ISING_ERR_BAD_COLOURING;
+    if (max_replicas < 1 || max_replicas > 65536) return ISING_ERR_TOO_MANY_REPLICAS;
+    if (ising_status s = check_device()) return s;
+    if ((reinterpret_cast<uintptr_t>(workspace) & (kAlign - 1)) != 0 || !is_device_ptr(workspace))
+        return ISING_ERR_WORKSPACE_TOO_SMALL;
+    cudaStream_t st = (cudaStream_t)stream;
+
+    Bump ws{(uint8_t*)workspace, workspace_bytes, 0, false};
+    BuildReport* d_rep = (BuildReport*)ws.take(sizeof(BuildReport));
+    if (ws.overflow) return ISING_ERR_WORKSPACE_TOO_SMALL;
+
+    // ---- bring the raw CSR to the device (staged in the workspace when it is host memory)
+    const bool rp_dev = is_device_ptr(row_ptr), ci_dev = nnz == 0 || is_device_ptr(col_idx);
+    const bool w_dev = nnz == 0 || is_device_ptr(weights), co_dev = colour && is_device_ptr(colour);
+    const long long* d_row_ptr = (const long long*)row_ptr;
+    const int32_t* d_col = col_idx;
+    const void* d_w = weights;
+    const int32_t* d_colour = colour;
+    if (!rp_dev) {
+        void* b = ws.take(8 * (size_t)(n + 1));
+        if (!b) return ISING_ERR_WORKSPACE_TOO_SMALL;
+        CK(cudaMemcpyAsync(b, row_ptr, 8 * (size_t)(n + 1), cudaMemcpyHostToDevice, st));
+        d_row_ptr = (const long long*)b;
+    }
+    if (!ci_dev) {
+        void* b = ws.take(4 * (size_t)nnz);
+        if (!b) return ISING_ERR_WORKSPACE_TOO_SMALL;
+        CK(cudaMemcpyAsync(b, col_idx, 4 * (size_t)nnz, cudaMemcpyHostToDevice, st));
+        d_col = (const int32_t*)b;
+    }
+    if (!w_dev) {
+        void* b = ws.take((size_t)wtype * (size_t)nnz);
+        if (!b) return ISING_ERR_WORKSPACE_TOO_SMALL;
+        CK(cudaMemcpyAsync(b, weights, (size_t)wtype * (size_t)nnz, cudaMemcpyHostToDevice, st));
+        d_w = b;
+    }
+    if (colour && !co_dev) {
+        void* b = ws.take(4 * (size_t)n);
+        if (!b) return ISING_ERR_WORKSPACE_TOO_SMALL;
+        CK(cudaMemcpyAsync(b, colour, 4 * (size_t)n, cudaMemcpyHostToDevice, st));
+        d_colour = (const int32_t*)b;
+    }
+
+    // ---- validate on the device
+    CK(cudaMemsetAsync(d_rep, 0, sizeof(BuildReport), st));
+    k_check_rowptr<<<(unsigned)((n + 1 + 255) / 256), 256, 0, st>>>(d_row_ptr, n, nnz, d_rep);
+    BuildReport rep{};
+    CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (rep.err_mask) return ISING_ERR_BAD_SHAPE;
+    {
+        const long long warps = n;
+        const unsigned blocks = (unsigned)((warps * 32 + 255) / 256);
+        k_validate<<<blocks, 256, 0, st>>>(n, d_row_ptr, d_col, d_w, wtype, d_colour, n_colours, d_rep);
+    }
+    CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    for (int code : {ISING_ERR_BAD_SHAPE, ISING_ERR_UNSORTED_OR_DUP, ISING_ERR_SELF_LOOP, ISING_ERR_ASYMMETRIC,
+                     ISING_ERR_BAD_COLOURING, ISING_ERR_FIELD_OVERFLOW})
+        if (rep.err_mask & (1u << code)) return code;
+
+    // ---- O(n) planning on the host: relabelling and slices
+    std::vector<int64_t> h_row_ptr(n + 1);
+    std::vector<int32_t> h_colour(n, 0);
+    if (rp_dev) CK(cudaMemcpy(h_row_ptr.data(), row_ptr, 8 * (size_t)(n + 1), cudaMemcpyDeviceToHost));
+    else std::memcpy(h_row_ptr.data(), row_ptr, 8 * (size_t)(n + 1));
+    if (colour) {
+        if (co_dev) CK(cudaMemcpy(h_colour.data(), colour, 4 * (size_t)n, cudaMemcpyDeviceToHost));
+        else std::memcpy(h_colour.data(), colour, 4 * (size_t)n);
+    }
+    const int32_t C = n_colours > 0 ? n_colours : 1;
+    std::vector<int32_t> perm(n), inv(n);
+    {
+        // stable counting sorts: by degree descending, then by colour ascending
+        int64_t dmax = 0;
+        for (int32_t i = 0; i < n; ++i) dmax = std::max(dmax, h_row_ptr[i + 1] - h_row_ptr[i]);
+        std::vector<int64_t> cnt((size_t)dmax + 2, 0);
+        for (int32_t i = 0; i < n; ++i) cnt[(size_t)(dmax - (h_row_ptr[i + 1] - h_row_ptr[i])) + 1]++;
+        for (size_t k = 1; k < cnt.size(); ++k) cnt[k] += cnt[k - 1];
+        std::vector<int32_t> by_deg(n);
+        for (int32_t i = 0; i < n; ++i) by_deg[(size_t)cnt[(size_t)(dmax - (h_row_ptr[i + 1] - h_row_ptr[i]))]++] = i;
+        std::vector<int64_t> cc((size_t)C + 1, 0);
+        for (int32_t i = 0; i < n; ++i) cc[(size_t)h_colour[i] + 1]++;
+        for (size_t k = 1; k < cc.size(); ++k) cc[k] += cc[k - 1];
+        for (int32_t k = 0; k < n; ++k) perm[(size_t)cc[(size_t)h_colour[by_deg[k]]]++] = by_deg[k];
+        for (int32_t k = 0; k < n; ++k) inv[perm[k]] = k;
+    }
+    std::vector<SliceDesc> slices;
+    std::vector<uint32_t> phase_begin((size_t)C + 1, 0);
+    uint64_t cells = 0;   // (group, sub-row) cells = 4 edge slots each
+    {
+        int32_t k = 0;
+        for (int32_t c = 0; c < C; ++c) {
+            phase_begin[c] = (uint32_t)slices.size();
+            while (k < n && h_colour[perm[k]] == c) {
+                const int64_t deg = h_row_ptr[perm[k] + 1] - h_row_ptr[perm[k]];
+                const int l = spr_log2_for_degree(deg);
+                const int rps = kSubRows >> l;
+                int nr = 1;
+                while (nr < rps && k + nr < n && h_colour[perm[k + nr]] == c) {
+                    const int64_t d2 = h_row_ptr[perm[k + nr] + 1] - h_row_ptr[perm[k + nr]];
+                    if (spr_log2_for_degree(d2) != l) break;
+                    ++nr;
+                }
+                const int64_t groups = (deg + 3) / 4;
+                const int64_t G = (groups + (1ll << l) - 1) >> l;
+                if (G > 0xffffffffll || cells > 0xffffffffull) return ISING_ERR_BAD_SHAPE;
+                SliceDesc d;
+                d.off = (uint32_t)cells;
+                d.row0 = (uint32_t)k;
+                d.G = (uint32_t)G;
+                d.meta = (uint32_t)l | ((uint32_t)nr << 8);
+                slices.push_back(d);
+                cells += (uint64_t)G * kSubRows;
+                k += nr;
+            }
+        }
+        phase_begin[C] = (uint32_t)slices.size();
+        if (cells > 0xffffffffull) return ISING_ERR_BAD_SHAPE;
+    }
+    const uint64_t slots = cells * 4;
+    const bool wide = rep.max_abs_w > 127 || (uint64_t)rep.absw_max * 2ull >= (1ull << 31);
+    const bool complete = n >= 2 && nnz == (int64_t)n * (n - 1);
+    const bool want_dense = kDenseEnabled && complete && !(flags & ISING_LOAD_NO_DENSE) && rep.max_abs_w <= 127;
+
+    ising_problem* p = new (std::nothrow) ising_problem();
+    if (!p) return ISING_ERR_CUDA;
+    p->n = n; p->nnz = nnz; p->n_colours = n_colours; p->max_replicas = max_replicas;
+    p->tiles_max = (max_replicas + kTile - 1) / kTile;
+    p->W = rep.w_sum / 2; p->absw_max = rep.absw_max; p->wide = wide;
+    p->n_slices = (uint32_t)slices.size(); p->slots = slots;
+    p->phase_begin = phase_begin;
+    p->flush_rows = wide ? 0x7fffffffu
+                         : (uint32_t)std::max<int64_t>(1, ((1ll << 31) - 1) / std::max<int64_t>(1, 2 * rep.absw_max));
+
+    const size_t tiles = (size_t)p->tiles_max;
+    p->perm = (int32_t*)ws.take(4 * (size_t)n);
+    p->inv = (int32_t*)ws.take(4 * (size_t)n);
+    p->slices = (SliceDesc*)ws.take(sizeof(SliceDesc) * std::max<size_t>(1, slices.size()));
+    p->col4 = (int4*)ws.take(16 * std::max<size_t>(1, (size_t)cells));
+    p->w4 = (uint32_t*)ws.take(4 * std::max<size_t>(1, (size_t)cells));
+    if (wide) p->w4w = (int4*)ws.take(16 * std::max<size_t>(1, (size_t)cells));
+    p->state[0] = (uint8_t*)ws.take(tiles * (size_t)n * kTile);
+    p->state[1] = (uint8_t*)ws.take(tiles * (size_t)n * kTile);
+    p->best = (uint8_t*)ws.take(tiles * (size_t)n * kTile);
+    p->io_stage = (int8_t*)ws.take((size_t)max_replicas * (size_t)n);
+    for (int k = 0; k < 2; ++k) {
+        p->sm.accum[k] = (long long*)ws.take(8 * tiles * kTile);
+        p->sm.E[k] = (long long*)ws.take(8 * tiles * kTile);
+        p->sm.bestcut[k] = (long long*)ws.take(8 * tiles * kTile);
+    }
+    p->sm.accum_eval = (long long*)ws.take(8 * tiles * kTile);
+    p->sm.out_tmp = (long long*)ws.take(16 * tiles * kTile);
+    p->sm.best_sweep = (int32_t*)ws.take(4 * tiles * kTile);
+    p->sm.flag = (int*)ws.take(256);
+    void* dense_mem = nullptr;
+    size_t dense_bytes = 0;
+    if (want_dense) {
+        dense_bytes = dense_workspace_bytes(n, max_replicas);
+        dense_mem = ws.take(dense_bytes);
+    }
+    if (ws.overflow) { delete p; return ISING_ERR_WORKSPACE_TOO_SMALL; }
+    p->ws_used = ws.used;
+
+    auto fail = [&](ising_status s) { delete p; return s; };
+#define CKP(call) do { if ((call) != cudaSuccess) { (void)cudaGetLastError(); return fail(ISING_ERR_CUDA); } } while (0)
+    CKP(cudaMemcpyAsync(p->perm, perm.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
+    CKP(cudaMemcpyAsync(p->inv, inv.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
+    if (!slices.empty())
+        CKP(cudaMemcpyAsync(p->slices, slices.data(), sizeof(SliceDesc) * slices.size(), cudaMemcpyHostToDevice, st));
+    if (!slices.empty()) {
+        const unsigned blocks = (unsigned)(((long long)slices.size() * 32 + 255) / 256);
+        k_pack<<<blocks, 256, 0, st>>>(p->slices, (uint32_t)slices.size(), p->perm, p->inv, d_row_ptr, d_col, d_w,
+                                       wtype, p->col4, p->w4, p->w4w);
+    }
+    if (want_dense) {
+        p->dense = dense_create(n, max_replicas, dense_mem, dense_bytes, d_row_ptr, d_col, d_w, wtype, st);
+        if (!p->dense) return fail(ISING_ERR_CUDA);
+    }
+    CKP(cudaStreamSynchronize(st));   // perm / slices host vectors die at return
+    CKP(cudaGetLastError());
+
+    int dev = 0;
+    CKP(cudaGetDevice(&dev));
+    CKP(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    {
+        int o = 1;
+        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindGS, false>, kSweepThreads, 0)); p->ctas_per_sm[0][0] = std::max(1, o);
+        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindJacobi, false>, kSweepThreads, 0)); p->ctas_per_sm[0][1] = std::max(1, o);
+        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindEval, false>, kSweepThreads, 0)); p->ctas_per_sm[0][2] = std::max(1, o);
+        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindGS, true>, kSweepThreads, 0)); p->ctas_per_sm[1][0] = std::max(1, o);
+        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindJacobi, true>, kSweepThreads, 0)); p->ctas_per_sm[1][1] = std::max(1, o);
+        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindEval, true>, kSweepThreads, 0)); p->ctas_per_sm[1][2] = std::max(1, o);
+    }
+#undef CKP
+    *out = p;
+    return ISING_OK;
+}
+
+ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int32_t n_replicas,
+                          int32_t first_replica, uint64_t seed, const uint32_t* thresholds, int32_t n_sweeps,
+                          int32_t sweep_offset, int32_t init_mode, const int8_t* init_spins, int64_t* cut_trace,
+                          void* stream) {
+    if (!p) return ISING_ERR_NULL_ARG;
+    if (mode < 0 || mode > 2 || tie_rule < 0 || tie_rule > 1 || init_mode < 0 || init_mode > 2 || n_sweeps < 0 ||
+        sweep_offset < 0 || first_replica < 0)
+        return ISING_ERR_BAD_SHAPE;
+    if (n_replicas < 1 || n_replicas > p->max_replicas) return ISING_ERR_TOO_MANY_REPLICAS;
+    if (n_sweeps > 0 && !thresholds) return ISING_ERR_NULL_ARG;
+    if (init_mode == ISING_INIT_GIVEN && !init_spins) return ISING_ERR_NULL_ARG;
+    if (mode == ISING_MODE_GS && p->n_colours == 0) return ISING_ERR_NO_COLOURING_FOR_GS;
+    if (init_mode == ISING_INIT_CONTINUE && (!p->have_state || p->last_R != n_replicas)) return ISING_ERR_NO_STATE;
+    if (cut_trace && !is_device_ptr(cut_trace)) return ISING_ERR_BAD_SHAPE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int tiles = (n_replicas + kTile - 1) / kTile;
+    const uint32_t n = (uint32_t)p->n;
+    const unsigned long long tile_stride = (unsigned long long)n * kTile;
+    const PhiloxKeys keys = philox_make_keys(seed);
+    const bool use_dense = p->dense && mode == ISING_MODE_JACOBI;
+
+    // ---- a2: initial state (into the sparse layout; the dense engine imports from it)
+    if (p->state_in_dense && !(use_dense && init_mode == ISING_INIT_CONTINUE)) {
+        // the state of the previous call lives in the dense layout: bring it back first
+        if (init_mode == ISING_INIT_CONTINUE) {
+            if (ising_status s = dense_export_state(p->dense, p->io_stage, n_replicas, /*best=*/false, st)) return s;
+            CK(cudaMemsetAsync(p->sm.flag, 0, sizeof(int), st));
+            k_import<<<dim3((unsigned)(((unsigned long long)n * kTile + 255) / 256), tiles), 256, 0, st>>>(
+                p->state[p->cur], p->io_stage, p->perm, n, tile_stride, n_replicas, p->sm.flag);
+            p->launches++;
+        }
+        p->state_in_dense = false;
+    }
+    if (init_mode == ISING_INIT_PHILOX) {
+        p->cur = 0;
+        k_init_philox<<<dim3((unsigned)((2ull * n + 255) / 256), tiles), 256, 0, st>>>(p->state[0], p->perm, n,
+                                                                                     tile_stride, (uint32_t)first_replica, keys);
+        p->launches++;
+    } else if (init_mode == ISING_INIT_GIVEN) {
+        const int8_t* d_in = init_spins;
+        if (!is_device_ptr(init_spins)) {
+            CK(cudaMemcpyAsync(p->io_stage, init_spins, (size_t)n_replicas * n, cudaMemcpyHostToDevice, st));
+            d_in = p->io_stage;
+        }
+        p->cur = 0;
+        CK(cudaMemsetAsync(p->sm.flag, 0, sizeof(int), st));
+        k_import<<<dim3((unsigned)(((unsigned long long)n * kTile + 255) / 256), tiles), 256, 0, st>>>(
+            p->state[0], d_in, p->perm, n, tile_stride, n_replicas, p->sm.flag);
+        p->launches++;
+        int bad = 0;
+        CK(cudaMemcpyAsync(&bad, p->sm.flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        if (bad) { p->have_state = false; return ISING_ERR_BAD_SPINS; }
+    }
+    p->have_state = true;
+    p->last_R = n_replicas;
+    p->have_best = false;
+    if (n_sweeps == 0) { CK(cudaGetLastError()); return ISING_OK; }
+
+    const size_t small_bytes = 8 * (size_t)tiles * kTile;
+    CK(cudaMemsetAsync(p->sm.accum[0], 0, small_bytes, st));
+    CK(cudaMemsetAsync(p->sm.accum[1], 0, small_bytes, st));
+    CK(cudaMemsetAsync(p->sm.bestcut[0], 0, small_bytes, st));
+    CK(cudaMemsetAsync(p->sm.bestcut[1], 0, small_bytes, st));
+    p->parity = 0;
+
+    if (use_dense) {
+        DenseAnnealArgs a{};
+        a.tie_rule = tie_rule; a.n_replicas = n_replicas; a.first_replica = first_replica; a.keys = keys;
+        a.thresholds = thresholds; a.n_sweeps = n_sweeps; a.sweep_offset = sweep_offset; a.cut_trace = cut_trace;
+        a.W = p->W;
+        a.import_from_sparse = !(p->state_in_dense && init_mode == ISING_INIT_CONTINUE);
+        a.sparse_state = p->state[p->cur]; a.perm = p->perm; a.io_stage = p->io_stage;
+        ising_status s = dense_anneal(p->dense, a, st, &p->launches);
+        if (s) return s;
+        p->state_in_dense = true;
+        p->have_best = true;
+        CK(cudaGetLastError());
+        return ISING_OK;
+    }
+
+    SweepParams sp = base_params(p);
+    sp.rep0 = (uint32_t)first_replica;
+    sp.tie_rule = tie_rule;
+    sp.keys = keys;
+
+    if (mode == ISING_MODE_GS) {
+        // initial energy from the definition (evaluation pass), then incremental dE per phase
+        SweepParams ev = sp;
+        ev.src = p->state[p->cur]; ev.dst = p->state[p->cur]; ev.accum = p->sm.accum[p->parity];
+        launch_sweep(p, kKindEval, ev, tiles, st);
+        launch_sweep_end(p, p->state[p->cur], 2, 0, 0, nullptr, n_replicas, tiles, st);
+        for (int32_t t = 0; t < n_sweeps; ++t) {
+            SweepParams q = sp;
+            q.src = p->state[p->cur]; q.dst = p->state[p->cur];
+            q.accum = p->sm.accum[p->parity];
+            q.thr = thresholds[t]; q.T = (uint32_t)(sweep_offset + t);
+            for (int32_t c = 0; c < p->n_colours; ++c) {
+                q.slice_begin = p->phase_begin[c]; q.slice_end = p->phase_begin[c + 1];
+                launch_sweep(p, kKindGS, q, tiles, st);
+            }
+            launch_sweep_end(p, p->state[p->cur], 0, t == 0, sweep_offset + t,
+                             cut_trace ? (long long*)cut_trace + (size_t)t * n_replicas : nullptr, n_replicas, tiles, st);
+        }
+    } else if (mode == ISING_MODE_JACOBI) {
+        // pass t reads s^t and yields 2E(s^t) as a by-product; pass n_sweeps is evaluation only
+        for (int32_t t = 0; t <= n_sweeps; ++t) {
+            SweepParams q = sp;
+            q.src = p->state[p->cur]; q.dst = p->state[p->cur ^ 1];
+            q.accum = p->sm.accum[p->parity];
+            if (t < n_sweeps) {
+                q.thr = thresholds[t]; q.T = (uint32_t)(sweep_offset + t);
+                launch_sweep(p, kKindJacobi, q, tiles, st);
+            } else {
+                launch_sweep(p, kKindEval, q, tiles, st);
+            }
+            if (t == 0) launch_sweep_end(p, p->state[p->cur], 2, 0, 0, nullptr, n_replicas, tiles, st);
+            else launch_sweep_end(p, p->state[p->cur], 1, t == 1, sweep_offset + t - 1,
+                                  cut_trace ? (long long*)cut_trace + (size_t)(t - 1) * n_replicas : nullptr,
+                                  n_replicas, tiles, st);
+            if (t < n_sweeps) p->cur ^= 1;
+        }
+    } else {
+        // paper-like racy in-place update of all spins (L158), then an evaluation pass for the cut
+        for (int32_t t = 0; t < n_sweeps; ++t) {
+            SweepParams q = sp;
+            q.src = p->state[p->cur]; q.dst = p->state[p->cur];
+            q.accum = p->sm.accum_eval;   // meaningless under races; discarded
+            q.thr = thresholds[t]; q.T = (uint32_t)(sweep_offset + t);
+            launch_sweep(p, kKindGS, q, tiles, st);
+            SweepParams ev = sp;
+            ev.src = p->state[p->cur]; ev.dst = p->state[p->cur]; ev.accum = p->sm.accum[p->parity];
+            launch_sweep(p, kKindEval, ev, tiles, st);
+            launch_sweep_end(p, p->state[p->cur], 1, t == 0, sweep_offset + t,
+                             cut_trace ? (long long*)cut_trace + (size_t)t * n_replicas : nullptr, n_replicas, tiles, st);
+        }
+    }
+    p->have_best = true;
+    CK(cudaGetLastError());
+    return ISING_OK;
+}
+
+ising_status ising_energy_cut(ising_problem* p, const int8_t* spins, int32_t n_replicas, int64_t* energy_out,
+                              int64_t* cut_out, void* stream) {
+    if (!p) return ISING_ERR_NULL_ARG;
+    if (n_replicas < 1 || n_replicas > p->max_replicas) return ISING_ERR_TOO_MANY_REPLICAS;
+    if (!spins && (!p->have_state || n_replicas != p->last_R)) return ISING_ERR_NO_STATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int tiles = (n_replicas + kTile - 1) / kTile;
+    const uint32_t n = (uint32_t)p->n;
+    const unsigned long long tile_stride = (unsigned long long)n * kTile;
+    const uint8_t* eval_state = nullptr;
+    uint8_t* scratch = p->state[p->cur ^ 1];
+    if (spins || p->state_in_dense) {
+        const int8_t* d_in = spins;
+        if (!spins) {
+            if (ising_status s = dense_export_state(p->dense, p->io_stage, n_replicas, false, st)) return s;
+            d_in = p->io_stage;
+        } else if (!is_device_ptr(spins)) {
+            CK(cudaMemcpyAsync(p->io_stage, spins, (size_t)n_replicas * n, cudaMemcpyHostToDevice, st));
+            d_in = p->io_stage;
+        }
+        CK(cudaMemsetAsync(p->sm.flag, 0, sizeof(int), st));
+        k_import<<<dim3((unsigned)(((unsigned long long)n * kTile + 255) / 256), tiles), 256, 0, st>>>(
+            scratch, d_in, p->perm, n, tile_stride, n_replicas, p->sm.flag);
+        p->launches++;
+        int bad = 0;
+        CK(cudaMemcpyAsync(&bad, p->sm.flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        if (bad) return ISING_ERR_BAD_SPINS;
+        eval_state = scratch;
+    } else {
+        eval_state = p->state[p->cur];
+    }
+    CK(cudaMemsetAsync(p->sm.accum_eval, 0, 8 * (size_t)tiles * kTile, st));
+    SweepParams ev = base_params(p);
+    ev.src = eval_state; ev.dst = const_cast<uint8_t*>(eval_state); ev.accum = p->sm.accum_eval;
+    launch_sweep(p, kKindEval, ev, tiles, st);
+    const bool e_host = energy_out && !is_device_ptr(energy_out);
+    const bool c_host = cut_out && !is_device_ptr(cut_out);
+    long long* d_e = energy_out ? (e_host ? p->sm.out_tmp : (long long*)energy_out) : nullptr;
+    long long* d_c = cut_out ? (c_host ? p->sm.out_tmp + (size_t)tiles * kTile : (long long*)cut_out) : nullptr;
+    k_finish_energy<<<(unsigned)((n_replicas + 255) / 256), 256, 0, st>>>(p->sm.accum_eval, p->W, n_replicas, d_e, d_c);
+    p->launches++;
+    if (e_host) CK(cudaMemcpyAsync(energy_out, d_e, 8 * (size_t)n_replicas, cudaMemcpyDeviceToHost, st));
+    if (c_host) CK(cudaMemcpyAsync(cut_out, d_c, 8 * (size_t)n_replicas, cudaMemcpyDeviceToHost, st));
+    if (e_host || c_host) CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    return ISING_OK;
+}
+
+ising_status ising_best_state(ising_problem* p, int32_t replica, int8_t* spins_out, int64_t* cut_out,
+                              int32_t* sweep_out, int32_t* replica_out, void* stream) {
+    if (!p) return ISING_ERR_NULL_ARG;
+    if (!p->have_best) return ISING_ERR_NO_STATE;
+    if (replica < -1 || replica >= p->last_R) return ISING_ERR_BAD_SHAPE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int R = p->last_R;
+    std::vector<long long> bc(R);
+    std::vector<int32_t> bs(R);
+    if (p->state_in_dense) {
+        if (ising_status s = dense_best_arrays(p->dense, bc.data(), bs.data(), R, st)) return s;
+    } else {
+        CK(cudaMemcpyAsync(bc.data(), p->sm.bestcut[p->parity], 8 * (size_t)R, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(bs.data(), p->sm.best_sweep, 4 * (size_t)R, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    int sel = replica;
+    if (sel < 0) {
+        sel = 0;
+        for (int r = 1; r < R; ++r)
+            if (bc[r] > bc[sel]) sel = r;
+    }
+    if (spins_out) {
+        const bool host_out = !is_device_ptr(spins_out);
+        int8_t* d_out = host_out ? p->io_stage : spins_out;
+        if (p->state_in_dense) {
+            if (ising_status s = dense_export_one(p->dense, d_out, sel, /*best=*/true, st)) return s;
+        } else {
+            k_export<<<(unsigned)((p->n + 255) / 256), 256, 0, st>>>(p->best, d_out, p->perm, (uint32_t)p->n,
+                                                                    (unsigned long long)p->n * kTile, R, sel);
+        }
+        p->launches++;
+        if (host_out) CK(cudaMemcpyAsync(spins_out, d_out, (size_t)p->n, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    if (cut_out) *cut_out = bc[sel];
+    if (sweep_out) *sweep_out = bs[sel];
+    if (replica_out) *replica_out = sel;
+    CK(cudaGetLastError());
+    return ISING_OK;
+}
+
+ising_status ising_current_state(ising_problem* p, int8_t* spins_out, int32_t n_replicas, void* stream) {
+    if (!p || !spins_out) return ISING_ERR_NULL_ARG;
+    if (!p->have_state || n_replicas != p->last_R) return ISING_ERR_NO_STATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host_out = !is_device_ptr(spins_out);
+    int8_t* d_out = host_out ? p->io_stage : spins_out;
+    const int tiles = (n_replicas + kTile - 1) / kTile;
+    if (p->state_in_dense) {
+        if (ising_status s = dense_export_state(p->dense, d_out, n_replicas, false, st)) return s;
+    } else {
+        k_export<<<dim3((unsigned)(((unsigned long long)p->n * kTile + 255) / 256), tiles), 256, 0, st>>>(
+            p->state[p->cur], d_out, p->perm, (uint32_t)p->n, (unsigned long long)p->n * kTile, n_replicas, -1);
+    }
+    p->launches++;
+    if (host_out) {
+        CK(cudaMemcpyAsync(spins_out, d_out, (size_t)n_replicas * p->n, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    CK(cudaGetLastError());
+    return ISING_OK;
+}
+
+ising_status ising_problem_info(const ising_problem* p, int32_t what, int64_t* value_out) {
+    if (!p || !value_out) return ISING_ERR_NULL_ARG;
+    switch (what) {
+        case 0: *value_out = p->n; break;
+        case 1: *value_out = p->nnz; break;
+        case 2: *value_out = p->n_colours; break;
+        case 3: *value_out = p->max_replicas; break;
+        case 4: *value_out = p->W; break;
+        case 5: *value_out = p->dense ? 1 : 0; break;
+        case 6: *value_out = p->launches; break;
+        case 7: *value_out = p->absw_max; break;
+        case 8: *value_out = (int64_t)p->ws_used; break;
+        case 9: *value_out = p->n_slices; break;
+        case 10: *value_out = (int64_t)p->slots; break;
+        default: return ISING_ERR_BAD_SHAPE;
+    }
+    return ISING_OK;
+}
+
+ising_status ising_free(ising_problem* p) {
+    if (p) {
+        if (p->dense) dense_destroy(p->dense);
+        delete p;
+    }
+    return ISING_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,43 @@
+"""`-m gpu`: parity at BASELINE.json's full size for the workload bench.py times (config 5:
+1M-spin power-law graph, 32 replicas), in the same launch configuration, on what the oracle can
+compute in bounded time: every replica for the first sweeps, and a subset of replicas for longer.
+Replicas are independent, so any subset is an exact check (SURVEY 8(c) sampling plan)."""
+import numpy as np
+import pytest
+
+import paper_1807_10750_b200 as P
+from paper_1807_10750_b200 import workloads as W
+
+from gpu_util import assert_same, gpu_anneal, oracle_anneal
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def cfg5():
+    return W.config5()
+
+
+def test_config5_full_size_all_replicas_first_sweeps(cfg5):
+    wl = cfg5
+    M = 6
+    g = gpu_anneal(wl, thr=wl.thr[:M], want_best_spins=False)
+    o = oracle_anneal(wl, thr=wl.thr[:M])
+    assert_same(g, o, best_spins=False)
+    # best state of one replica, full vector
+    s, cut, sweep, rep = P.ising_best_state(g["problem"], 17)
+    np.testing.assert_array_equal(s.cpu().numpy(), o["best_spins"][17])
+    # a replica subset straddling the Philox groups, run longer, same problem handle
+    for first in (3,):
+        g2 = gpu_anneal(wl, thr=wl.thr[:40], n_replicas=2, first_replica=first, problem=g["problem"],
+                        want_best_spins=False)
+        o2 = oracle_anneal(wl, thr=wl.thr[:40], n_replicas=2, first_replica=first)
+        assert_same(g2, o2, best_spins=False)
+
+
+def test_config5_energy_cut_of_final_state(cfg5):
+    wl = cfg5
+    p = P.load_workload(wl)
+    trace = P.anneal_workload(p, wl, thr=wl.thr[:3], cut_trace=True)
+    E, cut = P.ising_energy_cut(p, None, wl.n_replicas)     # from the definition, current state
+    np.testing.assert_array_equal(cut.cpu().numpy(), trace.cpu().numpy()[2])

@@ -1,0 +1,294 @@
+"""`-m gpu` parity tests: the CUDA path, called through the C ABI (binding.py), against the CPU
+oracle on the same seeded inputs.  All quantities are integers, so the bar is BIT-EXACT:
+the cut of every replica after every sweep, the final spin vectors, and the best cut / sweep /
+state per replica (SURVEY 8(c) "Whole trajectory")."""
+import ctypes
+
+import numpy as np
+import pytest
+
+import paper_1807_10750_b200 as P
+from paper_1807_10750_b200 import binding
+from paper_1807_10750_b200 import workloads as W
+from oracle import ising_oracle as O
+
+from gpu_util import assert_same, gpu_anneal, oracle_anneal
+
+pytestmark = pytest.mark.gpu
+
+
+def wl_from_csr(n, csr, colour, nc, R, thr, mode="gs", seed=0, name="custom"):
+    row_ptr, col, w = csr
+    return W.Workload(name=name, n=n, row_ptr=row_ptr, col=col, w=w, colour=colour, n_colours=nc, n_replicas=R,
+                      first_replica=0, seed=seed, thr=thr, mode=mode)
+
+
+def er_workload(n, p, gseed, wkind, wdtype, R, M, colouring="index", mode="gs", seed=0, p0=0.1):
+    u, v = W.erdos_renyi_edges(n, p, gseed)
+    wt = W.weights_from_hash(W.hash_pairs(gseed, u, v), wkind)
+    csr = W.csr_from_edges(n, u, v, wt, wdtype)
+    if colouring:
+        colour, nc = W.greedy_colouring(n, csr[0], csr[1], colouring)
+    else:
+        colour, nc = None, 0
+    return wl_from_csr(n, csr, colour, nc, R, W.linear_schedule(p0, 0.0, M), mode=mode, seed=seed)
+
+
+# ---------------------------------------------------------------------------------------------
+# energy / cut reduction (a7) from the definition
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("device_inputs", [False, True])
+def test_energy_cut_matches_oracle(device_inputs):
+    import torch
+    wl = er_workload(1500, 0.02, 11, "pm4", np.int8, 40, 4)
+    p = P.load_workload(wl, max_replicas=40, device_inputs=device_inputs)
+    spins = W.random_spins(5, 40, wl.n)
+    E, cut = P.ising_energy_cut(p, torch.from_numpy(spins).cuda() if device_inputs else spins)
+    oE, ocut = O.energy_cut(wl.n, wl.row_ptr, wl.col, wl.w, spins)
+    np.testing.assert_array_equal(E.cpu().numpy(), oE)
+    np.testing.assert_array_equal(cut.cpu().numpy(), ocut)
+    assert p.w_total == wl.w_total
+    # host output pointers
+    e_h = np.zeros(40, dtype=np.int64)
+    c_h = np.zeros(40, dtype=np.int64)
+    st = binding.lib().ising_energy_cut(p.handle, spins.ctypes.data, 40, e_h.ctypes.data, c_h.ctypes.data, None)
+    assert st == 0
+    np.testing.assert_array_equal(e_h, oE)
+    np.testing.assert_array_equal(c_h, ocut)
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE.json configs 1-3 (and a cut-down 5) : colour-class Gauss-Seidel
+# ---------------------------------------------------------------------------------------------
+def test_config1_full():
+    wl = W.config1()
+    g = gpu_anneal(wl)
+    o = oracle_anneal(wl, n_threads=1)
+    assert_same(g, o)
+    assert g["trace"].shape == (1000, 1)
+
+
+def test_config2_full():
+    wl = W.config2()
+    g = gpu_anneal(wl)
+    o = oracle_anneal(wl)
+    assert_same(g, o)
+
+
+def test_config3_all_replicas_first_sweeps_and_some_replicas_longer():
+    wl = W.config3()
+    g = gpu_anneal(wl, thr=wl.thr[:150])
+    o = oracle_anneal(wl, thr=wl.thr[:150])
+    assert_same(g, o)
+    # replicas straddling Philox groups / tiles, longer run (first_replica offsets, R = 3: ragged tile)
+    for first in (0, 31, 126, 253):
+        g = gpu_anneal(wl, thr=wl.thr[:1500], n_replicas=3, first_replica=first, problem=g["problem"])
+        o = oracle_anneal(wl, thr=wl.thr[:1500], n_replicas=3, first_replica=first)
+        assert_same(g, o)
+
+
+def test_config3_all_plus_torus_reaches_known_max_cut():
+    """Even torus with all weights +1: max cut = #E = 2 L^2 = 20000 (SURVEY 8(c) closed forms)."""
+    wl = W.config3(all_plus=True)
+    p = P.load_workload(wl)
+    P.anneal_workload(p, wl)
+    s, cut, sweep, rep = P.ising_best_state(p, -1)
+    assert cut == 20000
+    E, c = P.ising_energy_cut(p, s.reshape(1, -1))
+    assert int(c[0]) == 20000 and int(E[0]) == wl.w_total - 2 * 20000
+    # the recorded best must be the checkerboard (or its negation)
+    s = s.cpu().numpy()
+    assert np.all(s == s[0] * np.where(wl.colour == wl.colour[0], 1, -1))
+    # first sweeps agree with the oracle for every replica
+    g = gpu_anneal(wl, thr=wl.thr[:40], problem=p)
+    o = oracle_anneal(wl, thr=wl.thr[:40])
+    assert_same(g, o)
+
+
+@pytest.mark.parametrize("colouring", ["ldf", "index"])
+def test_config5_cutdown(colouring):
+    wl = W.config5(n=30000, sweeps=40, replicas=32, colouring=colouring)
+    assert np.diff(wl.row_ptr).max() > 1024     # hub rows: warp-per-row slices
+    g = gpu_anneal(wl)
+    o = oracle_anneal(wl)
+    assert_same(g, o)
+
+
+# ---------------------------------------------------------------------------------------------
+# Jacobi on the sparse path (dense engine disabled), racy mode invariants
+# ---------------------------------------------------------------------------------------------
+def test_jacobi_sparse_path():
+    wl = er_workload(3000, 0.004, 21, "pm4", np.int8, 40, 60, colouring=None, mode="jacobi", seed=3)
+    g = gpu_anneal(wl)
+    o = oracle_anneal(wl)
+    assert_same(g, o)
+    wl = W.config4(n=200, sweeps=30, replicas=37)
+    g = gpu_anneal(wl, flags=P.ISING_LOAD_NO_DENSE)
+    o = oracle_anneal(wl)
+    assert_same(g, o)
+    assert not g["problem"].has_dense_engine
+
+
+def test_jacobi_two_cycle_on_all_plus_bipartite():
+    """Zero-temperature Jacobi from all +1 on a bipartite all-(+1) graph oscillates with cut 0."""
+    wl = W.config3(L=20, sweeps=6, replicas=2, all_plus=True)
+    init = np.ones((2, wl.n), dtype=np.int8)
+    g = gpu_anneal(wl, thr=np.zeros(6, dtype=np.uint32), mode=P.ISING_MODE_JACOBI, init_spins=init)
+    assert np.all(g["trace"] == 0)
+    assert np.all(g["final"] == 1)      # even number of sweeps: back to all +1
+
+
+def test_racy_mode_invariants():
+    wl = W.config2(sweeps=200, replicas=8)
+    p = P.load_workload(wl)
+    trace = P.anneal_workload(p, wl, mode=P.ISING_MODE_RACY, cut_trace=True)
+    final = P.ising_current_state(p, 8).cpu().numpy()
+    assert set(np.unique(final)) <= {-1, 1}
+    E, cut = P.ising_energy_cut(p, final)
+    np.testing.assert_array_equal(cut.cpu().numpy(), trace.cpu().numpy()[-1])
+    for r in range(8):
+        s, c, sw, _ = P.ising_best_state(p, r)
+        _, c2 = P.ising_energy_cut(p, s.reshape(1, -1))
+        assert int(c2[0]) == c == int(trace[:, r].max())
+
+
+# ---------------------------------------------------------------------------------------------
+# semantics: tie rule, replica / sweep split, given init, wide weights, degenerate graphs
+# ---------------------------------------------------------------------------------------------
+def test_tie_rule_keep():
+    wl = W.config3(L=30, sweeps=80, replicas=5, all_plus=True)
+    g = gpu_anneal(wl, tie_rule=1)
+    o = oracle_anneal(wl, tie_rule=1)
+    assert_same(g, o)
+    assert not np.array_equal(g["final"], gpu_anneal(wl, tie_rule=0)["final"])
+
+
+@pytest.mark.parametrize("first", [1, 2, 3, 6, 33])
+def test_first_replica_not_multiple_of_four(first):
+    wl = er_workload(600, 0.03, 31, "pm1", np.int8, 7, 50)
+    g = gpu_anneal(wl, first_replica=first)
+    o = oracle_anneal(wl, first_replica=first)
+    assert_same(g, o)
+
+
+def test_batch_split_and_sweep_split_invariance():
+    wl = er_workload(900, 0.02, 41, "pm4", np.int8, 35, 60)
+    full = gpu_anneal(wl)
+    p = full["problem"]
+    # R batch == R singles with first_replica = r
+    for r in (0, 5, 34):
+        one = gpu_anneal(wl, n_replicas=1, first_replica=r, problem=p)
+        np.testing.assert_array_equal(one["final"][0], full["final"][r])
+        np.testing.assert_array_equal(one["trace"][:, 0], full["trace"][:, r])
+    # 0..M == 0..k then k..M with init continue and sweep_offset
+    k = 23
+    a = gpu_anneal(wl, thr=wl.thr[:k], problem=p)
+    b = gpu_anneal(wl, thr=wl.thr[k:], sweep_offset=k, init_mode=P.ISING_INIT_CONTINUE, problem=p)
+    np.testing.assert_array_equal(np.vstack([a["trace"], b["trace"]]), full["trace"])
+    np.testing.assert_array_equal(b["final"], full["final"])
+    o = oracle_anneal(wl)
+    assert_same(full, o)
+
+
+def test_given_init_host_and_device():
+    import torch
+    wl = er_workload(700, 0.02, 51, "pm4", np.int8, 9, 30)
+    init = W.random_spins(9, 9, wl.n)
+    o = oracle_anneal(wl, init_spins=init)
+    assert_same(gpu_anneal(wl, init_spins=init), o)
+    assert_same(gpu_anneal(wl, init_spins=torch.from_numpy(init).cuda()), o)
+    bad = init.copy()
+    bad[3, 17] = 0
+    with pytest.raises(P.IsingError) as e:
+        gpu_anneal(wl, init_spins=bad)
+    assert e.value.status == 13
+
+
+def test_wide_int32_weights():
+    n = 500
+    u, v = W.erdos_renyi_edges(n, 0.05, 61)
+    h = W.hash_pairs(61, u, v)
+    wt = ((h >> np.uint64(8)) % np.uint64(200001)).astype(np.int64) - 100000     # |w| up to 1e5
+    csr = W.csr_from_edges(n, u, v, wt, np.int32)
+    colour, nc = W.greedy_colouring(n, csr[0], csr[1], "index")
+    wl = wl_from_csr(n, csr, colour, nc, 6, W.linear_schedule(0.2, 0.0, 40), seed=9)
+    assert_same(gpu_anneal(wl), oracle_anneal(wl))
+    wlj = wl_from_csr(n, csr, None, 0, 6, W.linear_schedule(0.2, 0.0, 20), mode="jacobi", seed=9)
+    assert_same(gpu_anneal(wlj), oracle_anneal(wlj))
+
+
+def test_isolated_vertices_and_empty_graph():
+    n = 70
+    u = np.array([0, 3, 3], dtype=np.int64)
+    v = np.array([3, 5, 69], dtype=np.int64)
+    csr = W.csr_from_edges(n, u, v, np.array([2, -3, 1]), np.int8)
+    colour, nc = W.greedy_colouring(n, csr[0], csr[1], "index")
+    wl = wl_from_csr(n, csr, colour, nc, 3, W.linear_schedule(0.3, 0.0, 12), seed=4)
+    assert_same(gpu_anneal(wl), oracle_anneal(wl))
+    empty = (np.zeros(n + 1, dtype=np.int64), np.zeros(0, dtype=np.int32), np.zeros(0, dtype=np.int8))
+    wl = wl_from_csr(n, empty, np.zeros(n, dtype=np.int32), 1, 2, W.linear_schedule(0.3, 0.0, 5), seed=4)
+    g = gpu_anneal(wl)
+    assert_same(g, oracle_anneal(wl))
+    assert np.all(g["trace"] == 0)
+
+
+def test_n_sweeps_zero_only_initialises():
+    wl = er_workload(300, 0.05, 71, "pm1", np.int8, 4, 0)
+    g = gpu_anneal(wl, thr=np.zeros(0, dtype=np.uint32))
+    o = oracle_anneal(wl, thr=np.zeros(0, dtype=np.uint32))
+    np.testing.assert_array_equal(g["final"], o["final"])
+
+
+# ---------------------------------------------------------------------------------------------
+# error behaviour of ising_load_csr / ising_anneal
+# ---------------------------------------------------------------------------------------------
+def _load_status(row_ptr, col, w, colour=None, nc=0, R=1, ws=None):
+    try:
+        P.ising_load_csr(row_ptr, col, w, colour, nc, R, workspace_bytes=ws)
+    except P.IsingError as e:
+        return e.status
+    return 0
+
+
+def test_load_errors():
+    n = 6
+    u = np.array([0, 1, 2], dtype=np.int64)
+    v = np.array([1, 2, 3], dtype=np.int64)
+    rp, col, w = W.csr_from_edges(n, u, v, np.array([1, 2, 3]), np.int8)
+    assert _load_status(rp, col, w) == 0
+    a = w.copy(); a[0] = 5
+    assert _load_status(rp, col, a) == 5                      # asymmetric weight
+    c2 = col.copy(); c2[0] = 0
+    assert _load_status(rp, c2, w) in (4, 5)                  # self loop
+    rp2 = rp.copy(); rp2[2] = rp2[3] + 1
+    assert _load_status(rp2, col, w) == 2                     # row_ptr not monotone
+    c3 = col.copy(); c3[1], c3[2] = c3[2], c3[1]              # row 1 = (0, 2) -> (2, 0)
+    assert _load_status(rp, c3, w) == 3
+    c4 = col.copy(); c4[0] = 99
+    assert _load_status(rp, c4, w) == 2
+    good = np.array([0, 1, 0, 1, 0, 0], dtype=np.int32)
+    assert _load_status(rp, col, w, good, 2) == 0
+    bad = np.array([0, 0, 1, 0, 0, 0], dtype=np.int32)
+    assert _load_status(rp, col, w, bad, 2) == 6              # neighbours share a colour
+    assert _load_status(rp, col, w, good, 1) == 6             # colour out of range
+    assert _load_status(rp, col, w, ws=64) == 9               # workspace too small
+    assert _load_status(rp, col, w, R=0) == 8
+    big = np.full(col.shape, 2**30, dtype=np.int32)
+    assert _load_status(rp, col, big) == 7                    # sum_j |w_ij| >= 2^31
+    p = P.ising_load_csr(rp, col, w)
+    with pytest.raises(P.IsingError) as e:
+        P.ising_anneal(p, np.zeros(3, dtype=np.uint32), mode=P.ISING_MODE_GS)
+    assert e.value.status == 10
+    with pytest.raises(P.IsingError) as e:
+        P.ising_anneal(p, np.zeros(3, dtype=np.uint32), mode=P.ISING_MODE_JACOBI, n_replicas=2)
+    assert e.value.status == 8
+    with pytest.raises(P.IsingError) as e:
+        P.ising_best_state(p, 0)
+    assert e.value.status == 14
+
+
+def test_run_twice_is_bit_identical():
+    wl = W.config5(n=20000, sweeps=25, replicas=32)
+    a = gpu_anneal(wl)
+    b = gpu_anneal(wl, problem=a["problem"])
+    assert_same(a, b)
