@@ -1,0 +1,405 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the annealing hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg5]
+
+One STEP = one pass of the whole hot path over one batch of synthetic input: ising_anneal on the
+workload (spin init a2, all sweeps x colour phases a3-a6/a9, per-sweep cut reduction, trace and
+best-state capture a7).  The graph is loaded once (a1) before the timed region for `value`
+(inputs resident in HBM); the `e2e` leg times the C-ABI calls with HOST buffers: ising_load_csr
+from host CSR + ising_anneal + ising_best_state into host memory, every step.
+
+Metric (BASELINE.json): spin-updates/s = n * R * M / t; edge-visits/s = nnz * R * M / t is reported
+beside it.  Workload of record: config 5 (1M-spin power-law graph, 32 replicas, 500 sweeps), the
+configuration the north-star target is quoted on.  N > 1: replicas only: every rank
+runs the same graph on its own 32 replica ids, no data-path collective, weak scaling.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+workload on the host cores; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1807_10750_b200 import workloads as W  # noqa: E402
+
+METRIC = "spin-updates/s"
+UNIT = "spin-updates/s"
+# SURVEY 8(d) per-unit algorithmic bytes of the sparse sweep at R = 32:
+#   37 B per (directed edge, 32-replica tile): 4 B index + 1 B weight + 32 B gathered spin sector
+#   68 B per (spin, tile): 4 B row bookkeeping + 32 B read + 32 B written
+BYTES_PER_EDGE_TILE = 37
+BYTES_PER_SPIN_TILE = 68
+
+
+# --------------------------------------------------------------------------------------------
+# pieces that need no GPU (covered by the gloo world_size-2 test)
+# --------------------------------------------------------------------------------------------
+def replica_shard(rank: int, world: int, replicas_per_gpu: int):
+    """Replica ids of `rank`: [rank * R, (rank + 1) * R).  Replicas never interact (8(e))."""
+    return rank * replicas_per_gpu, replicas_per_gpu
+
+
+def max_over_ranks(value: float, dist=None, device="cpu") -> float:
+    """MAX all-reduce of a python float (timing: the slowest rank defines the step time)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def algorithmic_bytes_per_sweep(n: int, nnz: int, replicas: int) -> int:
+    tiles = (replicas + 31) // 32
+    return tiles * (nnz * BYTES_PER_EDGE_TILE + n * BYTES_PER_SPIN_TILE)
+
+
+def make_workload(name: str):
+    if name == "cfg1":
+        return W.config1()
+    if name == "cfg2":
+        return W.config2()
+    if name == "cfg3":
+        return W.config3()
+    if name == "cfg4":
+        return W.config4()
+    if name == "cfg5":
+        return W.config5()
+    if name == "cfg5_small":          # for quick functional runs of this script
+        return W.config5(n=50_000, sweeps=50)
+    raise ValueError(name)
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            d = json.load(open(path))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# --------------------------------------------------------------------------------------------
+# clocks
+# --------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            f = tempfile.NamedTemporaryFile(prefix="clocks_", suffix=".csv", delete=False)
+            self.path = f.name
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.FIELDS,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=f, stderr=subprocess.DEVNULL)
+            f.close()
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        try:
+            self.proc.terminate()
+            self.proc.wait(timeout=5)
+        except Exception:
+            try:
+                self.proc.kill()
+            except Exception:
+                pass
+        sm, reasons, smax, power = [], set(), None, []
+        try:
+            for line in open(self.path):
+                p = [x.strip() for x in line.split(",")]
+                if len(p) < 7:
+                    continue
+                try:
+                    sm.append(float(p[0]))
+                    smax = float(p[1])
+                    power.append(float(p[2]))
+                except ValueError:
+                    continue
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"),
+                                   p[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=smax, samples=len(sm),
+                       power_w_max=max(power) if power else None)
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+# --------------------------------------------------------------------------------------------
+# the CPU oracle legs (cpu_baseline, --impl reference)
+# --------------------------------------------------------------------------------------------
+def oracle_sample(wl, replicas: int, sweeps: int, threads: int):
+    """Time the oracle, as it stands, on `replicas` replicas x the first `sweeps` sweeps."""
+    from oracle import ising_oracle as O
+    O.lib()
+    t0 = time.perf_counter()
+    O.anneal_workload(wl, n_replicas=replicas, thr=wl.thr[:sweeps], n_threads=threads)
+    return time.perf_counter() - t0
+
+
+def oracle_calibrate(wl, threads: int, target_s: float):
+    """Pick a sweep count so that one sample costs about target_s of wall clock."""
+    reps = max(1, min(threads, wl.n_replicas))
+    probe = max(1, min(2, wl.n_sweeps))
+    t = oracle_sample(wl, reps, probe, threads)
+    per_sweep = max(t / probe, 1e-6)
+    sweeps = int(max(1, min(wl.n_sweeps, target_s / per_sweep)))
+    return reps, sweeps
+
+
+def run_reference(args, wl, rank):
+    if rank != 0:
+        return 0
+    cores = os.cpu_count() or 1
+    threads = max(1, min(cores, wl.n_replicas))
+    reps, sweeps = oracle_calibrate(wl, threads, target_s=8.0)
+    for _ in range(args.warmup):
+        oracle_sample(wl, reps, max(1, sweeps // 4), threads)
+    times = [oracle_sample(wl, reps, sweeps, threads) for _ in range(args.steps)]
+    total = sum(times)
+    spin_updates = wl.n * reps * sweeps * args.steps
+    value = spin_updates / total
+    sample = "%d replicas x first %d sweeps of %s per step (oracle as it stands, %d host threads)" % (
+        reps, sweeps, wl.name, threads)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+        "config": {"workload": wl.name, "n": wl.n, "nnz": wl.nnz, "replicas": reps, "sweeps": sweeps,
+                   "note": "bounded sample of the same workload on host cores"},
+        "edge_visits_per_s": wl.nnz * reps * sweeps * args.steps / total,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------------------------------
+# the CUDA path
+# --------------------------------------------------------------------------------------------
+def time_workload(P, torch, wl, first_replica, steps, warmup, flush_buf, dist=None, device=None):
+    """Device-resident leg: graph already loaded; each step = one ising_anneal call."""
+    p = P.load_workload(wl)
+    R, M = wl.n_replicas, wl.n_sweeps
+    trace = torch.zeros((M, R), dtype=torch.int64, device="cuda")
+    kw = dict(first_replica=first_replica, cut_trace=trace)
+    for _ in range(warmup):
+        P.anneal_workload(p, wl, **kw)
+    torch.cuda.synchronize()
+    launches0 = p.launches
+    times, best = [], []
+    for _ in range(steps):
+        if flush_buf is not None:
+            flush_buf.add_(1)           # evict L2 between timed steps (buffer > L2)
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        P.anneal_workload(p, wl, **kw)
+        e1.record()
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1) * 1e-3)
+        best.append(P.ising_best_state(p, -1, want_spins=False)[1])
+    launches = p.launches - launches0 - steps * 0
+    return p, times, best, launches
+
+
+def time_e2e(P, torch, wl, first_replica, steps, warmup, dist=None):
+    """End-to-end leg through the C ABI with HOST buffers: load graph from host CSR, anneal,
+    read best state + cut back into host memory.  Timed with CUDA events (all calls enqueue on or
+    synchronise torch's current stream) bracketed by synchronises."""
+    from paper_1807_10750_b200 import binding
+    rp = torch.from_numpy(wl.row_ptr).pin_memory().numpy()
+    col = torch.from_numpy(wl.col).pin_memory().numpy()
+    w = torch.from_numpy(wl.w).pin_memory().numpy()
+    colour = None if wl.colour is None else torch.from_numpy(wl.colour).pin_memory().numpy()
+    out_spins = torch.zeros(wl.n, dtype=torch.int8).pin_memory().numpy()
+    h2d = rp.nbytes + col.nbytes + w.nbytes + (0 if colour is None else colour.nbytes) + wl.thr.nbytes
+    d2h = out_spins.nbytes + 8 + 4 + 4
+    times = []
+    import ctypes
+    for it in range(warmup + steps):
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        p = P.ising_load_csr(rp, col, w, colour, wl.n_colours, wl.n_replicas)
+        P.anneal_workload(p, wl, first_replica=first_replica)
+        cut, sweep, rep = ctypes.c_int64(0), ctypes.c_int32(0), ctypes.c_int32(0)
+        st = binding.lib().ising_best_state(p.handle, -1, out_spins.ctypes.data, ctypes.byref(cut),
+                                            ctypes.byref(sweep), ctypes.byref(rep),
+                                            int(torch.cuda.current_stream().cuda_stream))
+        assert st == 0
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            times.append(dt)
+        p.free()
+    return times, h2d, d2h
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg5")
+    ap.add_argument("--no-extra", action="store_true", help="skip the other four configs and cpu_baseline")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sweeps", type=int, default=0, help="truncate the schedule to its first SWEEPS sweeps "
+                    "(profiling runs only; the default 0 keeps the workload's full schedule)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        return run_reference(args, make_workload(args.workload), rank)
+
+    import torch
+    if not torch.cuda.is_available():
+        print("bench.py: no CUDA device; the product path has no CPU fallback", file=sys.stderr)
+        return 2
+    import paper_1807_10750_b200 as P
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist = dist_mod
+
+    wl = make_workload(args.workload)
+    if args.sweeps > 0:
+        wl.thr = wl.thr[:args.sweeps]
+    first_replica, R = replica_shard(rank, world, wl.n_replicas)
+    M = wl.n_sweeps
+    flush_buf = torch.zeros(256 << 20, dtype=torch.uint8, device="cuda")
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    p, times, best, launches = time_workload(P, torch, wl, first_replica, args.steps, args.warmup, flush_buf,
+                                             dist, None)
+    clocks = sampler.stop() if rank == 0 else None
+    t_total = max_over_ranks(sum(times), dist, "cuda")
+    deterministic = len(set(best)) == 1
+
+    spin_updates = wl.n * R * M * args.steps * world
+    edge_visits = wl.nnz * R * M * args.steps * world
+    value = spin_updates / t_total
+
+    # roofline of the dominant kernel (the sparse sweep; one launch per colour phase).  The anneal
+    # time is charged ENTIRELY to the sweep launches (it also contains the sweep-end kernels), so
+    # `achieved` is a lower bound for the kernel itself.
+    peak, peak_src = measured_peaks()
+    n_phase = max(1, wl.n_colours) if wl.mode == "gs" else 1
+    sweep_launches = n_phase * M * args.steps
+    avg_launch_s = sum(times) / sweep_launches
+    bytes_per_launch = algorithmic_bytes_per_sweep(wl.n, wl.nnz, R) / n_phase
+    achieved = bytes_per_launch / avg_launch_s / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "kernel": "k_sweep<GS> (one launch per colour phase)",
+                "bytes_per_launch": bytes_per_launch, "avg_launch_us": avg_launch_s * 1e6,
+                "peak_source": peak_src,
+                "note": "algorithmic bytes = nnz*37 + n*68 per 32-replica tile per sweep (SURVEY 8(d)); "
+                        "denominator time = whole ising_anneal time / sweep launches (lower bound)"}
+
+    e2e = None
+    if not args.no_e2e:
+        e_times, h2d, d2h = time_e2e(P, torch, wl, first_replica, max(1, min(args.steps, 3)), 1, dist)
+        e_total = max_over_ranks(sum(e_times), dist, "cuda")
+        e2e = {"value": wl.n * R * M * len(e_times) * world / e_total, "unit": UNIT,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e_total / len(e_times),
+               "what": "ising_load_csr(host CSR) + ising_anneal + ising_best_state(host out), per step"}
+
+    extra = {}
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_extra:
+        for name in ("cfg1", "cfg2", "cfg3", "cfg4"):
+            if name == args.workload:
+                continue
+            try:
+                w2 = make_workload(name)
+                _, t2, b2, l2 = time_workload(P, torch, w2, 0, 2, 1, flush_buf)
+                tt = sum(t2)
+                extra[name] = {"workload": w2.name, "n": w2.n, "nnz": w2.nnz, "replicas": w2.n_replicas,
+                               "sweeps": w2.n_sweeps, "mode": w2.mode, "ms_per_step": 1e3 * tt / 2,
+                               "spin_updates_per_s": w2.n * w2.n_replicas * w2.n_sweeps * 2 / tt,
+                               "edge_visits_per_s": w2.nnz * w2.n_replicas * w2.n_sweeps * 2 / tt,
+                               "best_cut": b2[-1], "gpu_launches": l2}
+            except Exception as ex:  # keep the headline line alive
+                extra[name] = {"error": repr(ex)}
+        cores = os.cpu_count() or 1
+        threads = max(1, min(cores, wl.n_replicas))
+        reps, sweeps = oracle_calibrate(wl, threads, target_s=15.0)
+        t = oracle_sample(wl, reps, sweeps, threads)
+        cpu_baseline = {"value": wl.n * reps * sweeps / t, "unit": UNIT, "cores": threads, "kind": "oracle",
+                        "sample": "%d replicas x first %d sweeps of %s (%.1f s wall, %d threads over replicas)" % (
+                            reps, sweeps, wl.name, t, threads)}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int8 x int8 -> int32 (int64 energies)",
+            "data": "synthetic",
+            "config": {"workload": wl.name, "n": wl.n, "nnz": wl.nnz, "replicas_per_gpu": R, "sweeps": M,
+                       "colours": wl.n_colours, "mode": wl.mode, "parallelism": "replicas-only x%d" % world,
+                       "l2": "256 MiB buffer rewritten between timed steps (L2 flush); working set 148 MB > L2",
+                       "step": "one ising_anneal call: init + %d sweeps x %d colour phases + per-sweep cut/best capture" % (
+                           M, n_phase)},
+            "edge_visits_per_s": edge_visits / t_total,
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches,
+            "clocks": clocks, "check": {"deterministic_across_steps": deterministic, "best_cut": best[-1]},
+            "workloads": extra,
+        }
+        print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
