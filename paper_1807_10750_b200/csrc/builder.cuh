@@ -83,47 +83,71 @@ __global__ void k_validate(int32_t n, const long long* row_ptr, const int32_t* c
     }
 }
 
-// One warp per slice: fill col4 / w4 (or w4w).  Cell (g, sr) of the slice holds group
-// q = g * SPR + part of row row0 + (sr >> log_spr), part = sr & (SPR - 1); edges 4q .. 4q+3.
+// One warp per slice: fill the cells of the slice (head cell for group 0, tail cells for the
+// rest) and the per-sub-row caller ids.  Cell (g, sr) holds group q = g * SPR + part of row
+// row0 + (sr >> log_spr), part = sr & (SPR - 1); edges 4q .. 4q+3.
+__device__ __forceinline__ void store_cell(int4* col4, uint32_t* w4, int4* w4w, size_t at, const int (&cc)[4],
+                                           const int (&ww)[4]) {
+    col4[at] = make_int4(cc[0], cc[1], cc[2], cc[3]);
+    if (w4w) w4w[at] = make_int4(ww[0], ww[1], ww[2], ww[3]);
+    else w4[at] = ((uint32_t)ww[0] & 0xffu) | (((uint32_t)ww[1] & 0xffu) << 8) |
+                  (((uint32_t)ww[2] & 0xffu) << 16) | (((uint32_t)ww[3] & 0xffu) << 24);
+}
+
+__device__ __forceinline__ void fetch_group(const int32_t* inv, const int32_t* col, const void* w, int wtype,
+                                            long long b, long long deg, long long q, int (&cc)[4], int (&ww)[4]) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const long long e = 4 * q + j;
+        cc[j] = -1;
+        ww[j] = 0;
+        if (e < deg) {
+            cc[j] = inv[col[b + e]];
+            ww[j] = (int)load_w(w, wtype, b + e);
+        }
+    }
+}
+
 __global__ void k_pack(const SliceDesc* slices, uint32_t n_slices, const int32_t* perm, const int32_t* inv,
                        const long long* row_ptr, const int32_t* col, const void* w, int wtype, int4* col4,
-                       uint32_t* w4, int4* w4w) {
+                       uint32_t* w4, int4* w4w, uint32_t* sorig) {
     const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (gw >= n_slices) return;
     const SliceDesc d = slices[gw];
     const int log_spr = (int)(d.meta & 0xffu), nrows = (int)(d.meta >> 8);
     const uint32_t spr = 1u << log_spr;
+    if (lane < kSubRows) {
+        const uint32_t rloc = (uint32_t)lane >> log_spr;
+        sorig[(size_t)gw * kSubRows + lane] = (int)rloc < nrows ? (uint32_t)perm[d.row0 + rloc] : 0xffffffffu;
+    }
     const unsigned long long cells = (unsigned long long)d.G * kSubRows;
     for (unsigned long long cell = lane; cell < cells; cell += 32) {
         const uint32_t g = (uint32_t)(cell / kSubRows), sr = (uint32_t)(cell % kSubRows);
         const uint32_t rloc = sr >> log_spr, part = sr & (spr - 1);
-        int cc[4];
+        int cc[4] = {-1, -1, -1, -1};
         int ww[4] = {0, 0, 0, 0};
         if ((int)rloc < nrows) {
-            const uint32_t row = d.row0 + rloc;
-            const int32_t orig = perm[row];
+            const int32_t orig = perm[d.row0 + rloc];
             const long long b = row_ptr[orig], deg = row_ptr[orig + 1] - b;
-            const long long q = (long long)g * spr + part;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const long long e = 4 * q + j;
-                if (e < deg) {
-                    cc[j] = inv[col[b + e]];
-                    ww[j] = (int)load_w(w, wtype, b + e);
-                } else {
-                    cc[j] = (int)row;
-                }
-            }
-        } else {
-#pragma unroll
-            for (int j = 0; j < 4; ++j) cc[j] = (int)d.row0;
+            fetch_group(inv, col, w, wtype, b, deg, (long long)g * spr + part, cc, ww);
         }
-        const size_t at = (size_t)d.off + cell;
-        col4[at] = make_int4(cc[0], cc[1], cc[2], cc[3]);
-        if (w4w) w4w[at] = make_int4(ww[0], ww[1], ww[2], ww[3]);
-        else w4[at] = ((uint32_t)ww[0] & 0xffu) | (((uint32_t)ww[1] & 0xffu) << 8) |
-                      (((uint32_t)ww[2] & 0xffu) << 16) | (((uint32_t)ww[3] & 0xffu) << 24);
+        const size_t at = g == 0 ? (size_t)gw * kSubRows + sr : (size_t)d.off + (size_t)(g - 1) * kSubRows + sr;
+        store_cell(col4, w4, w4w, at, cc, ww);
+    }
+}
+
+// One CTA per hub: cell (g, j) holds group q = g * kHubSub + j of the hub's row.
+__global__ void k_pack_hubs(const HubDesc* hubs, uint32_t n_hubs, const int32_t* inv, const long long* row_ptr,
+                            const int32_t* col, const void* w, int wtype, int4* col4, uint32_t* w4, int4* w4w) {
+    if (blockIdx.x >= n_hubs) return;
+    const HubDesc d = hubs[blockIdx.x];
+    const long long b = row_ptr[d.orig], deg = row_ptr[d.orig + 1] - b;
+    const unsigned long long cells = (unsigned long long)d.G * kHubSub;
+    for (unsigned long long cell = threadIdx.x; cell < cells; cell += blockDim.x) {
+        int cc[4], ww[4];
+        fetch_group(inv, col, w, wtype, b, deg, (long long)cell, cc, ww);
+        store_cell(col4, w4, w4w, (size_t)d.off + cell, cc, ww);
     }
 }
 

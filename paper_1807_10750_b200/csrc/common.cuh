@@ -1,19 +1,27 @@
 // Shared declarations of the CUDA path: device-side graph layout and small helpers.
 //
-// Device layout of a loaded graph ("SELL-16 with row splitting"):
+// Device layout of a loaded graph ("SELL-16 with row splitting + CTA hubs"):
 //   * vertices are relabelled by (colour asc, degree desc, caller id asc); `perm` maps the
 //     internal row back to the caller's vertex id (which is what enters the Philox counter);
 //   * a SLICE is the work of one warp: 16 sub-rows x G groups x 4 edges.  A row of
-//     degree d is split into SPR in {1,2,4,8,16} sub-rows (group q of the row goes to
-//     sub-row q % SPR), so a slice holds 16/SPR rows; hub rows (SPR = 16) own a whole
-//     warp and are finished by a warp-level segmented reduction;
-//   * col4[off + g*16 + sr] is an int4 with the four (relabelled) neighbour rows of group g
-//     of sub-row sr, w4[...] the four int8 weights packed in one word (w4w[...]: int4 of
-//     int32 weights for graphs whose weights do not fit int8).  Padding slots carry
-//     weight 0 and point at a valid row, so they contribute nothing;
+//     degree d <= kHubDegree is split into SPR in {1,2,4,8,16} sub-rows (group q of the row goes
+//     to sub-row q % SPR), so a slice holds 16/SPR rows; the sub-rows of one row are
+//     finished by a warp-level segmented (butterfly) reduction;
+//   * a HUB is a row of degree > kHubDegree; it is the work of one whole CTA (kHubSub = 256
+//     sub-rows, group q goes to sub-row q % 256) and is finished through shared memory;
+//   * a CELL is one int4 of four (relabelled) neighbour rows plus one word of four int8
+//     weights (w4w: an int4 of int32 weights for graphs whose weights do not fit int8).
+//     Padding entries carry column -1 (the gather is predicated off) and weight 0.
+//     Cell arrays: group 0 of slice s sits at HEAD cell s*16 + sub-row, so that everything
+//     a warp needs to start a slice (descriptor, first cells, caller ids) is addressed by the
+//     slice index alone and can be prefetched with independent loads, also across the grid
+//     barrier that separates colour phases; groups g >= 1 sit at desc.off + (g-1)*16 + sub-row;
+//     hub cells sit at hub.off + g*256 + sub-row;
 //   * spins are replica-interleaved: state[tile][row][32] int8 (+1/-1), one 32-byte
 //     sector per spin per tile of 32 replicas, so a neighbour gather is one sector and a
-//     thread pair reads it with two 16-byte loads.
+//     thread pair reads it with two 16-byte loads;
+//   * ranges[phase][cta] is the static, cost-balanced split of every colour phase over the
+//     CTAs of the persistent grid.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -25,30 +33,54 @@ namespace ising {
 
 constexpr int kTile = 32;            // replicas per tile == bytes per spin per tile
 constexpr int kSubRows = 16;         // sub-rows per slice (lane pairs per warp)
-constexpr int kWarpsPerCta = 8;
+constexpr int kWarpsPerCta = 16;
 constexpr int kSweepThreads = kWarpsPerCta * 32;
-constexpr int kSubRowEdges = 32;     // a row is split until a sub-row has <= this many edges
+constexpr int kSubRowEdges = 16;     // a row is split until a sub-row has <= this many edges
+constexpr int kHubDegree = kSubRows * kSubRowEdges;    // 256: larger rows are CTA hubs
+constexpr int kHubSub = kWarpsPerCta * kSubRows;       // 256 sub-rows of a hub
+constexpr int kMaxPersistReplicas = 1024;              // replicas per persistent launch
 
 struct SliceDesc {
-    uint32_t off;    // first (group, sub-row) cell of this slice in col4 / w4
+    uint32_t off;    // first tail cell (groups >= 1) of this slice
     uint32_t row0;   // first internal row
-    uint32_t G;      // groups (of 4 edges) per sub-row
+    uint32_t G;      // groups (of 4 edges) per sub-row, >= 1
     uint32_t meta;   // log2(SPR) | (valid rows << 8)
+};
+
+struct HubDesc {
+    uint32_t off;    // first cell
+    uint32_t row;    // internal row
+    uint32_t G;      // groups per sub-row (iterations of the CTA)
+    uint32_t orig;   // caller's vertex id
+};
+
+struct PhaseRange {  // work of one CTA in one colour phase (absolute indices)
+    uint32_t s0, s1; // slices
+    uint32_t h0, h1; // hubs
 };
 
 enum SweepKind : int { kKindGS = 0, kKindJacobi = 1, kKindEval = 2 };
 
-struct SweepParams {
+struct GraphView {
     const int4* col4;
     const uint32_t* w4;
     const int4* w4w;            // wide weights, or nullptr
     const SliceDesc* slices;
-    const int32_t* perm;
+    const uint32_t* sorig;      // [n_slices * 16] caller id of each sub-row's row (0xffffffff: none)
+    const HubDesc* hubs;
+    const PhaseRange* ranges;   // [n_phases][n_cta]
+    uint32_t n_cta;             // CTAs the ranges were built for (== gridDim.x)
+    uint32_t n_phases;
+};
+
+struct SweepParams {
+    GraphView g;
     const uint8_t* src;         // state read
     uint8_t* dst;               // state written (== src for in-place Gauss-Seidel)
     long long* accum;           // [tiles * 32] energy bookkeeping, atomically added
     unsigned long long tile_stride;   // bytes between tiles = n * 32
-    uint32_t slice_begin, slice_end;
+    uint32_t phase_begin, phase_end;  // colour phases processed by this launch
+    uint32_t tiles;
     uint32_t thr;               // flip threshold of this sweep
     uint32_t T;                 // absolute sweep index (Philox counter word 1)
     uint32_t rep0;              // global id of replica 0 of this call
@@ -69,13 +101,17 @@ __device__ __forceinline__ uint32_t ld_stream(const uint32_t* p) {
     asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(r) : "l"(p));
     return r;
 }
-// Spin sectors: coherent loads.  Every phase is its own launch and a colour class is an
-// independent set, so no spin read in a phase is written in the same phase (except a row's
-// own spin, read and written by the same thread).
+// Spin sectors: L2-coherent loads (ld.global.cg).  Inside the persistent kernel a spin
+// written in colour phase c by another SM is read in phase c+1 after the grid barrier, so
+// the (incoherent) L1 must never serve it.
 __device__ __forceinline__ uint4 ld_spin(const uint8_t* p) {
-    return *reinterpret_cast<const uint4*>(p);
+    return __ldcg(reinterpret_cast<const uint4*>(p));
 }
-
-__device__ __forceinline__ uint32_t warp_bcast(uint32_t v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+// Neighbour gather; padding entries (col < 0) are predicated off and read as zero.
+__device__ __forceinline__ uint4 ld_nbr(const uint8_t* base, int c) {
+    uint4 r = make_uint4(0u, 0u, 0u, 0u);
+    if (c >= 0) r = __ldcg(reinterpret_cast<const uint4*>(base + (size_t)(uint32_t)c * kTile));
+    return r;
+}
 
 }  // namespace ising

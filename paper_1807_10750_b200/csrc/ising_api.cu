@@ -59,13 +59,22 @@ inline int spr_log2_for_degree(int64_t deg) {
     return l;
 }
 
-// Upper bounds used by ising_workspace_bytes (any degree distribution).
+constexpr uint32_t kThrCap = 1u << 16;   // thresholds per persistent launch (longer schedules are chunked)
+
+// Upper bounds used by ising_workspace_bytes (any degree distribution; DESIGN.md "Workspace bound").
 inline uint64_t bound_slices(int64_t n, int64_t nnz, int64_t C) {
-    return (uint64_t)n / 16 + 4 * ((uint64_t)nnz / 256) + 6 * (uint64_t)(C + 1) + 8;
+    // full slices of rows with <= 16 edges, full row-split slices (> 128 edges each), one ragged
+    // slice per (colour, SPR)
+    return (uint64_t)n / 16 + (uint64_t)nnz / 128 + 5 * (uint64_t)(C + 1) + 8;
 }
-inline uint64_t bound_slots(int64_t n, int64_t nnz, int64_t C) {
-    return (uint64_t)nnz + 128 * bound_slices(n, nnz, C) + 2048 * (uint64_t)(C + 1);
+inline uint64_t bound_hubs(int64_t nnz) { return (uint64_t)nnz / (kHubDegree + 1) + 1; }
+inline uint64_t bound_cells(int64_t n, int64_t nnz, int64_t C) {
+    // slices: rows are degree-sorted inside a colour, so a slice's cells are covered by the rows of the
+    // slice before it (nnz/4 + rounding n + nnz/8) plus the first slice of every (colour, SPR) group;
+    // hubs: nnz_h/4 + 256 cells of rounding per hub
+    return 320 * (uint64_t)(C + 1) + (uint64_t)n + (uint64_t)nnz / 2 + (uint64_t)nnz / 4 + kHubSub * bound_hubs(nnz) + 64;
 }
+constexpr uint64_t kMaxCtas = 1024;
 
 struct SmallArrays {
     long long* accum[2];
@@ -73,13 +82,17 @@ struct SmallArrays {
     long long* bestcut[2];
     long long* accum_eval;
     long long* out_tmp;    // 2 * max_replicas
+    long long* accum3;     // 3 * kMaxPersistReplicas (persistent kernel)
     int32_t* best_sweep;
+    uint32_t* thr;         // kThrCap
+    unsigned int* barrier;
     int* flag;
 };
 
 size_t workspace_need(int64_t n, int64_t nnz, int wtype, int64_t max_replicas, int64_t C, bool wide,
-                      uint64_t n_slices, uint64_t slots, bool with_raw, bool dense) {
+                      uint64_t n_slices, uint64_t n_hubs, uint64_t cells, bool with_raw, bool dense) {
     const uint64_t tiles = (uint64_t)(max_replicas + kTile - 1) / kTile;
+    const uint64_t phases = (uint64_t)std::max<int64_t>(1, C);
     size_t s = 0;
     auto add = [&](size_t b) { s = align_up(s) + b; };
     add(sizeof(BuildReport));
@@ -91,15 +104,21 @@ size_t workspace_need(int64_t n, int64_t nnz, int wtype, int64_t max_replicas, i
     }
     add(4 * (size_t)n);                       // perm
     add(4 * (size_t)n);                       // inv
-    add(sizeof(SliceDesc) * (size_t)n_slices);
-    add(4 * (size_t)slots);                   // col4
-    add(1 * (size_t)slots);                   // w4
-    if (wide) add(4 * (size_t)slots);         // w4w
+    add(sizeof(SliceDesc) * (size_t)(n_slices + 1));
+    add(4 * 16 * (size_t)(n_slices + 1));     // sorig
+    add(sizeof(HubDesc) * (size_t)(n_hubs + 1));
+    add(sizeof(PhaseRange) * (size_t)(phases * kMaxCtas));
+    add(16 * (size_t)(cells + 1));            // col4
+    add(4 * (size_t)(cells + 1));             // w4
+    if (wide) add(16 * (size_t)(cells + 1));  // w4w
     for (int k = 0; k < 3; ++k) add((size_t)tiles * (size_t)n * kTile);   // state x2, best
     add((size_t)max_replicas * (size_t)n);    // io staging
     for (int k = 0; k < 7; ++k) add(8 * (size_t)tiles * kTile);
     add(16 * (size_t)tiles * kTile);          // out_tmp
+    add(8 * 3 * (size_t)kMaxPersistReplicas); // accum3
     add(4 * (size_t)tiles * kTile);           // best_sweep
+    add(4 * (size_t)kThrCap);                 // thr
+    add(256);                                 // barrier
     add(256);                                 // flag
     if (dense) add(dense_workspace_bytes(n, max_replicas));
     return align_up(s) + kAlign;
@@ -120,6 +139,9 @@ struct ising_problem {
     int32_t* perm = nullptr;
     int32_t* inv = nullptr;
     SliceDesc* slices = nullptr;
+    uint32_t* sorig = nullptr;
+    HubDesc* hubs = nullptr;
+    PhaseRange* ranges = nullptr;
     int4* col4 = nullptr;
     uint32_t* w4 = nullptr;
     int4* w4w = nullptr;
@@ -129,9 +151,8 @@ struct ising_problem {
     SmallArrays sm{};
     DenseEngine* dense = nullptr;
     // host bookkeeping
-    std::vector<uint32_t> phase_begin;   // [n_colours + 1] slice ranges per colour (GS)
-    uint32_t n_slices = 0;
-    uint64_t slots = 0;
+    uint32_t n_slices = 0, n_hubs = 0, n_phases = 1, n_cta = 1;
+    uint64_t cells = 0;
     size_t ws_used = 0;
     int cur = 0;
     int parity = 0;
@@ -141,43 +162,49 @@ struct ising_problem {
     int32_t last_R = 0;
     int64_t launches = 0;
     int sm_count = 148;
-    int ctas_per_sm[2][3] = {{1, 1, 1}, {1, 1, 1}};
+    bool cooperative = false;
     uint32_t flush_rows = 1;
 };
 
 namespace {
 
-template <int KIND>
-void launch_sweep_kind(ising_problem* p, const SweepParams& sp, dim3 grid, cudaStream_t st) {
-    if (p->wide) k_sweep<KIND, true><<<grid, kSweepThreads, 0, st>>>(sp);
-    else k_sweep<KIND, false><<<grid, kSweepThreads, 0, st>>>(sp);
+GraphView graph_view(const ising_problem* p) {
+    GraphView g{};
+    g.col4 = p->col4; g.w4 = p->w4; g.w4w = p->w4w; g.slices = p->slices; g.sorig = p->sorig; g.hubs = p->hubs;
+    g.ranges = p->ranges; g.n_cta = p->n_cta; g.n_phases = p->n_phases;
+    return g;
 }
 
+template <int KIND>
+void launch_sweep_kind(ising_problem* p, const SweepParams& sp, cudaStream_t st) {
+    if (p->wide) k_sweep<KIND, true><<<p->n_cta, kSweepThreads, 0, st>>>(sp);
+    else k_sweep<KIND, false><<<p->n_cta, kSweepThreads, 0, st>>>(sp);
+}
+
+// One pass over colour phases [sp.phase_begin, sp.phase_end) for `tiles` replica tiles, in batches of
+// kMaxPersistReplicas replicas (the kernels keep per-replica bookkeeping in shared memory).
 void launch_sweep(ising_problem* p, int kind, SweepParams sp, int tiles, cudaStream_t st) {
-    const uint32_t nsl = sp.slice_end - sp.slice_begin;
-    if (nsl == 0) return;
-    const int occ = p->ctas_per_sm[p->wide ? 1 : 0][kind];
-    long long cap = ((long long)p->sm_count * occ + tiles - 1) / tiles;
-    if (cap < 1) cap = 1;
-    long long bx = (nsl + kWarpsPerCta - 1) / kWarpsPerCta;
-    if (bx > cap) bx = cap;
-    dim3 grid((unsigned)bx, (unsigned)tiles, 1);
-    if (kind == kKindGS) launch_sweep_kind<kKindGS>(p, sp, grid, st);
-    else if (kind == kKindJacobi) launch_sweep_kind<kKindJacobi>(p, sp, grid, st);
-    else launch_sweep_kind<kKindEval>(p, sp, grid, st);
-    p->launches++;
+    constexpr int kBatchTiles = kMaxPersistReplicas / kTile;
+    for (int t0 = 0; t0 < tiles; t0 += kBatchTiles) {
+        SweepParams q = sp;
+        q.tiles = (uint32_t)std::min(kBatchTiles, tiles - t0);
+        q.src = sp.src + (size_t)t0 * sp.tile_stride;
+        q.dst = sp.dst + (size_t)t0 * sp.tile_stride;
+        q.accum = sp.accum + (size_t)t0 * kTile;
+        q.rep0 = sp.rep0 + (uint32_t)t0 * kTile;
+        if (kind == kKindGS) launch_sweep_kind<kKindGS>(p, q, st);
+        else if (kind == kKindJacobi) launch_sweep_kind<kKindJacobi>(p, q, st);
+        else launch_sweep_kind<kKindEval>(p, q, st);
+        p->launches++;
+    }
 }
 
 SweepParams base_params(const ising_problem* p) {
     SweepParams sp{};
-    sp.col4 = p->col4;
-    sp.w4 = p->w4;
-    sp.w4w = p->w4w;
-    sp.slices = p->slices;
-    sp.perm = p->perm;
+    sp.g = graph_view(p);
     sp.tile_stride = (unsigned long long)p->n * kTile;
-    sp.slice_begin = 0;
-    sp.slice_end = p->n_slices;
+    sp.phase_begin = 0;
+    sp.phase_end = p->n_phases;
     sp.flush_rows = p->flush_rows;
     return sp;
 }
@@ -257,7 +284,8 @@ ising_status ising_workspace_bytes(int32_t n, int64_t nnz, int32_t wtype, int32_
     if (max_replicas < 1 || max_replicas > 65536) return ISING_ERR_TOO_MANY_REPLICAS;
     const bool dense = kDenseEnabled && nnz == (int64_t)n * (n - 1) && n >= 2;
     *bytes_out = workspace_need(n, nnz, wtype, max_replicas, n_colours, wtype == ISING_W_INT32,
-                                bound_slices(n, nnz, n_colours), bound_slots(n, nnz, n_colours), true, dense);
+                                bound_slices(n, nnz, n_colours), bound_hubs(nnz), bound_cells(n, nnz, n_colours), true,
+                                dense);
     return ISING_OK;
 }
 
@@ -356,40 +384,119 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         for (int32_t k = 0; k < n; ++k) perm[(size_t)cc[(size_t)h_colour[by_deg[k]]]++] = by_deg[k];
         for (int32_t k = 0; k < n; ++k) inv[perm[k]] = k;
     }
+    // ---- work units: hubs (rows above kHubDegree, one CTA each) and slices (one warp each)
+    int sm_count = 148, coop = 0;
+    {
+        int dev = 0;
+        CK(cudaGetDevice(&dev));
+        CK(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
+        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    }
     std::vector<SliceDesc> slices;
-    std::vector<uint32_t> phase_begin((size_t)C + 1, 0);
-    uint64_t cells = 0;   // (group, sub-row) cells = 4 edge slots each
+    std::vector<HubDesc> hubs_sorted;                           // per phase, degree descending
+    std::vector<uint32_t> slice_begin((size_t)C + 1, 0), hub_begin((size_t)C + 1, 0);
+    uint64_t tail_cells = 0, hub_cells = 0;
+    auto degree_of = [&](int32_t k) { return h_row_ptr[perm[k] + 1] - h_row_ptr[perm[k]]; };
     {
         int32_t k = 0;
         for (int32_t c = 0; c < C; ++c) {
-            phase_begin[c] = (uint32_t)slices.size();
+            slice_begin[c] = (uint32_t)slices.size();
+            hub_begin[c] = (uint32_t)hubs_sorted.size();
             while (k < n && h_colour[perm[k]] == c) {
-                const int64_t deg = h_row_ptr[perm[k] + 1] - h_row_ptr[perm[k]];
+                const int64_t deg = degree_of(k);
+                if (deg > kHubDegree) {
+                    HubDesc h;
+                    h.off = 0;
+                    h.row = (uint32_t)k;
+                    h.G = (uint32_t)(((deg + 3) / 4 + kHubSub - 1) / kHubSub);
+                    h.orig = (uint32_t)perm[k];
+                    hubs_sorted.push_back(h);
+                    hub_cells += (uint64_t)h.G * kHubSub;
+                    ++k;
+                    continue;
+                }
                 const int l = spr_log2_for_degree(deg);
                 const int rps = kSubRows >> l;
                 int nr = 1;
-                while (nr < rps && k + nr < n && h_colour[perm[k + nr]] == c) {
-                    const int64_t d2 = h_row_ptr[perm[k + nr] + 1] - h_row_ptr[perm[k + nr]];
-                    if (spr_log2_for_degree(d2) != l) break;
+                while (nr < rps && k + nr < n && h_colour[perm[k + nr]] == c && spr_log2_for_degree(degree_of(k + nr)) == l)
                     ++nr;
-                }
                 const int64_t groups = (deg + 3) / 4;
-                const int64_t G = (groups + (1ll << l) - 1) >> l;
-                if (G > 0xffffffffll || cells > 0xffffffffull) return ISING_ERR_BAD_SHAPE;
+                const int64_t G = std::max<int64_t>(1, (groups + (1ll << l) - 1) >> l);
                 SliceDesc d;
-                d.off = (uint32_t)cells;
+                d.off = 0;
                 d.row0 = (uint32_t)k;
                 d.G = (uint32_t)G;
                 d.meta = (uint32_t)l | ((uint32_t)nr << 8);
                 slices.push_back(d);
-                cells += (uint64_t)G * kSubRows;
+                tail_cells += (uint64_t)(G - 1) * kSubRows;
                 k += nr;
             }
         }
-        phase_begin[C] = (uint32_t)slices.size();
-        if (cells > 0xffffffffull) return ISING_ERR_BAD_SHAPE;
+        slice_begin[C] = (uint32_t)slices.size();
+        hub_begin[C] = (uint32_t)hubs_sorted.size();
     }
-    const uint64_t slots = cells * 4;
+    const uint64_t head_cells = (uint64_t)slices.size() * kSubRows;
+    const uint64_t cells = head_cells + tail_cells + hub_cells;
+    if (cells > 0xffffffffull) return ISING_ERR_BAD_SHAPE;
+    {
+        uint64_t at = head_cells;
+        for (SliceDesc& d : slices) { d.off = (uint32_t)at; at += (uint64_t)(d.G - 1) * kSubRows; }
+    }
+
+    // ---- static split of every colour phase over the CTAs of the persistent grid.  Cost unit: one
+    // CTA-wide step (16 warps x one group of gathers); a hub costs G + 3 steps, a slice (G + 2) / 16.
+    uint32_t n_cta = 1;
+    for (int32_t c = 0; c < C; ++c)
+        n_cta = std::max(n_cta, (slice_begin[c + 1] - slice_begin[c]) + (hub_begin[c + 1] - hub_begin[c]));
+    n_cta = std::min<uint32_t>(n_cta, (uint32_t)std::min<int>(sm_count, (int)kMaxCtas));
+    std::vector<PhaseRange> ranges((size_t)C * n_cta);
+    std::vector<HubDesc> hubs;
+    hubs.reserve(hubs_sorted.size());
+    {
+        std::vector<double> load(n_cta);
+        uint64_t at = head_cells + tail_cells;
+        for (int32_t c = 0; c < C; ++c) {
+            const uint32_t hb = hub_begin[c], hn = hub_begin[c + 1] - hb;
+            double total = 0;
+            for (uint32_t b = 0; b < n_cta; ++b) {
+                PhaseRange& r = ranges[(size_t)c * n_cta + b];
+                r.h0 = (uint32_t)hubs.size();
+                load[b] = 0;
+                for (uint32_t q = b; q < hn; q += n_cta) {   // round robin over degree-sorted hubs
+                    HubDesc h = hubs_sorted[hb + q];
+                    h.off = (uint32_t)at;
+                    at += (uint64_t)h.G * kHubSub;
+                    load[b] += (double)h.G + 3.0;
+                    hubs.push_back(h);
+                }
+                r.h1 = (uint32_t)hubs.size();
+                total += load[b];
+            }
+            for (uint32_t q = slice_begin[c]; q < slice_begin[c + 1]; ++q) total += ((double)slices[q].G + 2.0) / kWarpsPerCta;
+            uint32_t pos = slice_begin[c];
+            const uint32_t end = slice_begin[c + 1];
+            double remaining = total;
+            for (uint32_t b = 0; b < n_cta; ++b) {
+                PhaseRange& r = ranges[(size_t)c * n_cta + b];
+                const double target = remaining / (double)(n_cta - b);
+                double mine = load[b];
+                r.s0 = pos;
+                if (b + 1 == n_cta) {
+                    while (pos < end) mine += ((double)slices[pos++].G + 2.0) / kWarpsPerCta;
+                } else {
+                    while (pos < end) {
+                        const double cs = ((double)slices[pos].G + 2.0) / kWarpsPerCta;
+                        if (mine + 0.5 * cs > target) break;
+                        mine += cs;
+                        ++pos;
+                    }
+                }
+                r.s1 = pos;
+                remaining -= mine;
+            }
+        }
+    }
+
     const bool wide = rep.max_abs_w > 127 || (uint64_t)rep.absw_max * 2ull >= (1ull << 31);
     const bool complete = n >= 2 && nnz == (int64_t)n * (n - 1);
     const bool want_dense = kDenseEnabled && complete && !(flags & ISING_LOAD_NO_DENSE) && rep.max_abs_w <= 127;
@@ -399,18 +506,21 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     p->n = n; p->nnz = nnz; p->n_colours = n_colours; p->max_replicas = max_replicas;
     p->tiles_max = (max_replicas + kTile - 1) / kTile;
     p->W = rep.w_sum / 2; p->absw_max = rep.absw_max; p->wide = wide;
-    p->n_slices = (uint32_t)slices.size(); p->slots = slots;
-    p->phase_begin = phase_begin;
+    p->n_slices = (uint32_t)slices.size(); p->n_hubs = (uint32_t)hubs.size(); p->cells = cells;
+    p->n_phases = (uint32_t)C; p->n_cta = n_cta; p->sm_count = sm_count; p->cooperative = coop != 0;
     p->flush_rows = wide ? 0x7fffffffu
                          : (uint32_t)std::max<int64_t>(1, ((1ll << 31) - 1) / std::max<int64_t>(1, 2 * rep.absw_max));
 
     const size_t tiles = (size_t)p->tiles_max;
     p->perm = (int32_t*)ws.take(4 * (size_t)n);
     p->inv = (int32_t*)ws.take(4 * (size_t)n);
-    p->slices = (SliceDesc*)ws.take(sizeof(SliceDesc) * std::max<size_t>(1, slices.size()));
-    p->col4 = (int4*)ws.take(16 * std::max<size_t>(1, (size_t)cells));
-    p->w4 = (uint32_t*)ws.take(4 * std::max<size_t>(1, (size_t)cells));
-    if (wide) p->w4w = (int4*)ws.take(16 * std::max<size_t>(1, (size_t)cells));
+    p->slices = (SliceDesc*)ws.take(sizeof(SliceDesc) * (slices.size() + 1));
+    p->sorig = (uint32_t*)ws.take(4 * kSubRows * (slices.size() + 1));
+    p->hubs = (HubDesc*)ws.take(sizeof(HubDesc) * (hubs.size() + 1));
+    p->ranges = (PhaseRange*)ws.take(sizeof(PhaseRange) * ranges.size());
+    p->col4 = (int4*)ws.take(16 * ((size_t)cells + 1));
+    p->w4 = (uint32_t*)ws.take(4 * ((size_t)cells + 1));
+    if (wide) p->w4w = (int4*)ws.take(16 * ((size_t)cells + 1));
     p->state[0] = (uint8_t*)ws.take(tiles * (size_t)n * kTile);
     p->state[1] = (uint8_t*)ws.take(tiles * (size_t)n * kTile);
     p->best = (uint8_t*)ws.take(tiles * (size_t)n * kTile);
@@ -422,7 +532,10 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     }
     p->sm.accum_eval = (long long*)ws.take(8 * tiles * kTile);
     p->sm.out_tmp = (long long*)ws.take(16 * tiles * kTile);
+    p->sm.accum3 = (long long*)ws.take(8 * 3 * (size_t)kMaxPersistReplicas);
     p->sm.best_sweep = (int32_t*)ws.take(4 * tiles * kTile);
+    p->sm.thr = (uint32_t*)ws.take(4 * (size_t)kThrCap);
+    p->sm.barrier = (unsigned int*)ws.take(256);
     p->sm.flag = (int*)ws.take(256);
     void* dense_mem = nullptr;
     size_t dense_bytes = 0;
@@ -437,32 +550,24 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
 #define CKP(call) do { if ((call) != cudaSuccess) { (void)cudaGetLastError(); return fail(ISING_ERR_CUDA); } } while (0)
     CKP(cudaMemcpyAsync(p->perm, perm.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
     CKP(cudaMemcpyAsync(p->inv, inv.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
-    if (!slices.empty())
-        CKP(cudaMemcpyAsync(p->slices, slices.data(), sizeof(SliceDesc) * slices.size(), cudaMemcpyHostToDevice, st));
+    CKP(cudaMemcpyAsync(p->ranges, ranges.data(), sizeof(PhaseRange) * ranges.size(), cudaMemcpyHostToDevice, st));
     if (!slices.empty()) {
+        CKP(cudaMemcpyAsync(p->slices, slices.data(), sizeof(SliceDesc) * slices.size(), cudaMemcpyHostToDevice, st));
         const unsigned blocks = (unsigned)(((long long)slices.size() * 32 + 255) / 256);
         k_pack<<<blocks, 256, 0, st>>>(p->slices, (uint32_t)slices.size(), p->perm, p->inv, d_row_ptr, d_col, d_w,
-                                       wtype, p->col4, p->w4, p->w4w);
+                                       wtype, p->col4, p->w4, p->w4w, p->sorig);
+    }
+    if (!hubs.empty()) {
+        CKP(cudaMemcpyAsync(p->hubs, hubs.data(), sizeof(HubDesc) * hubs.size(), cudaMemcpyHostToDevice, st));
+        k_pack_hubs<<<(unsigned)hubs.size(), 256, 0, st>>>(p->hubs, (uint32_t)hubs.size(), p->inv, d_row_ptr, d_col,
+                                                          d_w, wtype, p->col4, p->w4, p->w4w);
     }
     if (want_dense) {
         p->dense = dense_create(n, max_replicas, dense_mem, dense_bytes, d_row_ptr, d_col, d_w, wtype, st);
         if (!p->dense) return fail(ISING_ERR_CUDA);
     }
-    CKP(cudaStreamSynchronize(st));   // perm / slices host vectors die at return
+    CKP(cudaStreamSynchronize(st));   // the host vectors die at return
     CKP(cudaGetLastError());
-
-    int dev = 0;
-    CKP(cudaGetDevice(&dev));
-    CKP(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev));
-    {
-        int o = 1;
-        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindGS, false>, kSweepThreads, 0)); p->ctas_per_sm[0][0] = std::max(1, o);
-        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindJacobi, false>, kSweepThreads, 0)); p->ctas_per_sm[0][1] = std::max(1, o);
-        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindEval, false>, kSweepThreads, 0)); p->ctas_per_sm[0][2] = std::max(1, o);
-        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindGS, true>, kSweepThreads, 0)); p->ctas_per_sm[1][0] = std::max(1, o);
-        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindJacobi, true>, kSweepThreads, 0)); p->ctas_per_sm[1][1] = std::max(1, o);
-        CKP(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_sweep<kKindEval, true>, kSweepThreads, 0)); p->ctas_per_sm[1][2] = std::max(1, o);
-    }
 #undef CKP
     *out = p;
     return ISING_OK;
@@ -554,8 +659,57 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
     sp.tie_rule = tie_rule;
     sp.keys = keys;
 
-    if (mode == ISING_MODE_GS) {
-        // initial energy from the definition (evaluation pass), then incremental dE per phase
+    if (mode == ISING_MODE_GS && !p->wide && p->cooperative) {
+        // the hot path: initial energy from the definition (evaluation pass), then ONE persistent
+        // cooperative launch per batch of <= 1024 replicas and chunk of <= kThrCap sweeps
+        CK(cudaMemsetAsync(p->sm.accum_eval, 0, small_bytes, st));
+        SweepParams ev = sp;
+        ev.src = p->state[p->cur]; ev.dst = p->state[p->cur]; ev.accum = p->sm.accum_eval;
+        launch_sweep(p, kKindEval, ev, tiles, st);
+        k_finish_energy<<<(unsigned)((tiles * kTile + 255) / 256), 256, 0, st>>>(p->sm.accum_eval, p->W, tiles * kTile,
+                                                                              p->sm.E[0], nullptr);
+        p->launches++;
+        constexpr int kBatchTiles = kMaxPersistReplicas / kTile;
+        for (int t0 = 0; t0 < tiles; t0 += kBatchTiles) {
+            const int bt = std::min(kBatchTiles, tiles - t0);
+            for (int32_t s0 = 0; s0 < n_sweeps; s0 += (int32_t)kThrCap) {
+                const int32_t ns = std::min<int32_t>((int32_t)kThrCap, n_sweeps - s0);
+                CK(cudaMemcpyAsync(p->sm.thr, thresholds + s0, 4 * (size_t)ns, cudaMemcpyHostToDevice, st));
+                CK(cudaMemsetAsync(p->sm.accum3, 0, 8 * 3 * (size_t)kMaxPersistReplicas, st));
+                CK(cudaMemsetAsync(p->sm.barrier, 0, 256, st));
+                AnnealParams a{};
+                a.g = graph_view(p);
+                a.state = p->state[p->cur] + (size_t)t0 * tile_stride;
+                a.best = p->best + (size_t)t0 * tile_stride;
+                a.tile_stride = tile_stride;
+                a.n = n;
+                a.tiles = (uint32_t)bt;
+                a.n_replicas = (uint32_t)std::min(bt * kTile, n_replicas - t0 * kTile);
+                a.rep0 = (uint32_t)first_replica + (uint32_t)t0 * kTile;
+                a.tie_rule = tie_rule;
+                a.flush_rows = p->flush_rows;
+                a.n_sweeps = (uint32_t)ns;
+                a.sweep_offset = (uint32_t)(sweep_offset + s0);
+                a.thr = p->sm.thr;
+                a.W = p->W;
+                a.E0 = p->sm.E[0] + (size_t)t0 * kTile;
+                a.accum = p->sm.accum3;
+                a.trace = cut_trace ? (long long*)cut_trace + (size_t)s0 * n_replicas + (size_t)t0 * kTile : nullptr;
+                a.trace_stride = (unsigned long long)n_replicas;
+                a.E_out = p->sm.E[0] + (size_t)t0 * kTile;
+                a.best_out = p->sm.bestcut[0] + (size_t)t0 * kTile;
+                a.best_sweep_out = p->sm.best_sweep + (size_t)t0 * kTile;
+                a.barrier = p->sm.barrier;
+                a.resume = s0 > 0 ? 1 : 0;
+                a.keys = keys;
+                void* args[] = {&a};
+                CK(cudaLaunchCooperativeKernel((const void*)k_anneal_gs, dim3(p->n_cta), dim3(kSweepThreads), args, 0, st));
+                p->launches++;
+            }
+        }
+        p->parity = 0;
+    } else if (mode == ISING_MODE_GS) {
+        // wide (int32) weights: one launch per colour phase; incremental dE per phase
         SweepParams ev = sp;
         ev.src = p->state[p->cur]; ev.dst = p->state[p->cur]; ev.accum = p->sm.accum[p->parity];
         launch_sweep(p, kKindEval, ev, tiles, st);
@@ -566,7 +720,7 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
             q.accum = p->sm.accum[p->parity];
             q.thr = thresholds[t]; q.T = (uint32_t)(sweep_offset + t);
             for (int32_t c = 0; c < p->n_colours; ++c) {
-                q.slice_begin = p->phase_begin[c]; q.slice_end = p->phase_begin[c + 1];
+                q.phase_begin = (uint32_t)c; q.phase_end = (uint32_t)c + 1;
                 launch_sweep(p, kKindGS, q, tiles, st);
             }
             launch_sweep_end(p, p->state[p->cur], 0, t == 0, sweep_offset + t,
@@ -736,7 +890,9 @@ ising_status ising_problem_info(const ising_problem* p, int32_t what, int64_t* v
         case 7: *value_out = p->absw_max; break;
         case 8: *value_out = (int64_t)p->ws_used; break;
         case 9: *value_out = p->n_slices; break;
-        case 10: *value_out = (int64_t)p->slots; break;
+        case 10: *value_out = (int64_t)p->cells * 4; break;
+        case 11: *value_out = p->n_hubs; break;
+        case 12: *value_out = p->n_cta; break;
         default: return ISING_ERR_BAD_SHAPE;
     }
     return ISING_OK;

@@ -1,15 +1,24 @@
-// Sparse annealing sweep (SURVEY 8(a) a3-a7) and its bookkeeping kernels.
+// Sparse annealing sweep (SURVEY 8(a) a3-a7, a9) and its bookkeeping kernels.
 //
 // One warp owns one slice (common.cuh): lane = 2*sub_row + half, every lane keeps the
 // int32 local fields h_i = sum_j w_ij s_j (eq. (2)) of 16 replicas.  Four
-// neighbour sectors are gathered per step (16-byte loads), byte-transposed with PRMT so
+// neighbour sectors are gathered per step (16-byte L2 loads), byte-transposed with PRMT so
 // that one dp4a multiplies the four edge weights into one replica's field.  Rows split
-// over several sub-rows are finished by a warp-level segmented (butterfly) reduction.
+// over several sub-rows are finished by a warp-level segmented (butterfly) reduction; hub
+// rows are spread over the whole CTA and finished through shared memory.
 // The epilogue takes the energy-minimising value (L47-49 with the sign reading Q1:
 // s_i <- +1 if h_i < 0 else -1), applies the scheduled flip of Algorithm 2 (L177) with the
 // stateless Philox word, writes the spin sector and accumulates the energy bookkeeping
 // (a7): Gauss-Seidel  dE_i = (a_i - s_i) h_i  (exact because a colour class is an
 // independent set), Jacobi / evaluation  s_i h_i  (sum_i s_i h_i = 2 E).
+//
+// Two drivers share these passes:
+//   k_sweep      one launch = colour phases [phase_begin, phase_end) of one sweep (Jacobi,
+//                evaluation, racy mode, wide weights);
+//   k_anneal_gs  the persistent cooperative kernel of the Gauss-Seidel hot path: all sweeps x
+//                colour phases of one ising_anneal call in ONE launch, a grid barrier between
+//                phases, static graph data of the next phase prefetched across the barrier,
+//                the cut reduction, trace and best-state capture fused in (a7, a9).
 #pragma once
 #include "common.cuh"
 
@@ -46,16 +55,50 @@ __device__ __forceinline__ void field_word_wide(int (&h)[16], int k, uint32_t e,
     for (int b = 0; b < 4; ++b) h[4 * k + b] += sbyte(e, b) * w;
 }
 
-__device__ __forceinline__ uint32_t pick8(const uint4& u, const uint4& v, int idx) {
-    uint32_t r = u.x;
-    r = idx == 1 ? u.y : r;
-    r = idx == 2 ? u.z : r;
-    r = idx == 3 ? u.w : r;
-    r = idx == 4 ? v.x : r;
-    r = idx == 5 ? v.y : r;
-    r = idx == 6 ? v.z : r;
-    r = idx == 7 ? v.w : r;
-    return r;
+__device__ __forceinline__ void field_cell(int (&h)[16], const uint4& e0, const uint4& e1, const uint4& e2,
+                                           const uint4& e3, uint32_t w) {
+    field_word(h, 0, e0.x, e1.x, e2.x, e3.x, w);
+    field_word(h, 1, e0.y, e1.y, e2.y, e3.y, w);
+    field_word(h, 2, e0.z, e1.z, e2.z, e3.z, w);
+    field_word(h, 3, e0.w, e1.w, e2.w, e3.w, w);
+}
+
+__device__ __forceinline__ void field_cell_wide(int (&h)[16], const uint4& e0, const uint4& e1, const uint4& e2,
+                                                const uint4& e3, const int4& w) {
+    field_word_wide(h, 0, e0.x, w.x); field_word_wide(h, 1, e0.y, w.x);
+    field_word_wide(h, 2, e0.z, w.x); field_word_wide(h, 3, e0.w, w.x);
+    field_word_wide(h, 0, e1.x, w.y); field_word_wide(h, 1, e1.y, w.y);
+    field_word_wide(h, 2, e1.z, w.y); field_word_wide(h, 3, e1.w, w.y);
+    field_word_wide(h, 0, e2.x, w.z); field_word_wide(h, 1, e2.y, w.z);
+    field_word_wide(h, 2, e2.z, w.z); field_word_wide(h, 3, e2.w, w.z);
+    field_word_wide(h, 0, e3.x, w.w); field_word_wide(h, 1, e3.y, w.w);
+    field_word_wide(h, 2, e3.z, w.w); field_word_wide(h, 3, e3.w, w.w);
+}
+
+__device__ __forceinline__ uint32_t nibble_to_bytemask(uint32_t nib) {
+    // bit b of nib -> byte b = 0xff
+    uint32_t m = (nib & 1u) | ((nib & 2u) << 7) | ((nib & 4u) << 14) | ((nib & 8u) << 21);
+    return m * 0xffu;
+}
+
+__device__ __forceinline__ uint32_t lt4(const uint4& u, uint32_t thr) {
+    return (u.x < thr ? 1u : 0u) | (u.y < thr ? 2u : 0u) | (u.z < thr ? 4u : 0u) | (u.w < thr ? 8u : 0u);
+}
+
+// Flip decisions of Algorithm 2 (L177) for the 16 replicas rep_lane0 .. rep_lane0+15 of spin
+// `orig` in sweep T: bit j set <=> philox(seed; ctr=(orig, T, r>>2, FLIP))[r&3] < thr, r = rep_lane0 + j.
+__device__ __forceinline__ uint32_t flip_mask16(uint32_t orig, uint32_t T, uint32_t rep_lane0, uint32_t thr,
+                                                const PhiloxKeys& keys) {
+    if (thr == 0) return 0u;
+    const uint32_t cw = rep_lane0 >> 2, mis = rep_lane0 & 3u;
+    uint32_t m = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) m |= lt4(philox4x32_10(orig, T, cw + k, kDomainFlip, keys), thr) << (4 * k);
+    if (mis) {   // first_replica not a multiple of 4: the 16 replicas straddle five Philox calls
+        m |= lt4(philox4x32_10(orig, T, cw + 4, kDomainFlip, keys), thr) << 16;
+        m = (m >> mis) & 0xffffu;
+    }
+    return m;
 }
 
 template <typename AccT>
@@ -73,143 +116,509 @@ __device__ __forceinline__ void flush_acc(AccT (&acc)[16], long long* s_acc, int
     }
 }
 
-// KIND: kKindGS (in place, one colour class), kKindJacobi (src -> dst), kKindEval (no write).
+// Per-unit context of a lane (tile-adjusted pointers already include the lane's half).
+struct PassCtx {
+    const uint8_t* src;
+    uint8_t* dst;
+    uint8_t* best;         // best-state capture target of the fused path, or nullptr
+    uint32_t cap16;        // capture mask: bit j set = replica j of this lane improved in the last sweep
+    uint32_t rep_lane0;    // global id of this lane's replica 0
+    uint32_t thr, T;
+    int32_t tie_rule;
+};
+
+// a4-a7 for one row and this lane's 16 replicas.
+template <int KIND, typename AccT>
+__device__ __forceinline__ void row_update(const PassCtx& x, const int (&h)[16], const uint4& so4, uint32_t flip16,
+                                           size_t row_off, AccT (&acc)[16]) {
+    const uint32_t so[4] = {so4.x, so4.y, so4.z, so4.w};
+    if (KIND == kKindEval) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) acc[4 * k + b] += (AccT)sbyte(so[k], b) * (AccT)h[4 * k + b];
+        return;
+    }
+    uint32_t nv[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        uint32_t word = 0;
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const int hv = h[4 * k + b];
+            const int sold = sbyte(so[k], b);
+            int a = hv < 0 ? 1 : -1;
+            if (x.tie_rule == 1 && hv == 0) a = sold;
+            if ((flip16 >> (4 * k + b)) & 1u) a = -a;
+            if (KIND == kKindGS) acc[4 * k + b] += (AccT)(a - sold) * (AccT)hv;
+            else acc[4 * k + b] += (AccT)sold * (AccT)hv;
+            word |= ((uint32_t)a & 0xffu) << (8 * b);
+        }
+        nv[k] = word;
+    }
+    *reinterpret_cast<uint4*>(x.dst + row_off) = make_uint4(nv[0], nv[1], nv[2], nv[3]);
+    if (KIND == kKindGS && x.cap16 != 0u) {
+        // fused best-state capture: the value this row held after the previous sweep
+        uint4* bp = reinterpret_cast<uint4*>(x.best + row_off);
+        if (x.cap16 == 0xffffu) {
+            *bp = so4;
+        } else {
+            uint4 b = __ldcg(bp);
+            const uint32_t k0 = nibble_to_bytemask(x.cap16 & 15u), k1 = nibble_to_bytemask((x.cap16 >> 4) & 15u);
+            const uint32_t k2 = nibble_to_bytemask((x.cap16 >> 8) & 15u), k3 = nibble_to_bytemask((x.cap16 >> 12) & 15u);
+            b.x = (so4.x & k0) | (b.x & ~k0);
+            b.y = (so4.y & k1) | (b.y & ~k1);
+            b.z = (so4.z & k2) | (b.z & ~k2);
+            b.w = (so4.w & k3) | (b.w & ~k3);
+            *bp = b;
+        }
+    }
+}
+
+// Everything a warp needs to start a slice; addressed by the slice index alone.
+struct SliceHead {
+    SliceDesc d;
+    int4 c;
+    uint32_t w;
+    uint32_t orig;
+};
+
+template <bool WIDE>
+__device__ __forceinline__ SliceHead fetch_head(const GraphView& g, uint32_t s, int sr) {
+    SliceHead h;
+    const int4 dd = ld_stream(reinterpret_cast<const int4*>(g.slices + s));
+    h.d.off = (uint32_t)dd.x; h.d.row0 = (uint32_t)dd.y; h.d.G = (uint32_t)dd.z; h.d.meta = (uint32_t)dd.w;
+    const size_t at = (size_t)s * kSubRows + sr;
+    h.c = ld_stream(g.col4 + at);
+    h.w = WIDE ? 0u : ld_stream(g.w4 + at);
+    h.orig = ld_stream(g.sorig + at);
+    return h;
+}
+
+// One (slice, tile) unit, whole warp.
+template <int KIND, bool WIDE, typename AccT>
+__device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x, const SliceHead& hd, uint32_t s,
+                                           int sr, AccT (&acc)[16], const PhiloxKeys& keys) {
+    const SliceDesc d = hd.d;
+    const int log_spr = (int)(d.meta & 0xffu);
+    const int nrows = (int)(d.meta >> 8);
+    const int rloc = sr >> log_spr;
+    const bool owner = ((sr & ((1 << log_spr) - 1)) == 0) && rloc < nrows;
+    const size_t row_off = (size_t)(d.row0 + (uint32_t)rloc) * kTile;
+
+    int h[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) h[k] = 0;
+    int4 c = hd.c;
+    uint32_t w = hd.w;
+    const int4* cp = g.col4 + d.off + sr;
+    const uint32_t* wp = g.w4 + d.off + sr;
+    const int4* wwp = g.w4w + d.off + sr;
+    int4 ww = make_int4(0, 0, 0, 0);
+    if (WIDE) ww = ld_stream(g.w4w + (size_t)s * kSubRows + sr);
+
+    uint4 e0 = ld_nbr(x.src, c.x), e1 = ld_nbr(x.src, c.y), e2 = ld_nbr(x.src, c.z), e3 = ld_nbr(x.src, c.w);
+    uint4 so4 = make_uint4(0u, 0u, 0u, 0u);
+    if (owner) so4 = ld_spin(x.src + row_off);
+    uint32_t flip16 = 0;
+    if (KIND != kKindEval && owner) flip16 = flip_mask16(hd.orig, x.T, x.rep_lane0, x.thr, keys);
+
+    for (uint32_t gi = 1;; ++gi) {
+        const uint32_t wc = w;
+        const int4 wwc = ww;
+        const bool more = gi < d.G;
+        if (more) {   // indices of the next group while the gathers fly
+            c = ld_stream(cp + (size_t)(gi - 1) * kSubRows);
+            if (WIDE) ww = ld_stream(wwp + (size_t)(gi - 1) * kSubRows);
+            else w = ld_stream(wp + (size_t)(gi - 1) * kSubRows);
+        }
+        if (WIDE) field_cell_wide(h, e0, e1, e2, e3, wwc);
+        else field_cell(h, e0, e1, e2, e3, wc);
+        if (!more) break;
+        e0 = ld_nbr(x.src, c.x); e1 = ld_nbr(x.src, c.y); e2 = ld_nbr(x.src, c.z); e3 = ld_nbr(x.src, c.w);
+    }
+
+    // warp-level segmented reduction over the sub-rows of one row
+    for (int lvl = 0; lvl < log_spr; ++lvl) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) h[k] += __shfl_xor_sync(0xffffffffu, h[k], 2 << lvl);
+    }
+    if (owner) row_update<KIND>(x, h, so4, flip16, row_off, acc);
+}
+
+// One (hub, tile) unit, whole CTA.  s_hub: [kWarpsPerCta][32] ints of the buffer of this hub's
+// parity (the caller alternates two buffers, so one __syncthreads per hub suffices).
+template <int KIND, bool WIDE, typename AccT>
+__device__ __forceinline__ void hub_pass(const GraphView& g, const PassCtx& x, const HubDesc& hd, int warp, int sr,
+                                         int half, int (*s_hub)[kTile], bool epi_warp, AccT (&acc)[16],
+                                         const PhiloxKeys& keys) {
+    const bool owner = epi_warp && sr == 0;
+    const size_t row_off = (size_t)hd.row * kTile;
+    const size_t j = (size_t)hd.off + (size_t)(warp * kSubRows + sr);
+    int h[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) h[k] = 0;
+    int4 c = ld_stream(g.col4 + j);
+    uint32_t w = 0;
+    int4 ww = make_int4(0, 0, 0, 0);
+    if (WIDE) ww = ld_stream(g.w4w + j);
+    else w = ld_stream(g.w4 + j);
+    uint4 so4 = make_uint4(0u, 0u, 0u, 0u);
+    if (owner) so4 = ld_spin(x.src + row_off);
+    uint4 e0 = ld_nbr(x.src, c.x), e1 = ld_nbr(x.src, c.y), e2 = ld_nbr(x.src, c.z), e3 = ld_nbr(x.src, c.w);
+    uint32_t flip16 = 0;
+    if (KIND != kKindEval && owner) flip16 = flip_mask16(hd.orig, x.T, x.rep_lane0, x.thr, keys);
+    for (uint32_t gi = 1;; ++gi) {
+        const uint32_t wc = w;
+        const int4 wwc = ww;
+        const bool more = gi < hd.G;
+        if (more) {
+            c = ld_stream(g.col4 + j + (size_t)gi * kHubSub);
+            if (WIDE) ww = ld_stream(g.w4w + j + (size_t)gi * kHubSub);
+            else w = ld_stream(g.w4 + j + (size_t)gi * kHubSub);
+        }
+        if (WIDE) field_cell_wide(h, e0, e1, e2, e3, wwc);
+        else field_cell(h, e0, e1, e2, e3, wc);
+        if (!more) break;
+        e0 = ld_nbr(x.src, c.x); e1 = ld_nbr(x.src, c.y); e2 = ld_nbr(x.src, c.z); e3 = ld_nbr(x.src, c.w);
+    }
+#pragma unroll
+    for (int lvl = 0; lvl < 4; ++lvl) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) h[k] += __shfl_xor_sync(0xffffffffu, h[k], 2 << lvl);
+    }
+    if (sr == 0) {
+#pragma unroll
+        for (int k = 0; k < 16; k += 4)
+            *reinterpret_cast<int4*>(&s_hub[warp][half * 16 + k]) = make_int4(h[k], h[k + 1], h[k + 2], h[k + 3]);
+    }
+    __syncthreads();
+    if (owner) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) h[k] = 0;
+        for (int wv = 0; wv < kWarpsPerCta; ++wv) {
+#pragma unroll
+            for (int k = 0; k < 16; k += 4) {
+                const int4 v = *reinterpret_cast<const int4*>(&s_hub[wv][half * 16 + k]);
+                h[k] += v.x; h[k + 1] += v.y; h[k + 2] += v.z; h[k + 3] += v.w;
+            }
+        }
+        row_update<KIND>(x, h, so4, flip16, row_off, acc);
+    }
+}
+
+__device__ __forceinline__ PhaseRange ld_range(const PhaseRange* p) {
+    const int4 v = ld_stream(reinterpret_cast<const int4*>(p));
+    PhaseRange r;
+    r.s0 = (uint32_t)v.x; r.s1 = (uint32_t)v.y; r.h0 = (uint32_t)v.z; r.h1 = (uint32_t)v.w;
+    return r;
+}
+__device__ __forceinline__ HubDesc ld_hub(const HubDesc* p) {
+    const int4 v = ld_stream(reinterpret_cast<const int4*>(p));
+    HubDesc r;
+    r.off = (uint32_t)v.x; r.row = (uint32_t)v.y; r.G = (uint32_t)v.z; r.orig = (uint32_t)v.w;
+    return r;
+}
+
+__device__ __forceinline__ PassCtx make_ctx(const uint8_t* src, uint8_t* dst, uint8_t* best, uint32_t cap_mask,
+                                            unsigned long long tile_stride, uint32_t tile, int half, uint32_t rep0,
+                                            uint32_t thr, uint32_t T, int32_t tie_rule) {
+    PassCtx x;
+    const size_t o = (size_t)tile * tile_stride + (size_t)half * 16;
+    x.src = src + o;
+    x.dst = dst + o;
+    x.best = best ? best + o : nullptr;
+    x.cap16 = (cap_mask >> (half * 16)) & 0xffffu;
+    x.rep_lane0 = rep0 + tile * kTile + (uint32_t)half * 16u;
+    x.thr = thr;
+    x.T = T;
+    x.tie_rule = tie_rule;
+    return x;
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_sweep: colour phases [phase_begin, phase_end) of one sweep in one launch.
+// KIND: kKindGS (in place), kKindJacobi (src -> dst), kKindEval (no write).
 // WIDE: int32 weights (w4w) and int64 bookkeeping; otherwise int8 weights, dp4a, int32 bookkeeping
-// flushed every p.flush_rows rows.
+// flushed every p.flush_rows rows.  Grid = g.n_cta CTAs of kSweepThreads threads.
+// ---------------------------------------------------------------------------------------------
 template <int KIND, bool WIDE>
-__global__ void __launch_bounds__(kSweepThreads) k_sweep(const SweepParams p) {
+__global__ void __launch_bounds__(kSweepThreads, 1) k_sweep(const SweepParams p) {
     using AccT = typename std::conditional<WIDE, long long, int>::type;
-    __shared__ long long s_acc[kTile];
+    __shared__ long long s_acc[kMaxPersistReplicas];
+    __shared__ __align__(16) int s_hub[2][kWarpsPerCta][kTile];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int sr = lane >> 1, half = lane & 1;
-    const uint32_t tile = blockIdx.y;
-    if (threadIdx.x < kTile) s_acc[threadIdx.x] = 0;
+    const uint32_t tiles = p.tiles;
+    for (uint32_t i = threadIdx.x; i < tiles * kTile; i += blockDim.x) s_acc[i] = 0;
     __syncthreads();
-
-    const uint8_t* src = p.src + (size_t)tile * p.tile_stride + half * 16;
-    uint8_t* dst = p.dst + (size_t)tile * p.tile_stride + half * 16;
-    const uint32_t rep_lane0 = p.rep0 + tile * kTile + half * 16;   // global id of this lane's replica 0
 
     AccT acc[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) acc[k] = 0;
-    uint32_t rows_acc = 0;
+    uint32_t rows_acc = 0, acc_tile = 0, hub_count = 0;
 
-    for (uint32_t s = p.slice_begin + blockIdx.x * kWarpsPerCta + warp; s < p.slice_end;
-         s += gridDim.x * kWarpsPerCta) {
-        const SliceDesc d = p.slices[s];
-        int h[16];
-#pragma unroll
-        for (int k = 0; k < 16; ++k) h[k] = 0;
-
-        if (d.G > 0) {
-            const int4* cp = p.col4 + d.off + sr;
-            if (!WIDE) {
-                const uint32_t* wp = p.w4 + d.off + sr;
-                int4 c = ld_stream(cp);
-                uint32_t w = ld_stream(wp);
-                for (uint32_t g = 0; g < d.G; ++g) {
-                    const uint4 e0 = ld_spin(src + (size_t)(uint32_t)c.x * kTile);
-                    const uint4 e1 = ld_spin(src + (size_t)(uint32_t)c.y * kTile);
-                    const uint4 e2 = ld_spin(src + (size_t)(uint32_t)c.z * kTile);
-                    const uint4 e3 = ld_spin(src + (size_t)(uint32_t)c.w * kTile);
-                    const uint32_t wc = w;
-                    if (g + 1 < d.G) {   // prefetch the next group's indices while the gathers fly
-                        c = ld_stream(cp + (size_t)(g + 1) * kSubRows);
-                        w = ld_stream(wp + (size_t)(g + 1) * kSubRows);
-                    }
-                    field_word(h, 0, e0.x, e1.x, e2.x, e3.x, wc);
-                    field_word(h, 1, e0.y, e1.y, e2.y, e3.y, wc);
-                    field_word(h, 2, e0.z, e1.z, e2.z, e3.z, wc);
-                    field_word(h, 3, e0.w, e1.w, e2.w, e3.w, wc);
+    for (uint32_t ph = p.phase_begin; ph < p.phase_end; ++ph) {
+        const PhaseRange pr = ld_range(p.g.ranges + (size_t)ph * p.g.n_cta + blockIdx.x);
+        for (uint32_t hh = pr.h0; hh < pr.h1; ++hh) {
+            const HubDesc hd = ld_hub(p.g.hubs + hh);
+            for (uint32_t tile = 0; tile < tiles; ++tile, ++hub_count) {
+                const bool epi = (hub_count % kWarpsPerCta) == (uint32_t)warp;
+                if (epi && tile != acc_tile) {
+                    flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                    rows_acc = 0;
+                    acc_tile = tile;
                 }
-            } else {
-                const int4* wp = p.w4w + d.off + sr;
-                for (uint32_t g = 0; g < d.G; ++g) {
-                    const int4 c = ld_stream(cp + (size_t)g * kSubRows);
-                    const int4 w = ld_stream(wp + (size_t)g * kSubRows);
-                    const uint4 e0 = ld_spin(src + (size_t)(uint32_t)c.x * kTile);
-                    const uint4 e1 = ld_spin(src + (size_t)(uint32_t)c.y * kTile);
-                    const uint4 e2 = ld_spin(src + (size_t)(uint32_t)c.z * kTile);
-                    const uint4 e3 = ld_spin(src + (size_t)(uint32_t)c.w * kTile);
-                    field_word_wide(h, 0, e0.x, w.x); field_word_wide(h, 1, e0.y, w.x);
-                    field_word_wide(h, 2, e0.z, w.x); field_word_wide(h, 3, e0.w, w.x);
-                    field_word_wide(h, 0, e1.x, w.y); field_word_wide(h, 1, e1.y, w.y);
-                    field_word_wide(h, 2, e1.z, w.y); field_word_wide(h, 3, e1.w, w.y);
-                    field_word_wide(h, 0, e2.x, w.z); field_word_wide(h, 1, e2.y, w.z);
-                    field_word_wide(h, 2, e2.z, w.z); field_word_wide(h, 3, e2.w, w.z);
-                    field_word_wide(h, 0, e3.x, w.w); field_word_wide(h, 1, e3.y, w.w);
-                    field_word_wide(h, 2, e3.z, w.w); field_word_wide(h, 3, e3.w, w.w);
+                const PassCtx x = make_ctx(p.src, p.dst, nullptr, 0u, p.tile_stride, tile, half, p.rep0, p.thr, p.T,
+                                           p.tie_rule);
+                hub_pass<KIND, WIDE>(p.g, x, hd, warp, sr, half, s_hub[hub_count & 1], epi, acc, p.keys);
+                if (epi && !WIDE && ++rows_acc >= p.flush_rows) {
+                    flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                    rows_acc = 0;
                 }
             }
         }
-
-        // warp-level segmented reduction over the sub-rows of one row
-        const int log_spr = (int)(d.meta & 0xffu);
-        const int nrows = (int)(d.meta >> 8);
-        for (int lvl = 0; lvl < log_spr; ++lvl) {
-#pragma unroll
-            for (int k = 0; k < 16; ++k) h[k] += __shfl_xor_sync(0xffffffffu, h[k], 2 << lvl);
-        }
-        const int rloc = sr >> log_spr;
-        const bool owner = ((sr & ((1 << log_spr) - 1)) == 0) && rloc < nrows;
-        if (owner) {
-            const uint32_t row = d.row0 + (uint32_t)rloc;
-            const uint4 so4 = ld_spin(src + (size_t)row * kTile);
-            const uint32_t so[4] = {so4.x, so4.y, so4.z, so4.w};
-            if (KIND == kKindEval) {
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-#pragma unroll
-                    for (int b = 0; b < 4; ++b) acc[4 * k + b] += (AccT)sbyte(so[k], b) * (AccT)h[4 * k + b];
-            } else {
-                const uint32_t orig = (uint32_t)p.perm[row];
-                const int mis = (int)(rep_lane0 & 3u);
-                uint32_t nv[4];
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    uint4 u = make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu), u2 = u;
-                    if (p.thr != 0) {
-                        const uint32_t cw = (rep_lane0 + 4 * k) >> 2;
-                        u = philox4x32_10(orig, p.T, cw, kDomainFlip, p.keys);
-                        if (mis) u2 = philox4x32_10(orig, p.T, cw + 1, kDomainFlip, p.keys);
-                    }
-                    const uint32_t ur[4] = {u.x, u.y, u.z, u.w};
-                    uint32_t word = 0;
-#pragma unroll
-                    for (int b = 0; b < 4; ++b) {
-                        const int hv = h[4 * k + b];
-                        const int sold = sbyte(so[k], b);
-                        int a = hv < 0 ? 1 : -1;
-                        if (p.tie_rule == 1 && hv == 0) a = sold;
-                        const uint32_t rnd = mis ? pick8(u, u2, mis + b) : ur[b];
-                        if (rnd < p.thr) a = -a;
-                        if (KIND == kKindGS) {
-                            if (a != sold) acc[4 * k + b] += (AccT)(2 * a) * (AccT)hv;
-                        } else {
-                            acc[4 * k + b] += (AccT)sold * (AccT)hv;
-                        }
-                        word |= ((uint32_t)a & 0xffu) << (8 * b);
-                    }
-                    nv[k] = word;
-                }
-                *reinterpret_cast<uint4*>(dst + (size_t)row * kTile) = make_uint4(nv[0], nv[1], nv[2], nv[3]);
+        const uint32_t nu = (pr.s1 - pr.s0) * tiles;
+        for (uint32_t u = warp; u < nu; u += kWarpsPerCta) {
+            const uint32_t s = pr.s0 + u / tiles, tile = u % tiles;
+            const SliceHead hd = fetch_head<WIDE>(p.g, s, sr);
+            if (tile != acc_tile) {
+                flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                rows_acc = 0;
+                acc_tile = tile;
             }
-        }
-        if (!WIDE) {
-            if (++rows_acc >= p.flush_rows) {   // warp-uniform
-                flush_acc(acc, s_acc, lane);
+            const PassCtx x = make_ctx(p.src, p.dst, nullptr, 0u, p.tile_stride, tile, half, p.rep0, p.thr, p.T,
+                                       p.tie_rule);
+            slice_pass<KIND, WIDE>(p.g, x, hd, s, sr, acc, p.keys);
+            if (!WIDE && ++rows_acc >= p.flush_rows) {
+                flush_acc(acc, s_acc + acc_tile * kTile, lane);
                 rows_acc = 0;
             }
         }
     }
-    flush_acc(acc, s_acc, lane);
+    flush_acc(acc, s_acc + acc_tile * kTile, lane);
     __syncthreads();
-    if (threadIdx.x < kTile) {
-        const long long v = s_acc[threadIdx.x];
-        if (v != 0)
-            atomicAdd(reinterpret_cast<unsigned long long*>(p.accum + (size_t)tile * kTile + threadIdx.x),
-                      (unsigned long long)v);
+    for (uint32_t i = threadIdx.x; i < tiles * kTile; i += blockDim.x) {
+        const long long v = s_acc[i];
+        if (v != 0) atomicAdd(reinterpret_cast<unsigned long long*>(p.accum + i), (unsigned long long)v);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_anneal_gs: the persistent Gauss-Seidel annealer (int8 weights).  Cooperative launch,
+// grid = g.n_cta CTAs (one per SM at most), all co-resident.
+// ---------------------------------------------------------------------------------------------
+struct AnnealParams {
+    GraphView g;
+    uint8_t* state;                 // [tiles][n][32], updated in place
+    uint8_t* best;                  // captured best state, same layout
+    unsigned long long tile_stride;
+    unsigned long long n;           // rows
+    uint32_t tiles;
+    uint32_t n_replicas;            // live replicas of this batch (<= tiles * 32)
+    uint32_t rep0;                  // global id of replica 0 of this batch
+    int32_t tie_rule;
+    uint32_t flush_rows;
+    uint32_t n_sweeps, sweep_offset;
+    const uint32_t* thr;            // DEVICE [n_sweeps]
+    long long W;
+    const long long* E0;            // [tiles*32] energy of the initial state
+    long long* accum;               // [3][tiles*32], zero at launch
+    long long* trace;               // [n_sweeps][trace_stride] (column 0 = replica 0 of this batch) or nullptr
+    unsigned long long trace_stride;
+    long long* E_out;               // [tiles*32]
+    long long* best_out;            // [tiles*32]
+    int32_t* best_sweep_out;        // [tiles*32]
+    unsigned int* barrier;          // zero at launch
+    int32_t resume;                 // 1: best_out / best_sweep_out hold the bests of the sweeps before this chunk
+    PhiloxKeys keys;
+};
+
+__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& epoch, unsigned int n_cta) {
+    __syncthreads();
+    epoch += n_cta;
+    if (n_cta > 1) {
+        if (threadIdx.x == 0) {
+            __threadfence();
+            atomicAdd(counter, 1u);
+            unsigned int v;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
+            } while ((int)(v - epoch) < 0);
+            __threadfence();
+        }
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealParams p) {
+    __shared__ long long s_acc[kMaxPersistReplicas];
+    __shared__ long long s_E[kMaxPersistReplicas];
+    __shared__ long long s_best[kMaxPersistReplicas];
+    __shared__ int s_bsweep[kMaxPersistReplicas];
+    __shared__ uint32_t s_mask[kMaxPersistReplicas / kTile];
+    __shared__ __align__(16) int s_hub[2][kWarpsPerCta][kTile];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sr = lane >> 1, half = lane & 1;
+    const uint32_t tiles = p.tiles, nR = p.tiles * kTile, n_cta = p.g.n_cta, C = p.g.n_phases;
+    for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {
+        s_acc[i] = 0;
+        s_E[i] = p.E0[i];
+        s_best[i] = p.resume ? p.best_out[i] : (long long)0x8000000000000000ull;
+        s_bsweep[i] = p.resume ? p.best_sweep_out[i] : 0;
+    }
+    if (threadIdx.x < kMaxPersistReplicas / kTile) s_mask[threadIdx.x] = 0u;
+    __syncthreads();
+
+    int acc[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) acc[k] = 0;
+    uint32_t rows_acc = 0, acc_tile = 0, hub_count = 0;
+    unsigned int epoch = 0;
+
+    const PhaseRange* my_ranges = p.g.ranges + blockIdx.x;
+    PhaseRange pr = ld_range(my_ranges);
+    uint32_t nu = (pr.s1 - pr.s0) * tiles;
+    // one-slice lookahead of the static data, kept across the grid barrier
+    bool have = (uint32_t)warp < nu;
+    uint32_t nxt_s = 0, nxt_tile = 0;
+    SliceHead nxt{};
+    if (have) {
+        nxt_s = pr.s0 + (uint32_t)warp / tiles;
+        nxt_tile = (uint32_t)warp % tiles;
+        nxt = fetch_head<false>(p.g, nxt_s, sr);
+    }
+
+    for (uint32_t t = 0; t < p.n_sweeps; ++t) {
+        const uint32_t thr = __ldg(p.thr + t);
+        const uint32_t T = p.sweep_offset + t;
+        for (uint32_t ph = 0; ph < C; ++ph) {
+            const bool last_phase = ph + 1 == C;
+            const bool very_last = last_phase && t + 1 == p.n_sweeps;
+            const PhaseRange prn = ld_range(my_ranges + (size_t)(last_phase ? 0u : ph + 1u) * n_cta);
+
+            for (uint32_t hh = pr.h0; hh < pr.h1; ++hh) {
+                const HubDesc hd = ld_hub(p.g.hubs + hh);
+                for (uint32_t tile = 0; tile < tiles; ++tile, ++hub_count) {
+                    const bool epi = (hub_count % kWarpsPerCta) == (uint32_t)warp;
+                    if (epi && tile != acc_tile) {
+                        flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                        rows_acc = 0;
+                        acc_tile = tile;
+                    }
+                    const PassCtx x = make_ctx(p.state, p.state, p.best, s_mask[tile], p.tile_stride, tile, half,
+                                               p.rep0, thr, T, p.tie_rule);
+                    hub_pass<kKindGS, false>(p.g, x, hd, warp, sr, half, s_hub[hub_count & 1], epi, acc, p.keys);
+                    if (epi && ++rows_acc >= p.flush_rows) {
+                        flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                        rows_acc = 0;
+                    }
+                }
+            }
+
+            uint32_t u = (uint32_t)warp;
+            while (have) {
+                const SliceHead cur = nxt;
+                const uint32_t s = nxt_s, tile = nxt_tile;
+                u += kWarpsPerCta;
+                have = u < nu;
+                if (have) {
+                    nxt_s = pr.s0 + u / tiles;
+                    nxt_tile = u % tiles;
+                    nxt = fetch_head<false>(p.g, nxt_s, sr);
+                }
+                if (tile != acc_tile) {
+                    flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                    rows_acc = 0;
+                    acc_tile = tile;
+                }
+                const PassCtx x = make_ctx(p.state, p.state, p.best, s_mask[tile], p.tile_stride, tile, half, p.rep0,
+                                           thr, T, p.tie_rule);
+                slice_pass<kKindGS, false>(p.g, x, cur, s, sr, acc, p.keys);
+                if (++rows_acc >= p.flush_rows) {
+                    flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                    rows_acc = 0;
+                }
+            }
+
+            // static data of this warp's first slice of the next phase: issued before the barrier
+            pr = prn;
+            nu = (pr.s1 - pr.s0) * tiles;
+            have = !very_last && (uint32_t)warp < nu;
+            if (have) {
+                nxt_s = pr.s0 + (uint32_t)warp / tiles;
+                nxt_tile = (uint32_t)warp % tiles;
+                nxt = fetch_head<false>(p.g, nxt_s, sr);
+            }
+
+            if (last_phase) {   // a7: this sweep's energy increments -> accum slot t % 3
+                flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                rows_acc = 0;
+                __syncthreads();
+                long long* slot = p.accum + (size_t)(t % 3u) * nR;
+                for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {
+                    const long long v = s_acc[i];
+                    if (v != 0) {
+                        atomicAdd(reinterpret_cast<unsigned long long*>(slot + i), (unsigned long long)v);
+                        s_acc[i] = 0;
+                    }
+                }
+            }
+            grid_barrier(p.barrier, epoch, n_cta);
+        }
+
+        // sweep end (every CTA redundantly): E, cut = (W - E)/2 (eq. 4), improved mask
+        {
+            const long long* slot = p.accum + (size_t)(t % 3u) * nR;
+            long long* zero_slot = p.accum + (size_t)((t + 2u) % 3u) * nR;
+            for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {   // nR is a multiple of 32: warp-uniform
+                const long long E = s_E[i] + __ldcg(slot + i);
+                const long long cut = (p.W - E) / 2;
+                const bool live = i < p.n_replicas;
+                const bool improved = live && cut > s_best[i];
+                s_E[i] = E;
+                if (improved) { s_best[i] = cut; s_bsweep[i] = (int)T; }
+                const uint32_t m = __ballot_sync(0xffffffffu, improved);
+                if (lane == 0) s_mask[i >> 5] = m;
+                if (blockIdx.x == 0) {
+                    zero_slot[i] = 0;
+                    if (live && p.trace) p.trace[(size_t)t * p.trace_stride + i] = cut;
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    // capture of the improvements of the final sweep (earlier ones were captured in flight)
+    for (uint32_t tile = 0; tile < tiles; ++tile) {
+        const uint32_t mask = s_mask[tile];
+        if (mask == 0u) continue;
+        const uint4* src = reinterpret_cast<const uint4*>(p.state + (size_t)tile * p.tile_stride);
+        uint4* best = reinterpret_cast<uint4*>(p.best + (size_t)tile * p.tile_stride);
+        const uint32_t m_lo = mask & 0xffffu, m_hi = mask >> 16;
+        const unsigned long long units = p.n * 2ull;
+        for (unsigned long long uu = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; uu < units;
+             uu += (unsigned long long)gridDim.x * blockDim.x) {
+            const uint32_t m = (uu & 1ull) ? m_hi : m_lo;
+            if (m == 0u) continue;
+            const uint4 s = __ldcg(src + uu);
+            if (m == 0xffffu) { best[uu] = s; continue; }
+            uint4 b = __ldcg(best + uu);
+            const uint32_t k0 = nibble_to_bytemask(m & 15u), k1 = nibble_to_bytemask((m >> 4) & 15u);
+            const uint32_t k2 = nibble_to_bytemask((m >> 8) & 15u), k3 = nibble_to_bytemask((m >> 12) & 15u);
+            b.x = (s.x & k0) | (b.x & ~k0);
+            b.y = (s.y & k1) | (b.y & ~k1);
+            b.z = (s.z & k2) | (b.z & ~k2);
+            b.w = (s.w & k3) | (b.w & ~k3);
+            best[uu] = b;
+        }
+    }
+    if (blockIdx.x == 0) {
+        for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {
+            p.E_out[i] = s_E[i];
+            p.best_out[i] = s_best[i];
+            p.best_sweep_out[i] = s_bsweep[i];
+        }
     }
 }
 
@@ -240,12 +649,6 @@ struct SweepEndParams {
     int32_t first;                 // 1: no best recorded yet in this call
     int32_t T;
 };
-
-__device__ __forceinline__ uint32_t nibble_to_bytemask(uint32_t nib) {
-    // bit b of nib -> byte b = 0xff
-    uint32_t m = (nib & 1u) | ((nib & 2u) << 7) | ((nib & 4u) << 14) | ((nib & 8u) << 21);
-    return m * 0xffu;
-}
 
 __global__ void __launch_bounds__(256) k_sweep_end(const SweepEndParams p) {
     __shared__ uint32_t s_mask;
