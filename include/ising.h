@@ -186,9 +186,20 @@ ising_status ising_current_state(ising_problem* p, int8_t* spins_out, int32_t n_
  * Properties of a loaded problem (host-side bookkeeping, no device work).
  *   what: 0 n, 1 nnz, 2 n_colours, 3 max_replicas, 4 W = sum_{i<j} w_ij, 5 dense engine built (0/1),
  *         6 kernels launched by this handle so far, 7 max_i sum_j |w_ij|, 8 workspace bytes in use,
- *         9 slices of the sparse layout, 10 padded edge slots of the sparse layout
+ *         9 slices of the sparse layout, 10 padded edge slots of the sparse layout, 11 hub rows,
+ *         12 CTAs of the persistent grid
  */
 ising_status ising_problem_info(const ising_problem* p, int32_t what, int64_t* value_out);
+
+/*
+ * Diagnostics of the persistent Gauss-Seidel kernel: the next ising_anneal calls record, for sweep
+ * `sweep` of the call, the SM clock of every CTA when it arrives at and when it leaves the grid
+ * barrier that ends each colour phase.
+ *   stamps   uint64 [n_colours][n_cta][2] (arrive, leave), DEVICE; n_cta = ising_problem_info(12);
+ *            NULL switches the recording off
+ * Stamps of different CTAs come from different SM clocks: compare differences within one CTA.
+ */
+ising_status ising_debug_phase_timing(ising_problem* p, uint64_t* stamps, int32_t sweep);
 
 /* Release the handle (the workspace returns to the caller).  NULL is allowed. */
 ising_status ising_free(ising_problem* p);

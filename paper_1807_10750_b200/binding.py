@@ -73,6 +73,8 @@ def lib():
     L.ising_current_state.argtypes = [_vp, _vp, _i32, _vp]
     L.ising_problem_info.restype = _i32
     L.ising_problem_info.argtypes = [_vp, _i32, ctypes.POINTER(_i64)]
+    L.ising_debug_phase_timing.restype = _i32
+    L.ising_debug_phase_timing.argtypes = [_vp, _vp, _i32]
     L.ising_free.restype = _i32
     L.ising_free.argtypes = [_vp]
     _lib = L
@@ -147,6 +149,15 @@ class Problem:
     @property
     def launches(self) -> int:
         return self.info(6)
+
+    def phase_timing(self, sweep: int = 0):
+        """Diagnostics: record barrier arrive/leave SM clocks of sweep `sweep` of the next GS anneal.
+        Returns the int64 device tensor [n_colours][n_cta][2] the kernel will fill."""
+        t = _torch()
+        buf = t.zeros((max(1, self.n_colours), self.info(12), 2), dtype=t.int64, device="cuda")
+        _check(lib().ising_debug_phase_timing(self.handle, buf.data_ptr(), sweep), "ising_debug_phase_timing")
+        self._keep.append(buf)
+        return buf
 
     def free(self):
         if self.handle:

@@ -83,8 +83,8 @@ __global__ void k_validate(int32_t n, const long long* row_ptr, const int32_t* c
     }
 }
 
-// One warp per slice: fill the cells of the slice (head cell for group 0, tail cells for the
-// rest) and the per-sub-row caller ids.  Cell (g, sr) holds group q = g * SPR + part of row
+// One warp per slice: fill the cells of the slice (head cells for groups 0 and 1, tail cells for
+// the rest) and the per-sub-row caller ids.  Cell (g, sr) holds group q = g * SPR + part of row
 // row0 + (sr >> log_spr), part = sr & (SPR - 1); edges 4q .. 4q+3.
 __device__ __forceinline__ void store_cell(int4* col4, uint32_t* w4, int4* w4w, size_t at, const int (&cc)[4],
                                            const int (&ww)[4]) {
@@ -95,11 +95,12 @@ __device__ __forceinline__ void store_cell(int4* col4, uint32_t* w4, int4* w4w, 
 }
 
 __device__ __forceinline__ void fetch_group(const int32_t* inv, const int32_t* col, const void* w, int wtype,
-                                            long long b, long long deg, long long q, int (&cc)[4], int (&ww)[4]) {
+                                            long long b, long long deg, long long q, int pad, int (&cc)[4],
+                                            int (&ww)[4]) {
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const long long e = 4 * q + j;
-        cc[j] = -1;
+        cc[j] = pad;
         ww[j] = 0;
         if (e < deg) {
             cc[j] = inv[col[b + e]];
@@ -125,15 +126,25 @@ __global__ void k_pack(const SliceDesc* slices, uint32_t n_slices, const int32_t
     for (unsigned long long cell = lane; cell < cells; cell += 32) {
         const uint32_t g = (uint32_t)(cell / kSubRows), sr = (uint32_t)(cell % kSubRows);
         const uint32_t rloc = sr >> log_spr, part = sr & (spr - 1);
-        int cc[4] = {-1, -1, -1, -1};
+        const int pad = (int)((int)rloc < nrows ? d.row0 + rloc : d.row0);
+        int cc[4] = {pad, pad, pad, pad};
         int ww[4] = {0, 0, 0, 0};
         if ((int)rloc < nrows) {
             const int32_t orig = perm[d.row0 + rloc];
             const long long b = row_ptr[orig], deg = row_ptr[orig + 1] - b;
-            fetch_group(inv, col, w, wtype, b, deg, (long long)g * spr + part, cc, ww);
+            fetch_group(inv, col, w, wtype, b, deg, (long long)g * spr + part, pad, cc, ww);
         }
-        const size_t at = g == 0 ? (size_t)gw * kSubRows + sr : (size_t)d.off + (size_t)(g - 1) * kSubRows + sr;
+        const size_t at = g < kHeadGroups ? ((size_t)gw * kHeadGroups + g) * kSubRows + sr
+                                          : (size_t)d.off + (size_t)(g - kHeadGroups) * kSubRows + sr;
         store_cell(col4, w4, w4w, at, cc, ww);
+    }
+    if (d.G < kHeadGroups && lane < kSubRows) {   // unused head cells: all padding
+        const uint32_t rloc = (uint32_t)lane >> log_spr;
+        const int pad = (int)((int)rloc < nrows ? d.row0 + rloc : d.row0);
+        const int cc[4] = {pad, pad, pad, pad};
+        const int ww[4] = {0, 0, 0, 0};
+        for (uint32_t g = d.G; g < kHeadGroups; ++g)
+            store_cell(col4, w4, w4w, ((size_t)gw * kHeadGroups + g) * kSubRows + lane, cc, ww);
     }
 }
 
@@ -146,7 +157,7 @@ __global__ void k_pack_hubs(const HubDesc* hubs, uint32_t n_hubs, const int32_t*
     const unsigned long long cells = (unsigned long long)d.G * kHubSub;
     for (unsigned long long cell = threadIdx.x; cell < cells; cell += blockDim.x) {
         int cc[4], ww[4];
-        fetch_group(inv, col, w, wtype, b, deg, (long long)cell, cc, ww);
+        fetch_group(inv, col, w, wtype, b, deg, (long long)cell, (int)d.row, cc, ww);
         store_cell(col4, w4, w4w, (size_t)d.off + cell, cc, ww);
     }
 }

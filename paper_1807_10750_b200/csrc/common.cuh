@@ -11,11 +11,13 @@
 //     sub-rows, group q goes to sub-row q % 256) and is finished through shared memory;
 //   * a CELL is one int4 of four (relabelled) neighbour rows plus one word of four int8
 //     weights (w4w: an int4 of int32 weights for graphs whose weights do not fit int8).
-//     Padding entries carry column -1 (the gather is predicated off) and weight 0.
-//     Cell arrays: group 0 of slice s sits at HEAD cell s*16 + sub-row, so that everything
-//     a warp needs to start a slice (descriptor, first cells, caller ids) is addressed by the
-//     slice index alone and can be prefetched with independent loads, also across the grid
-//     barrier that separates colour phases; groups g >= 1 sit at desc.off + (g-1)*16 + sub-row;
+//     Padding entries carry weight 0 and point at the sub-row's own row (a sector that is read
+//     anyway), so gathers need no predicate.
+//     Cell arrays: groups 0 and 1 of slice s sit at HEAD cells (s*2 + g)*16 + sub-row, so that
+//     everything a warp needs to start a slice (descriptor, first cells, caller ids) is addressed
+//     by the slice index alone and can be prefetched with independent loads, also across the grid
+//     barrier that separates colour phases.  Rows of up to 128 edges live entirely in head cells;
+//     groups g >= 2 (rows of 129..256 edges) sit at desc.off + (g-2)*16 + sub-row;
 //     hub cells sit at hub.off + g*256 + sub-row;
 //   * spins are replica-interleaved: state[tile][row][32] int8 (+1/-1), one 32-byte
 //     sector per spin per tile of 32 replicas, so a neighbour gather is one sector and a
@@ -35,13 +37,14 @@ constexpr int kTile = 32;            // replicas per tile == bytes per spin per 
 constexpr int kSubRows = 16;         // sub-rows per slice (lane pairs per warp)
 constexpr int kWarpsPerCta = 16;
 constexpr int kSweepThreads = kWarpsPerCta * 32;
-constexpr int kSubRowEdges = 16;     // a row is split until a sub-row has <= this many edges
-constexpr int kHubDegree = kSubRows * kSubRowEdges;    // 256: larger rows are CTA hubs
+constexpr int kHeadGroups = 2;       // groups of every slice stored at slice-indexed (prefetchable) positions
+constexpr int kSubRowEdges = 4 * kHeadGroups;          // a row is split until a sub-row has <= this many edges ...
+constexpr int kHubDegree = 256;                        // ... up to 16 sub-rows; rows above this are CTA hubs
 constexpr int kHubSub = kWarpsPerCta * kSubRows;       // 256 sub-rows of a hub
 constexpr int kMaxPersistReplicas = 1024;              // replicas per persistent launch
 
 struct SliceDesc {
-    uint32_t off;    // first tail cell (groups >= 1) of this slice
+    uint32_t off;    // first tail cell (groups >= kHeadGroups) of this slice
     uint32_t row0;   // first internal row
     uint32_t G;      // groups (of 4 edges) per sub-row, >= 1
     uint32_t meta;   // log2(SPR) | (valid rows << 8)
@@ -107,11 +110,10 @@ __device__ __forceinline__ uint32_t ld_stream(const uint32_t* p) {
 __device__ __forceinline__ uint4 ld_spin(const uint8_t* p) {
     return __ldcg(reinterpret_cast<const uint4*>(p));
 }
-// Neighbour gather; padding entries (col < 0) are predicated off and read as zero.
+// Neighbour gather.  Padding entries point at the sub-row's own row with weight 0: all paddings of
+// a sub-row hit one sector (which the row's owner reads anyway), so they need no predicate.
 __device__ __forceinline__ uint4 ld_nbr(const uint8_t* base, int c) {
-    uint4 r = make_uint4(0u, 0u, 0u, 0u);
-    if (c >= 0) r = __ldcg(reinterpret_cast<const uint4*>(base + (size_t)(uint32_t)c * kTile));
-    return r;
+    return __ldcg(reinterpret_cast<const uint4*>(base + (size_t)(uint32_t)c * kTile));
 }
 
 }  // namespace ising

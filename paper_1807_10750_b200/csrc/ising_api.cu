@@ -63,16 +63,16 @@ constexpr uint32_t kThrCap = 1u << 16;   // thresholds per persistent launch (lo
 
 // Upper bounds used by ising_workspace_bytes (any degree distribution).
 inline uint64_t bound_slices(int64_t n, int64_t nnz, int64_t C) {
-    // full slices of rows with <= 16 edges, full row-split slices (> 128 edges each), one ragged
+    // full slices of rows with <= 8 edges, full row-split slices (> 64 edges each), one ragged
     // slice per (colour, SPR)
-    return (uint64_t)n / 16 + (uint64_t)nnz / 128 + 5 * (uint64_t)(C + 1) + 8;
+    return (uint64_t)n / 16 + (uint64_t)nnz / 64 + 5 * (uint64_t)(C + 1) + 8;
 }
 inline uint64_t bound_hubs(int64_t nnz) { return (uint64_t)nnz / (kHubDegree + 1) + 1; }
 inline uint64_t bound_cells(int64_t n, int64_t nnz, int64_t C) {
-    // slices: rows are degree-sorted inside a colour, so a slice's cells are covered by the rows of the
-    // slice before it (nnz/4 + rounding n + nnz/8) plus the first slice of every (colour, SPR) group;
-    // hubs: nnz_h/4 + 256 cells of rounding per hub
-    return 320 * (uint64_t)(C + 1) + (uint64_t)n + (uint64_t)nnz / 2 + (uint64_t)nnz / 4 + kHubSub * bound_hubs(nnz) + 64;
+    // two head cells per sub-row of every slice; tail cells only for rows of 129..256 edges (each
+    // holds >= 1 edge of a sub-row that is more than half full); hubs: nnz_h/4 + 256 cells of rounding each
+    return kHeadGroups * kSubRows * bound_slices(n, nnz, C) + (uint64_t)nnz / 2 + kHubSub * bound_hubs(nnz) +
+           (uint64_t)nnz / 4 + 64;
 }
 constexpr uint64_t kMaxCtas = 1024;
 
@@ -164,6 +164,8 @@ struct ising_problem {
     int sm_count = 148;
     bool cooperative = false;
     uint32_t flush_rows = 1;
+    unsigned long long* timing = nullptr;   // diagnostics buffer of the next Gauss-Seidel anneal
+    uint32_t timing_sweep = 0;
 };
 
 namespace {
@@ -428,19 +430,22 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
                 d.G = (uint32_t)G;
                 d.meta = (uint32_t)l | ((uint32_t)nr << 8);
                 slices.push_back(d);
-                tail_cells += (uint64_t)(G - 1) * kSubRows;
+                tail_cells += (uint64_t)std::max<int64_t>(0, G - kHeadGroups) * kSubRows;
                 k += nr;
             }
         }
         slice_begin[C] = (uint32_t)slices.size();
         hub_begin[C] = (uint32_t)hubs_sorted.size();
     }
-    const uint64_t head_cells = (uint64_t)slices.size() * kSubRows;
+    const uint64_t head_cells = (uint64_t)slices.size() * kSubRows * kHeadGroups;
     const uint64_t cells = head_cells + tail_cells + hub_cells;
     if (cells > 0xffffffffull) return ISING_ERR_BAD_SHAPE;
     {
         uint64_t at = head_cells;
-        for (SliceDesc& d : slices) { d.off = (uint32_t)at; at += (uint64_t)(d.G - 1) * kSubRows; }
+        for (SliceDesc& d : slices) {
+            d.off = (uint32_t)at;
+            at += (uint64_t)(d.G > (uint32_t)kHeadGroups ? d.G - kHeadGroups : 0u) * kSubRows;
+        }
     }
 
     // ---- static split of every colour phase over the CTAs of the persistent grid.  Cost unit: one
@@ -701,6 +706,8 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
                 a.best_sweep_out = p->sm.best_sweep + (size_t)t0 * kTile;
                 a.barrier = p->sm.barrier;
                 a.resume = s0 > 0 ? 1 : 0;
+                a.timing = (t0 == 0 && s0 == 0) ? p->timing : nullptr;
+                a.timing_sweep = p->timing_sweep;
                 a.keys = keys;
                 void* args[] = {&a};
                 CK(cudaLaunchCooperativeKernel((const void*)k_anneal_gs, dim3(p->n_cta), dim3(kSweepThreads), args, 0, st));
@@ -895,6 +902,14 @@ ising_status ising_problem_info(const ising_problem* p, int32_t what, int64_t* v
         case 12: *value_out = p->n_cta; break;
         default: return ISING_ERR_BAD_SHAPE;
     }
+    return ISING_OK;
+}
+
+ising_status ising_debug_phase_timing(ising_problem* p, uint64_t* stamps, int32_t sweep) {
+    if (!p) return ISING_ERR_NULL_ARG;
+    if (sweep < 0 || (stamps && !is_device_ptr(stamps))) return ISING_ERR_BAD_SHAPE;
+    p->timing = (unsigned long long*)stamps;
+    p->timing_sweep = (uint32_t)sweep;
     return ISING_OK;
 }
 

@@ -87,18 +87,26 @@ __device__ __forceinline__ uint32_t lt4(const uint4& u, uint32_t thr) {
 
 // Flip decisions of Algorithm 2 (L177) for the 16 replicas rep_lane0 .. rep_lane0+15 of spin
 // `orig` in sweep T: bit j set <=> philox(seed; ctr=(orig, T, r>>2, FLIP))[r&3] < thr, r = rep_lane0 + j.
-__device__ __forceinline__ uint32_t flip_mask16(uint32_t orig, uint32_t T, uint32_t rep_lane0, uint32_t thr,
-                                                const PhiloxKeys& keys) {
+// The 16 replicas span 4 Philox calls (5 when first_replica is not a multiple of 4).  The `spr`
+// lanes that share a row split the calls among themselves: lane part q takes calls q, q+spr, ...;
+// the partial masks are OR-ed by the caller's segmented reduction (finish_flip_mask after it).
+__device__ __forceinline__ uint32_t flip_mask_part(uint32_t orig, uint32_t T, uint32_t rep_lane0, uint32_t thr,
+                                                   uint32_t q, uint32_t spr, const PhiloxKeys& keys) {
     if (thr == 0) return 0u;
-    const uint32_t cw = rep_lane0 >> 2, mis = rep_lane0 & 3u;
+    const uint32_t cw = rep_lane0 >> 2;
+    const uint32_t ncalls = (rep_lane0 & 3u) ? 5u : 4u;
     uint32_t m = 0;
+    if (spr == 1 && ncalls == 4) {
 #pragma unroll
-    for (int k = 0; k < 4; ++k) m |= lt4(philox4x32_10(orig, T, cw + k, kDomainFlip, keys), thr) << (4 * k);
-    if (mis) {   // first_replica not a multiple of 4: the 16 replicas straddle five Philox calls
-        m |= lt4(philox4x32_10(orig, T, cw + 4, kDomainFlip, keys), thr) << 16;
-        m = (m >> mis) & 0xffffu;
+        for (int k = 0; k < 4; ++k) m |= lt4(philox4x32_10(orig, T, cw + k, kDomainFlip, keys), thr) << (4 * k);
+    } else {
+        for (uint32_t k = q; k < ncalls; k += spr)
+            m |= lt4(philox4x32_10(orig, T, cw + k, kDomainFlip, keys), thr) << (4 * k);
     }
     return m;
+}
+__device__ __forceinline__ uint32_t finish_flip_mask(uint32_t m, uint32_t rep_lane0) {
+    return (m >> (rep_lane0 & 3u)) & 0xffffu;
 }
 
 template <typename AccT>
@@ -127,10 +135,22 @@ struct PassCtx {
     int32_t tie_rule;
 };
 
-// a4-a7 for one row and this lane's 16 replicas.
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+    uint32_t r;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(sel));
+    return r;
+}
+// byte b of the result = 0xff if v_b < 0 else 0x00 (PRMT sign replication of the top bytes)
+__device__ __forceinline__ uint32_t sign_bytes(int v0, int v1, int v2, int v3) {
+    const uint32_t t0 = prmt((uint32_t)v0, (uint32_t)v1, 0xfbfbu);
+    const uint32_t t1 = prmt((uint32_t)v2, (uint32_t)v3, 0xfbfbu);
+    return prmt(t0, t1, 0x5410u);
+}
+
+// a4-a7 for one row and this lane's 16 replicas, four replicas (one word of spin bytes) at a time.
 template <int KIND, typename AccT>
-__device__ __forceinline__ void row_update(const PassCtx& x, const int (&h)[16], const uint4& so4, uint32_t flip16,
-                                           size_t row_off, AccT (&acc)[16]) {
+__device__ __forceinline__ void row_update(const PassCtx& x, const int (&h)[16], const uint4& so4, uint4 bold,
+                                           uint32_t flip16, size_t row_off, AccT (&acc)[16]) {
     const uint32_t so[4] = {so4.x, so4.y, so4.z, so4.w};
     if (KIND == kKindEval) {
 #pragma unroll
@@ -142,44 +162,61 @@ __device__ __forceinline__ void row_update(const PassCtx& x, const int (&h)[16],
     uint32_t nv[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        uint32_t word = 0;
+        // a4 (L47-49, reading Q1/Q3): +1 (0x01) where h < 0, else -1 (0xff)
+        uint32_t a = ~sign_bytes(h[4 * k], h[4 * k + 1], h[4 * k + 2], h[4 * k + 3]) | 0x01010101u;
+        if (x.tie_rule == 1) {   // KEEP: h == 0 leaves the spin as it is
+            uint32_t z = 0;
 #pragma unroll
-        for (int b = 0; b < 4; ++b) {
-            const int hv = h[4 * k + b];
-            const int sold = sbyte(so[k], b);
-            int a = hv < 0 ? 1 : -1;
-            if (x.tie_rule == 1 && hv == 0) a = sold;
-            if ((flip16 >> (4 * k + b)) & 1u) a = -a;
-            if (KIND == kKindGS) acc[4 * k + b] += (AccT)(a - sold) * (AccT)hv;
-            else acc[4 * k + b] += (AccT)sold * (AccT)hv;
-            word |= ((uint32_t)a & 0xffu) << (8 * b);
+            for (int b = 0; b < 4; ++b) z |= h[4 * k + b] == 0 ? (0xffu << (8 * b)) : 0u;
+            a = (a & ~z) | (so[k] & z);
         }
-        nv[k] = word;
+        // a5 (Alg. 2): negate the bytes whose flip bit is set (+1 <-> -1 is xor 0xfe)
+        const uint32_t f4 = (flip16 >> (4 * k)) & 15u;
+        a ^= ((f4 * 0x00204081u) & 0x01010101u) * 0xfeu;
+        nv[k] = a;
+        if (KIND == kKindGS) {
+            // a7: dE = (a - s) h; a - s is +-2 exactly where the byte changed (a ^ s == 0xfe)
+            const uint32_t d2 = (a << 1) & (a ^ so[k]);
+#pragma unroll
+            for (int b = 0; b < 4; ++b) acc[4 * k + b] += (AccT)sbyte(d2, b) * (AccT)h[4 * k + b];
+        } else {
+#pragma unroll
+            for (int b = 0; b < 4; ++b) acc[4 * k + b] += (AccT)sbyte(so[k], b) * (AccT)h[4 * k + b];
+        }
     }
     *reinterpret_cast<uint4*>(x.dst + row_off) = make_uint4(nv[0], nv[1], nv[2], nv[3]);
     if (KIND == kKindGS && x.cap16 != 0u) {
         // fused best-state capture: the value this row held after the previous sweep
+        // (bold = the captured row as loaded by the caller when the mask is partial)
         uint4* bp = reinterpret_cast<uint4*>(x.best + row_off);
         if (x.cap16 == 0xffffu) {
             *bp = so4;
         } else {
-            uint4 b = __ldcg(bp);
             const uint32_t k0 = nibble_to_bytemask(x.cap16 & 15u), k1 = nibble_to_bytemask((x.cap16 >> 4) & 15u);
             const uint32_t k2 = nibble_to_bytemask((x.cap16 >> 8) & 15u), k3 = nibble_to_bytemask((x.cap16 >> 12) & 15u);
-            b.x = (so4.x & k0) | (b.x & ~k0);
-            b.y = (so4.y & k1) | (b.y & ~k1);
-            b.z = (so4.z & k2) | (b.z & ~k2);
-            b.w = (so4.w & k3) | (b.w & ~k3);
-            *bp = b;
+            bold.x = (so4.x & k0) | (bold.x & ~k0);
+            bold.y = (so4.y & k1) | (bold.y & ~k1);
+            bold.z = (so4.z & k2) | (bold.z & ~k2);
+            bold.w = (so4.w & k3) | (bold.w & ~k3);
+            *bp = bold;
         }
     }
+}
+
+// Early load of the captured row for a partial capture mask (row_update merges into it).
+template <int KIND>
+__device__ __forceinline__ uint4 ld_best_early(const PassCtx& x, bool owner, size_t row_off) {
+    uint4 b = make_uint4(0u, 0u, 0u, 0u);
+    if (KIND == kKindGS && owner && x.cap16 != 0u && x.cap16 != 0xffffu)
+        b = __ldcg(reinterpret_cast<const uint4*>(x.best + row_off));
+    return b;
 }
 
 // Everything a warp needs to start a slice; addressed by the slice index alone.
 struct SliceHead {
     SliceDesc d;
-    int4 c;
-    uint32_t w;
+    int4 c0, c1;       // head cells (groups 0 and 1)
+    uint32_t w0, w1;
     uint32_t orig;
 };
 
@@ -188,10 +225,12 @@ __device__ __forceinline__ SliceHead fetch_head(const GraphView& g, uint32_t s, 
     SliceHead h;
     const int4 dd = ld_stream(reinterpret_cast<const int4*>(g.slices + s));
     h.d.off = (uint32_t)dd.x; h.d.row0 = (uint32_t)dd.y; h.d.G = (uint32_t)dd.z; h.d.meta = (uint32_t)dd.w;
-    const size_t at = (size_t)s * kSubRows + sr;
-    h.c = ld_stream(g.col4 + at);
-    h.w = WIDE ? 0u : ld_stream(g.w4 + at);
-    h.orig = ld_stream(g.sorig + at);
+    const size_t at = (size_t)s * (kHeadGroups * kSubRows) + sr;
+    h.c0 = ld_stream(g.col4 + at);
+    h.c1 = ld_stream(g.col4 + at + kSubRows);
+    h.w0 = WIDE ? 0u : ld_stream(g.w4 + at);
+    h.w1 = WIDE ? 0u : ld_stream(g.w4 + at + kSubRows);
+    h.orig = ld_stream(g.sorig + (size_t)s * kSubRows + sr);
     return h;
 }
 
@@ -202,48 +241,60 @@ __device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x,
     const SliceDesc d = hd.d;
     const int log_spr = (int)(d.meta & 0xffu);
     const int nrows = (int)(d.meta >> 8);
+    const uint32_t spr = 1u << log_spr;
     const int rloc = sr >> log_spr;
-    const bool owner = ((sr & ((1 << log_spr) - 1)) == 0) && rloc < nrows;
+    const bool owner = ((sr & (int)(spr - 1)) == 0) && rloc < nrows;
     const size_t row_off = (size_t)(d.row0 + (uint32_t)rloc) * kTile;
+    const size_t head_at = (size_t)s * (kHeadGroups * kSubRows) + sr;
+
+    // both head groups' gathers go out at once; everything else below overlaps their latency
+    uint4 e0 = ld_nbr(x.src, hd.c0.x), e1 = ld_nbr(x.src, hd.c0.y), e2 = ld_nbr(x.src, hd.c0.z), e3 = ld_nbr(x.src, hd.c0.w);
+    uint4 f0 = ld_nbr(x.src, hd.c1.x), f1 = ld_nbr(x.src, hd.c1.y), f2 = ld_nbr(x.src, hd.c1.z), f3 = ld_nbr(x.src, hd.c1.w);
+    uint4 so4 = make_uint4(0u, 0u, 0u, 0u);
+    if (owner) so4 = ld_spin(x.src + row_off);
+    const uint4 bold = ld_best_early<KIND>(x, owner, row_off);
+    int4 ww0 = make_int4(0, 0, 0, 0), ww1 = ww0;
+    if (WIDE) { ww0 = ld_stream(g.w4w + head_at); ww1 = ld_stream(g.w4w + head_at + kSubRows); }
+    // tail cells (groups >= 2, rows of more than 128 edges only)
+    const int4* cp = g.col4 + d.off + sr;
+    const uint32_t* wp = g.w4 + d.off + sr;
+    const int4* wwp = g.w4w + d.off + sr;
+    int4 c = make_int4(-1, -1, -1, -1), ww = make_int4(0, 0, 0, 0);
+    uint32_t w = 0;
+    if (d.G > kHeadGroups) {
+        c = ld_stream(cp);
+        if (WIDE) ww = ld_stream(wwp); else w = ld_stream(wp);
+    }
+    uint32_t flip = 0;
+    if (KIND != kKindEval && hd.orig != 0xffffffffu)
+        flip = flip_mask_part(hd.orig, x.T, x.rep_lane0, x.thr, (uint32_t)sr & (spr - 1), spr, keys);
 
     int h[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) h[k] = 0;
-    int4 c = hd.c;
-    uint32_t w = hd.w;
-    const int4* cp = g.col4 + d.off + sr;
-    const uint32_t* wp = g.w4 + d.off + sr;
-    const int4* wwp = g.w4w + d.off + sr;
-    int4 ww = make_int4(0, 0, 0, 0);
-    if (WIDE) ww = ld_stream(g.w4w + (size_t)s * kSubRows + sr);
-
-    uint4 e0 = ld_nbr(x.src, c.x), e1 = ld_nbr(x.src, c.y), e2 = ld_nbr(x.src, c.z), e3 = ld_nbr(x.src, c.w);
-    uint4 so4 = make_uint4(0u, 0u, 0u, 0u);
-    if (owner) so4 = ld_spin(x.src + row_off);
-    uint32_t flip16 = 0;
-    if (KIND != kKindEval && owner) flip16 = flip_mask16(hd.orig, x.T, x.rep_lane0, x.thr, keys);
-
-    for (uint32_t gi = 1;; ++gi) {
+    if (WIDE) field_cell_wide(h, e0, e1, e2, e3, ww0); else field_cell(h, e0, e1, e2, e3, hd.w0);
+    if (d.G > 1) {
+        if (WIDE) field_cell_wide(h, f0, f1, f2, f3, ww1); else field_cell(h, f0, f1, f2, f3, hd.w1);
+    }
+    for (uint32_t gi = kHeadGroups; gi < d.G; ++gi) {
+        e0 = ld_nbr(x.src, c.x); e1 = ld_nbr(x.src, c.y); e2 = ld_nbr(x.src, c.z); e3 = ld_nbr(x.src, c.w);
         const uint32_t wc = w;
         const int4 wwc = ww;
-        const bool more = gi < d.G;
-        if (more) {   // indices of the next group while the gathers fly
-            c = ld_stream(cp + (size_t)(gi - 1) * kSubRows);
-            if (WIDE) ww = ld_stream(wwp + (size_t)(gi - 1) * kSubRows);
-            else w = ld_stream(wp + (size_t)(gi - 1) * kSubRows);
+        if (gi + 1 < d.G) {   // indices of the next group while the gathers fly
+            c = ld_stream(cp + (size_t)(gi + 1 - kHeadGroups) * kSubRows);
+            if (WIDE) ww = ld_stream(wwp + (size_t)(gi + 1 - kHeadGroups) * kSubRows);
+            else w = ld_stream(wp + (size_t)(gi + 1 - kHeadGroups) * kSubRows);
         }
-        if (WIDE) field_cell_wide(h, e0, e1, e2, e3, wwc);
-        else field_cell(h, e0, e1, e2, e3, wc);
-        if (!more) break;
-        e0 = ld_nbr(x.src, c.x); e1 = ld_nbr(x.src, c.y); e2 = ld_nbr(x.src, c.z); e3 = ld_nbr(x.src, c.w);
+        if (WIDE) field_cell_wide(h, e0, e1, e2, e3, wwc); else field_cell(h, e0, e1, e2, e3, wc);
     }
 
-    // warp-level segmented reduction over the sub-rows of one row
+    // warp-level segmented reduction over the sub-rows of one row (fields add, flip bits OR)
     for (int lvl = 0; lvl < log_spr; ++lvl) {
 #pragma unroll
         for (int k = 0; k < 16; ++k) h[k] += __shfl_xor_sync(0xffffffffu, h[k], 2 << lvl);
+        flip |= __shfl_xor_sync(0xffffffffu, flip, 2 << lvl);
     }
-    if (owner) row_update<KIND>(x, h, so4, flip16, row_off, acc);
+    if (owner) row_update<KIND>(x, h, so4, bold, finish_flip_mask(flip, x.rep_lane0), row_off, acc);
 }
 
 // One (hub, tile) unit, whole CTA.  s_hub: [kWarpsPerCta][32] ints of the buffer of this hub's
@@ -265,9 +316,11 @@ __device__ __forceinline__ void hub_pass(const GraphView& g, const PassCtx& x, c
     else w = ld_stream(g.w4 + j);
     uint4 so4 = make_uint4(0u, 0u, 0u, 0u);
     if (owner) so4 = ld_spin(x.src + row_off);
+    const uint4 bold = ld_best_early<KIND>(x, owner, row_off);
     uint4 e0 = ld_nbr(x.src, c.x), e1 = ld_nbr(x.src, c.y), e2 = ld_nbr(x.src, c.z), e3 = ld_nbr(x.src, c.w);
-    uint32_t flip16 = 0;
-    if (KIND != kKindEval && owner) flip16 = flip_mask16(hd.orig, x.T, x.rep_lane0, x.thr, keys);
+    uint32_t flip = 0;
+    if (KIND != kKindEval && epi_warp)   // the 16 sub-row lane pairs of the epilogue warp share the Philox calls
+        flip = flip_mask_part(hd.orig, x.T, x.rep_lane0, x.thr, (uint32_t)sr, (uint32_t)kSubRows, keys);
     for (uint32_t gi = 1;; ++gi) {
         const uint32_t wc = w;
         const int4 wwc = ww;
@@ -286,6 +339,7 @@ __device__ __forceinline__ void hub_pass(const GraphView& g, const PassCtx& x, c
     for (int lvl = 0; lvl < 4; ++lvl) {
 #pragma unroll
         for (int k = 0; k < 16; ++k) h[k] += __shfl_xor_sync(0xffffffffu, h[k], 2 << lvl);
+        flip |= __shfl_xor_sync(0xffffffffu, flip, 2 << lvl);
     }
     if (sr == 0) {
 #pragma unroll
@@ -303,7 +357,7 @@ __device__ __forceinline__ void hub_pass(const GraphView& g, const PassCtx& x, c
                 h[k] += v.x; h[k + 1] += v.y; h[k + 2] += v.z; h[k + 3] += v.w;
             }
         }
-        row_update<KIND>(x, h, so4, flip16, row_off, acc);
+        row_update<KIND>(x, h, so4, bold, finish_flip_mask(flip, x.rep_lane0), row_off, acc);
     }
 }
 
@@ -431,24 +485,30 @@ struct AnnealParams {
     int32_t* best_sweep_out;        // [tiles*32]
     unsigned int* barrier;          // zero at launch
     int32_t resume;                 // 1: best_out / best_sweep_out hold the bests of the sweeps before this chunk
+    unsigned long long* timing;     // diagnostics: [n_phases][n_cta][2] SM-clock stamps of sweep timing_sweep, or nullptr
+    uint32_t timing_sweep;
     PhiloxKeys keys;
 };
 
-__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& epoch, unsigned int n_cta) {
+// Grid barrier of the persistent kernel (all CTAs co-resident: cooperative launch).  One
+// release-add per CTA on a monotone counter, acquire-polled by thread 0; bar.sync on both sides
+// extends the ordering to the whole CTA (PTX memory model: causality order is cumulative).
+__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& epoch, unsigned int n_cta,
+                                             unsigned long long* stamp) {
     __syncthreads();
     epoch += n_cta;
+    if (stamp && threadIdx.x == 0) stamp[0] = (unsigned long long)clock64();
     if (n_cta > 1) {
         if (threadIdx.x == 0) {
-            __threadfence();
-            atomicAdd(counter, 1u);
+            asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
             unsigned int v;
             do {
                 asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
             } while ((int)(v - epoch) < 0);
-            __threadfence();
         }
         __syncthreads();
     }
+    if (stamp && threadIdx.x == 0) stamp[1] = (unsigned long long)clock64();
 }
 
 __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealParams p) {
@@ -564,7 +624,8 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                     }
                 }
             }
-            grid_barrier(p.barrier, epoch, n_cta);
+            grid_barrier(p.barrier, epoch, n_cta,
+                         (p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + blockIdx.x) * 2 : nullptr);
         }
 
         // sweep end (every CTA redundantly): E, cut = (W - E)/2 (eq. 4), improved mask
