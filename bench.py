@@ -329,21 +329,37 @@ def main():
     edge_visits = wl.nnz * R * M * args.steps * world
     value = spin_updates / t_total
 
-    # roofline of the dominant kernel (the sparse sweep; one launch per colour phase).  The anneal
-    # time is charged ENTIRELY to the sweep launches (it also contains the sweep-end kernels), so
-    # `achieved` is a lower bound for the kernel itself.
+    # roofline of the dominant kernel: k_anneal_gs, the persistent Gauss-Seidel kernel -- ONE launch
+    # per ising_anneal call (per <= 1024 replicas) runs all M sweeps x colour phases.  Its duration is
+    # taken as the CUDA-event time of the whole ising_anneal call (which also holds the spin init,
+    # the initial-energy pass and two tiny kernels), so `achieved` is a lower bound for the kernel.
     peak, peak_src = measured_peaks()
     n_phase = max(1, wl.n_colours) if wl.mode == "gs" else 1
-    sweep_launches = n_phase * M * args.steps
-    avg_launch_s = sum(times) / sweep_launches
-    bytes_per_launch = algorithmic_bytes_per_sweep(wl.n, wl.nnz, R) / n_phase
+    persistent = wl.mode == "gs"
+    launches_per_step = 1 if persistent else M
+    avg_launch_s = sum(times) / (args.steps * launches_per_step)
+    bytes_per_launch = algorithmic_bytes_per_sweep(wl.n, wl.nnz, R) * (M if persistent else 1)
     achieved = bytes_per_launch / avg_launch_s / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            tj = json.load(open(tpath)).get(wl.name)
+            if tj:
+                traffic = tj["dram_bytes_per_sweep"] * (M if persistent else 1)
+        except Exception:
+            traffic = None
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "kernel": "k_sweep<GS> (one launch per colour phase)",
+                "traffic": traffic,
+                "kernel": "k_anneal_gs (persistent cooperative kernel: %d sweeps x %d colour phases per launch)" % (
+                    M, n_phase) if persistent else "k_sweep<Jacobi> (one launch per sweep)",
                 "bytes_per_launch": bytes_per_launch, "avg_launch_us": avg_launch_s * 1e6,
+                "us_per_sweep": 1e6 * sum(times) / (args.steps * M),
                 "peak_source": peak_src,
-                "note": "algorithmic bytes = nnz*37 + n*68 per 32-replica tile per sweep (SURVEY 8(d)); "
-                        "denominator time = whole ising_anneal time / sweep launches (lower bound)"}
+                "note": "algorithmic bytes = (nnz*37 + n*68) per 32-replica tile per sweep (SURVEY 8(d)) x sweeps per "
+                        "launch; the 32 B gathered per edge come from L2 (spin state is L2-resident), so frac can "
+                        "exceed what HBM alone would allow; traffic = ncu dram bytes per sweep (profiles/traffic.json) "
+                        "x sweeps per launch"}
 
     e2e = None
     if not args.no_e2e:
@@ -387,7 +403,7 @@ def main():
             "config": {"workload": wl.name, "n": wl.n, "nnz": wl.nnz, "replicas_per_gpu": R, "sweeps": M,
                        "colours": wl.n_colours, "mode": wl.mode, "parallelism": "replicas-only x%d" % world,
                        "l2": "256 MiB buffer rewritten between timed steps (L2 flush); working set 148 MB > L2",
-                       "step": "one ising_anneal call: init + %d sweeps x %d colour phases + per-sweep cut/best capture" % (
+                       "step": "one ising_anneal call: init + %d sweeps x %d colour phases + per-sweep cut/trace/best capture" % (
                            M, n_phase)},
             "edge_visits_per_s": edge_visits / t_total,
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches,

@@ -292,3 +292,48 @@ def test_run_twice_is_bit_identical():
     a = gpu_anneal(wl)
     b = gpu_anneal(wl, problem=a["problem"])
     assert_same(a, b)
+
+
+# ---------------------------------------------------------------------------------------------
+# persistent-kernel corner cases: hub rows x several replica tiles x ragged replica count, more
+# replicas than one persistent launch holds (1024), schedules longer than one threshold chunk
+# ---------------------------------------------------------------------------------------------
+def test_hub_rows_with_several_tiles_and_ragged_replicas():
+    wl = W.config5(n=12000, sweeps=12, replicas=75)
+    deg = np.diff(wl.row_ptr)
+    assert (deg > 256).sum() > 5 and deg.max() > 1024     # CTA-wide hub rows, several groups each
+    g = gpu_anneal(wl)
+    o = oracle_anneal(wl)
+    assert_same(g, o)
+    # Jacobi and evaluation share the hub pass
+    g = gpu_anneal(wl, mode=P.ISING_MODE_JACOBI, thr=wl.thr[:5], n_replicas=40)
+    o = oracle_anneal(wl, mode=1, thr=wl.thr[:5], n_replicas=40)
+    assert_same(g, o)
+
+
+def test_more_replicas_than_one_persistent_launch():
+    wl = er_workload(300, 0.05, 23, "pm4", np.int8, 1100, 6, p0=0.3)
+    g = gpu_anneal(wl, want_best_spins=False)
+    o = oracle_anneal(wl)
+    assert_same(g, o, best_spins=False)
+    s, cut, sweep, rep = P.ising_best_state(g["problem"], 1077)
+    np.testing.assert_array_equal(s.cpu().numpy(), o["best_spins"][1077])
+
+
+def test_schedule_longer_than_one_threshold_chunk():
+    wl = er_workload(24, 0.3, 29, "pm1", np.int8, 3, 70000, p0=0.05)
+    g = gpu_anneal(wl)
+    o = oracle_anneal(wl)
+    assert_same(g, o)
+
+
+def test_phase_timing_diagnostics_do_not_change_results():
+    wl = W.config5(n=8000, sweeps=6, replicas=32)
+    p = P.load_workload(wl)
+    stamps = p.phase_timing(2)
+    g = gpu_anneal(wl, problem=p)
+    o = oracle_anneal(wl)
+    assert_same(g, o)
+    t = stamps.cpu().numpy()
+    assert t.shape == (wl.n_colours, p.info(12), 2)
+    assert (t[:, :, 1] >= t[:, :, 0]).all() and (t[:, :, 0] > 0).all()
