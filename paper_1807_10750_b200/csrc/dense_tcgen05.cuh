@@ -1,14 +1,297 @@
-// Dense local-field engine for fully connected instances -- interface.
-// (placeholder until the tcgen05 kernel lands: kDenseEnabled = false keeps K_n on the sparse path)
+// Dense local-field engine for fully connected instances.
+//
+// For K_n the local fields of all replicas are one int8 contraction H = J . S (eq. (2), for
+// every spin and replica at once; general connectivity L57, Fig. 2 L61): J [n][n] symmetric int8 with zero
+// diagonal, S [n][R] spins.  It runs on the 5th-generation tensor cores: tcgen05.mma.kind::i8 issued by
+// one thread, both operands K-major in shared memory (A = J rows, B = S^T rows, i.e. the state is kept
+// replica-major [R][n] so that K = the neighbour index is contiguous), fed by TMA
+// (cp.async.bulk.tensor, 128-byte swizzle) through an mbarrier ring, int32 accumulators in TMEM.
+// The epilogue reads the accumulators with tcgen05.ld (one thread = one spin i, 16 replicas at a time)
+// and fuses a4-a7: energy-minimising value, Philox flip, int8 store of the next state (synchronous
+// Jacobi: into the other buffer) and sum_i s_i h_i = 2 E(s) per replica.
+//
+// One launch = one Jacobi sweep (every sweep needs the complete previous state); one CTA = one
+// 128 (spins) x 256 (replicas) output tile, K = n in blocks of 128.
 #pragma once
-#include "common.cuh"
+#include <cuda.h>
+
 #include "../../include/ising.h"
+#include "common.cuh"
+#include "sparse_sweep.cuh"
 
 namespace ising {
 
-constexpr bool kDenseEnabled = false;
+constexpr bool kDenseEnabled = true;
+constexpr int kDM = 128;        // spins per tile (UMMA M)
+constexpr int kDN = 256;        // replicas per tile (UMMA N)
+constexpr int kDK = 128;        // K bytes per pipeline stage (one 128-byte swizzle row)
+constexpr int kDStages = 4;
+constexpr int kDThreads = 192;  // warp 0 TMA, warp 1 MMA, warps 2-5 epilogue
+constexpr uint32_t kDStageBytesA = kDM * kDK, kDStageBytesB = kDN * kDK;
+constexpr uint32_t kDSmemBytes = kDStages * (kDStageBytesA + kDStageBytesB) + 1024 /*align*/ + 256 /*barriers*/;
 
-struct DenseEngine;
+struct DenseSweepParams {
+    const int8_t* src;     // [R_pad][n_pad] state read (also the TMA source of operand B)
+    int8_t* dst;           // [R_pad][n_pad] next state (update) -- unused for evaluation
+    long long* accum;      // [R_pad] += sum_i s_i h_i
+    int* error_flag;       // set when a pipeline wait times out
+    uint32_t n, n_pad;
+    uint32_t thr, T, rep0;
+    int32_t tie_rule;
+    int32_t update;        // 1: Jacobi sweep, 0: evaluation only
+    PhiloxKeys keys;
+};
+
+// ---- PTX wrappers ---------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// Bounded wait: a broken pipeline must not hang the GPU.
+__device__ __forceinline__ bool mbar_wait(uint64_t* bar, uint32_t parity, int* error_flag) {
+    const uint32_t addr = smem_u32(bar);
+    for (uint32_t spin = 0; spin < (1u << 24); ++spin) {
+        uint32_t done;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+        if (done) return true;
+    }
+    atomicExch(error_flag, 1);
+    return false;
+}
+__device__ __forceinline__ void tma_load_2d(const CUtensorMap* map, uint64_t* bar, void* dst, int x, int y) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y) : "memory");
+}
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr));
+}
+// K-major operand tile written by TMA with the 128-byte swizzle: rows of 128 bytes, 8-row atoms of
+// 1024 bytes stacked contiguously (stride byte offset 1024); descriptor version 1 (sm_100).
+__device__ __forceinline__ uint64_t umma_desc_k128(uint32_t smem_addr) {
+    return (uint64_t)((smem_addr & 0x3ffffu) >> 4) | ((uint64_t)(1024u >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+// kind::i8 instruction descriptor: D = S32, A = B = signed int8, both K-major, M x N.
+__host__ __device__ constexpr uint32_t umma_idesc_i8(int m, int n) {
+    return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_dense_sweep: one Jacobi sweep (or one evaluation pass) of a K_n instance.
+// grid = (n_pad / 128, R_pad / 256); CTA (bx, by) owns spins [128 bx, +128) x replicas [256 by, +256).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kDThreads, 1)
+k_dense_sweep(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_s,
+              const DenseSweepParams p) {
+    extern __shared__ uint8_t dsm_raw[];
+    uint8_t* dsm = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(dsm_raw) + 1023) & ~(uintptr_t)1023);
+    uint8_t* sm_a = dsm;                                         // [stages][128 x 128 B]
+    uint8_t* sm_b = dsm + kDStages * kDStageBytesA;              // [stages][256 x 128 B]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(dsm + kDStages * (kDStageBytesA + kDStageBytesB));
+    uint64_t* full = bars;                    // [stages] TMA -> MMA
+    uint64_t* empty = bars + kDStages;        // [stages] MMA -> TMA
+    uint64_t* acc_full = bars + 2 * kDStages; // MMA -> epilogue
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kDStages + 1);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t m0 = blockIdx.x * kDM, n0 = blockIdx.y * kDN;
+    const uint32_t num_kb = p.n_pad / kDK;
+
+    if (warp == 0 && lane == 0) {
+        for (int s = 0; s < kDStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        mbar_init(acc_full, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 2) {   // TMEM: 256 columns of int32 accumulators; this warp also frees them
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(kDN));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        if (lane == 0) {   // ---- TMA producer
+            for (uint32_t kb = 0; kb < num_kb; ++kb) {
+                const uint32_t s = kb % kDStages, ph = (kb / kDStages) & 1u;
+                if (!mbar_wait(&empty[s], ph ^ 1u, p.error_flag)) break;
+                mbar_expect_tx(&full[s], kDStageBytesA + kDStageBytesB);
+                tma_load_2d(&tm_j, &full[s], sm_a + s * kDStageBytesA, (int)(kb * kDK), (int)m0);
+                tma_load_2d(&tm_s, &full[s], sm_b + s * kDStageBytesB, (int)(kb * kDK), (int)n0);
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {   // ---- MMA issuer
+            constexpr uint32_t idesc = umma_idesc_i8(kDM, kDN);
+            bool ok = true;
+            for (uint32_t kb = 0; kb < num_kb && ok; ++kb) {
+                const uint32_t s = kb % kDStages, ph = (kb / kDStages) & 1u;
+                ok = mbar_wait(&full[s], ph, p.error_flag);
+                if (!ok) break;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint64_t da = umma_desc_k128(smem_u32(sm_a + s * kDStageBytesA));
+                const uint64_t db = umma_desc_k128(smem_u32(sm_b + s * kDStageBytesB));
+#pragma unroll
+                for (uint32_t k = 0; k < kDK / 32; ++k)   // K = 32 int8 per instruction: +32 B = +2 in the address field
+                    umma_i8(tmem_base, da + 2 * k, db + 2 * k, idesc, (kb | k) != 0u ? 1u : 0u);
+                umma_commit(&empty[s]);   // frees the stage when these MMAs have read it
+            }
+            umma_commit(acc_full);        // accumulators complete (arrives even after a time-out)
+        }
+    } else {
+        // ---- epilogue: warp q = warp & 3 owns TMEM lanes [32 q, +32) = spins m0 + 32 q + lane
+        const uint32_t q = (uint32_t)warp & 3u;
+        const uint32_t row = m0 + q * 32u + (uint32_t)lane;   // caller's vertex id (dense layout keeps caller order)
+        const bool live = row < p.n;
+        const bool ok = mbar_wait(acc_full, 0u, p.error_flag);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        if (ok) {
+            long long colsum = 0;   // this lane's column (c & 31 == lane) of the current block of 32 replicas
+#pragma unroll 1
+            for (uint32_t c0 = 0; c0 < (uint32_t)kDN; c0 += 16) {
+                uint32_t hreg[16];
+                tmem_ld16(tmem_base + ((q * 32u) << 16) + c0, hreg);
+                int sold[16];
+#pragma unroll
+                for (int j = 0; j < 16; ++j)
+                    sold[j] = (int)p.src[(size_t)(n0 + c0 + j) * p.n_pad + row];   // 32 lanes = 32 consecutive bytes
+                const uint32_t rep = p.rep0 + n0 + c0;
+                uint32_t flip16 = 0;
+                if (p.update) flip16 = finish_flip_mask(flip_mask_part(row, p.T, rep, p.thr, 0u, 1u, p.keys), rep);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const int hv = (int)hreg[j];
+                    const int so = sold[j];
+                    if (p.update) {
+                        int a = hv < 0 ? 1 : -1;                    // a4 (L47-49, Q1/Q3)
+                        if (p.tie_rule == 1 && hv == 0) a = so;
+                        if ((flip16 >> j) & 1u) a = -a;             // a5 (Alg. 2)
+                        if (!live) a = 0;
+                        p.dst[(size_t)(n0 + c0 + j) * p.n_pad + row] = (int8_t)a;   // a6: the other buffer
+                    }
+                    const int part = __reduce_add_sync(0xffffffffu, so * hv);       // a7: sum over 32 spins
+                    if (lane == (int)((c0 + j) & 31u)) colsum += part;
+                }
+                if (c0 & 16u) {   // block of 32 replicas finished
+                    if (colsum != 0)
+                        atomicAdd(reinterpret_cast<unsigned long long*>(p.accum + n0 + (c0 & ~31u) + lane),
+                                  (unsigned long long)colsum);
+                    colsum = 0;
+                }
+            }
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 2) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kDN));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Small kernels of the dense engine
+// ---------------------------------------------------------------------------------------------
+// J[i][j] = w_ij from the caller's CSR (one warp per row); J is zero elsewhere (diagonal, padding).
+__global__ void k_dense_build_j(int8_t* J, uint32_t n, uint32_t n_pad, const long long* row_ptr, const int32_t* col,
+                                const void* w, int wtype) {
+    const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (gw >= n) return;
+    for (long long e = row_ptr[gw] + lane; e < row_ptr[gw + 1]; e += 32) {
+        const int v = wtype == 1 ? (int)reinterpret_cast<const int8_t*>(w)[e] : reinterpret_cast<const int32_t*>(w)[e];
+        J[(size_t)gw * n_pad + (uint32_t)col[e]] = (int8_t)v;
+    }
+}
+
+// sparse interleaved layout (state[tile][row][32], internal rows) -> dense replica-major [R_pad][n_pad]
+__global__ void k_dense_import(int8_t* S, const uint8_t* sparse, const int32_t* perm, uint32_t n, uint32_t n_pad,
+                               unsigned long long tile_stride, int32_t n_replicas) {
+    const unsigned long long t = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;   // (row, rr)
+    const uint32_t tile = blockIdx.y;
+    if (t >= (unsigned long long)n * kTile) return;
+    const uint32_t row = (uint32_t)(t >> 5), rr = (uint32_t)(t & 31);
+    const int rep = (int)(tile * kTile + rr);
+    if (rep < n_replicas)
+        S[(size_t)rep * n_pad + (uint32_t)perm[row]] = (int8_t)sparse[(size_t)tile * tile_stride + (size_t)row * kTile + rr];
+}
+
+// dense [R_pad][n_pad] -> caller layout [R][n] (replica_sel >= 0: that one replica to out[n])
+__global__ void k_dense_export(const int8_t* S, int8_t* out, uint32_t n, uint32_t n_pad, int32_t n_replicas,
+                               int32_t replica_sel) {
+    const unsigned long long t = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (replica_sel >= 0) {
+        if (t < n) out[t] = S[(size_t)replica_sel * n_pad + t];
+        return;
+    }
+    if (t >= (unsigned long long)n * (unsigned long long)n_replicas) return;
+    const uint32_t rep = (uint32_t)(t / n), i = (uint32_t)(t % n);
+    out[t] = S[(size_t)rep * n_pad + i];
+}
+
+// Per replica (one block each): E = accum / 2, cut = (W - E)/2 (eq. 4), trace, best capture of the
+// candidate state (a7).  record_only: initial state, no candidate.
+__global__ void __launch_bounds__(256) k_dense_sweep_end(const int8_t* S, int8_t* best, long long* accum, long long* E_out,
+                                                         long long* bestcut, int32_t* best_sweep, long long* trace_row,
+                                                         uint32_t n_pad, long long W, int32_t record_only, int32_t first,
+                                                         int32_t T) {
+    const uint32_t r = blockIdx.x;
+    const long long E = accum[r] / 2;
+    const long long cut = (W - E) / 2;
+    const bool improved = !record_only && (first || cut > bestcut[r]);
+    __syncthreads();   // everyone has read accum / bestcut before thread 0 rewrites them
+    if (threadIdx.x == 0) {
+        accum[r] = 0;
+        E_out[r] = E;
+        if (!record_only && trace_row) trace_row[r] = cut;
+        if (improved) { bestcut[r] = cut; best_sweep[r] = T; }
+    }
+    if (!improved) return;
+    const uint4* src = reinterpret_cast<const uint4*>(S + (size_t)r * n_pad);
+    uint4* dst = reinterpret_cast<uint4*>(best + (size_t)r * n_pad);
+    for (uint32_t k = threadIdx.x; k < n_pad / 16; k += blockDim.x) dst[k] = src[k];
+}
+
+// ---------------------------------------------------------------------------------------------
+// Host side of the engine
+// ---------------------------------------------------------------------------------------------
+struct DenseEngine {
+    uint32_t n = 0, n_pad = 0, r_pad = 0;
+    int8_t* J = nullptr;
+    int8_t* S[2] = {nullptr, nullptr};
+    int8_t* best = nullptr;
+    long long* accum = nullptr;
+    long long* E = nullptr;
+    long long* bestcut = nullptr;
+    int32_t* best_sweep = nullptr;
+    int* error_flag = nullptr;
+    int cur = 0;
+    CUtensorMap tm_j{}, tm_s[2]{};
+};
 
 struct DenseAnnealArgs {
     int32_t tie_rule, n_replicas, first_replica;
@@ -23,13 +306,127 @@ struct DenseAnnealArgs {
     int8_t* io_stage;
 };
 
-inline size_t dense_workspace_bytes(int64_t, int64_t) { return 0; }
-inline DenseEngine* dense_create(int32_t, int32_t, void*, size_t, const long long*, const int32_t*, const void*, int,
-                                 cudaStream_t) { return nullptr; }
-inline void dense_destroy(DenseEngine*) {}
-inline ising_status dense_anneal(DenseEngine*, const DenseAnnealArgs&, cudaStream_t, int64_t*) { return ISING_ERR_CUDA; }
-inline ising_status dense_export_state(DenseEngine*, int8_t*, int32_t, bool, cudaStream_t) { return ISING_ERR_CUDA; }
-inline ising_status dense_export_one(DenseEngine*, int8_t*, int32_t, bool, cudaStream_t) { return ISING_ERR_CUDA; }
-inline ising_status dense_best_arrays(DenseEngine*, long long*, int32_t*, int32_t, cudaStream_t) { return ISING_ERR_CUDA; }
+inline uint32_t dense_round_up(uint32_t x, uint32_t m) { return (x + m - 1) / m * m; }
+
+inline size_t dense_workspace_bytes(int64_t n, int64_t max_replicas) {
+    const size_t n_pad = dense_round_up((uint32_t)n, kDK), r_pad = dense_round_up((uint32_t)max_replicas, kDN);
+    return n_pad * n_pad + 3 * r_pad * n_pad + r_pad * (8 * 3 + 4) + 4096 + 8 * 1024;
+}
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// 2-D uint8 tensor [rows][cols] (cols contiguous), box = box_rows x 128 bytes, 128-byte swizzle.
+inline bool dense_make_map(CUtensorMap* map, void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+    static PFN_encodeTiled fn = nullptr;
+    if (!fn) {
+        void* sym = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &q) != cudaSuccess || !sym) {
+            (void)cudaGetLastError();
+            return false;
+        }
+        fn = (PFN_encodeTiled)sym;
+    }
+    const cuuint64_t dims[2] = {cols, rows};
+    const cuuint64_t strides[1] = {cols};
+    const cuuint32_t box[2] = {(cuuint32_t)kDK, box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    return fn(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) ==
+           CUDA_SUCCESS;
+}
+
+inline DenseEngine* dense_create(int32_t n, int32_t max_replicas, void* mem, size_t bytes, const long long* row_ptr,
+                                 const int32_t* col, const void* w, int wtype, cudaStream_t st) {
+    DenseEngine* d = new (std::nothrow) DenseEngine();
+    if (!d) return nullptr;
+    d->n = (uint32_t)n;
+    d->n_pad = dense_round_up((uint32_t)n, kDK);
+    d->r_pad = dense_round_up((uint32_t)max_replicas, kDN);
+    uint8_t* base = (uint8_t*)mem;
+    size_t off = 0;
+    auto take = [&](size_t b) { void* p = base + off; off = (off + b + 1023) / 1024 * 1024; return p; };
+    const size_t sb = (size_t)d->r_pad * d->n_pad;
+    d->J = (int8_t*)take((size_t)d->n_pad * d->n_pad);
+    d->S[0] = (int8_t*)take(sb);
+    d->S[1] = (int8_t*)take(sb);
+    d->best = (int8_t*)take(sb);
+    d->accum = (long long*)take(8 * (size_t)d->r_pad);
+    d->E = (long long*)take(8 * (size_t)d->r_pad);
+    d->bestcut = (long long*)take(8 * (size_t)d->r_pad);
+    d->best_sweep = (int32_t*)take(4 * (size_t)d->r_pad);
+    d->error_flag = (int*)take(256);
+    bool ok = off <= bytes;
+    ok = ok && cudaMemsetAsync(d->J, 0, (size_t)d->n_pad * d->n_pad, st) == cudaSuccess;
+    ok = ok && cudaMemsetAsync(d->S[0], 0, 3 * sb, st) == cudaSuccess;   // S[0], S[1], best are adjacent
+    ok = ok && cudaMemsetAsync(d->error_flag, 0, 256, st) == cudaSuccess;
+    if (ok) {
+        k_dense_build_j<<<(unsigned)(((long long)n * 32 + 255) / 256), 256, 0, st>>>(d->J, d->n, d->n_pad, row_ptr, col, w, wtype);
+        ok = dense_make_map(&d->tm_j, d->J, d->n_pad, d->n_pad, kDM) &&
+             dense_make_map(&d->tm_s[0], d->S[0], d->r_pad, d->n_pad, kDN) &&
+             dense_make_map(&d->tm_s[1], d->S[1], d->r_pad, d->n_pad, kDN);
+        ok = ok && cudaFuncSetAttribute(k_dense_sweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDSmemBytes) == cudaSuccess;
+    }
+    if (!ok) { (void)cudaGetLastError(); delete d; return nullptr; }
+    return d;
+}
+
+inline void dense_destroy(DenseEngine* d) { delete d; }
+
+inline ising_status dense_anneal(DenseEngine* d, const DenseAnnealArgs& a, cudaStream_t st, int64_t* launches) {
+    const uint32_t R = (uint32_t)a.n_replicas;
+    const dim3 grid(d->n_pad / kDM, dense_round_up(R, kDN) / kDN);
+    if (a.import_from_sparse) {
+        d->cur = 0;
+        const size_t sb = (size_t)d->r_pad * d->n_pad;
+        if (cudaMemsetAsync(d->S[0], 0, 2 * sb, st) != cudaSuccess) return ISING_ERR_CUDA;
+        const int tiles = (a.n_replicas + kTile - 1) / kTile;
+        k_dense_import<<<dim3((unsigned)(((unsigned long long)d->n * kTile + 255) / 256), tiles), 256, 0, st>>>(
+            d->S[0], a.sparse_state, a.perm, d->n, d->n_pad, (unsigned long long)d->n * kTile, a.n_replicas);
+        ++*launches;
+    }
+    if (cudaMemsetAsync(d->accum, 0, 8 * (size_t)d->r_pad, st) != cudaSuccess) return ISING_ERR_CUDA;
+    // pass t reads s^t and yields 2 E(s^t) as a by-product; pass n_sweeps is evaluation only
+    for (int32_t t = 0; t <= a.n_sweeps; ++t) {
+        DenseSweepParams p{};
+        p.src = d->S[d->cur]; p.dst = d->S[d->cur ^ 1]; p.accum = d->accum; p.error_flag = d->error_flag;
+        p.n = d->n; p.n_pad = d->n_pad; p.rep0 = (uint32_t)a.first_replica; p.tie_rule = a.tie_rule; p.keys = a.keys;
+        p.update = t < a.n_sweeps ? 1 : 0;
+        if (p.update) { p.thr = a.thresholds[t]; p.T = (uint32_t)(a.sweep_offset + t); }
+        k_dense_sweep<<<grid, kDThreads, kDSmemBytes, st>>>(d->tm_j, d->tm_s[d->cur], p);
+        k_dense_sweep_end<<<R, 256, 0, st>>>(d->S[d->cur], d->best, d->accum, d->E, d->bestcut, d->best_sweep,
+                                            (t > 0 && a.cut_trace) ? (long long*)a.cut_trace + (size_t)(t - 1) * R : nullptr,
+                                            d->n_pad, a.W, t == 0 ? 1 : 0, t == 1 ? 1 : 0, a.sweep_offset + t - 1);
+        *launches += 2;
+        if (p.update) d->cur ^= 1;
+    }
+    int err = 0;
+    if (cudaMemcpyAsync(&err, d->error_flag, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
+        return ISING_ERR_CUDA;
+    return err ? ISING_ERR_CUDA : ISING_OK;
+}
+
+// caller layout [n_replicas][n] of the current (or best) state
+inline ising_status dense_export_state(DenseEngine* d, int8_t* out, int32_t n_replicas, bool best, cudaStream_t st) {
+    const unsigned long long total = (unsigned long long)d->n * (unsigned long long)n_replicas;
+    k_dense_export<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(best ? d->best : d->S[d->cur], out, d->n, d->n_pad,
+                                                                    n_replicas, -1);
+    return cudaGetLastError() == cudaSuccess ? ISING_OK : ISING_ERR_CUDA;
+}
+inline ising_status dense_export_one(DenseEngine* d, int8_t* out, int32_t replica, bool best, cudaStream_t st) {
+    k_dense_export<<<(unsigned)((d->n + 255) / 256), 256, 0, st>>>(best ? d->best : d->S[d->cur], out, d->n, d->n_pad, 1,
+                                                                   replica);
+    return cudaGetLastError() == cudaSuccess ? ISING_OK : ISING_ERR_CUDA;
+}
+inline ising_status dense_best_arrays(DenseEngine* d, long long* bc, int32_t* bs, int32_t R, cudaStream_t st) {
+    if (cudaMemcpyAsync(bc, d->bestcut, 8 * (size_t)R, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaMemcpyAsync(bs, d->best_sweep, 4 * (size_t)R, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+        return ISING_ERR_CUDA;
+    return ISING_OK;
+}
 
 }  // namespace ising
