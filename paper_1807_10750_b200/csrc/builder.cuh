@@ -148,9 +148,10 @@ __global__ void k_pack(const SliceDesc* slices, uint32_t n_slices, const int32_t
     }
 }
 
-// One CTA per hub: cell (g, j) holds group q = g * kHubSub + j of the hub's row.
-__global__ void k_pack_hubs(const HubDesc* hubs, uint32_t n_hubs, const int32_t* inv, const long long* row_ptr,
-                            const int32_t* col, const void* w, int wtype, int4* col4, uint32_t* w4, int4* w4w) {
+// One CTA per hub: cell (g, j) holds group q = g * kHubSub + j of the hub's row (g = 0: hub-indexed head cell).
+__global__ void k_pack_hubs(const HubDesc* hubs, uint32_t n_hubs, uint32_t hub_head, const int32_t* inv,
+                            const long long* row_ptr, const int32_t* col, const void* w, int wtype, int4* col4,
+                            uint32_t* w4, int4* w4w) {
     if (blockIdx.x >= n_hubs) return;
     const HubDesc d = hubs[blockIdx.x];
     const long long b = row_ptr[d.orig], deg = row_ptr[d.orig + 1] - b;
@@ -158,7 +159,9 @@ __global__ void k_pack_hubs(const HubDesc* hubs, uint32_t n_hubs, const int32_t*
     for (unsigned long long cell = threadIdx.x; cell < cells; cell += blockDim.x) {
         int cc[4], ww[4];
         fetch_group(inv, col, w, wtype, b, deg, (long long)cell, (int)d.row, cc, ww);
-        store_cell(col4, w4, w4w, (size_t)d.off + cell, cc, ww);
+        const size_t at = cell < (unsigned long long)kHubSub ? (size_t)hub_head + (size_t)blockIdx.x * kHubSub + cell
+                                                             : (size_t)d.off + (cell - kHubSub);
+        store_cell(col4, w4, w4w, at, cc, ww);
     }
 }
 

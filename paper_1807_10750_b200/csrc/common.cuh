@@ -18,7 +18,8 @@
 //     by the slice index alone and can be prefetched with independent loads, also across the grid
 //     barrier that separates colour phases.  Rows of up to 128 edges live entirely in head cells;
 //     groups g >= 2 (rows of 129..256 edges) sit at desc.off + (g-2)*16 + sub-row;
-//     hub cells sit at hub.off + g*256 + sub-row;
+//     group 0 of hub h sits at hub_head + h*256 + sub-row (prefetchable as well), its groups g >= 1 at
+//     hub.off + (g-1)*256 + sub-row;
 //   * spins are replica-interleaved: state[tile][row][32] int8 (+1/-1), one 32-byte
 //     sector per spin per tile of 32 replicas, so a neighbour gather is one sector and a
 //     thread pair reads it with two 16-byte loads;
@@ -38,7 +39,7 @@ constexpr int kSubRows = 16;         // sub-rows per slice (lane pairs per warp)
 constexpr int kWarpsPerCta = 16;
 constexpr int kSweepThreads = kWarpsPerCta * 32;
 constexpr int kHeadGroups = 2;       // groups of every slice stored at slice-indexed (prefetchable) positions
-constexpr int kSubRowEdges = 4 * kHeadGroups;          // a row is split until a sub-row has <= this many edges ...
+constexpr int kSubRowEdges = 16;                      // a row is split until a sub-row has <= this many edges ...
 constexpr int kHubDegree = 256;                        // ... up to 16 sub-rows; rows above this are CTA hubs
 constexpr int kHubSub = kWarpsPerCta * kSubRows;       // 256 sub-rows of a hub
 constexpr int kMaxPersistReplicas = 1024;              // replicas per persistent launch
@@ -51,7 +52,7 @@ struct SliceDesc {
 };
 
 struct HubDesc {
-    uint32_t off;    // first cell
+    uint32_t off;    // first tail cell (groups >= 1)
     uint32_t row;    // internal row
     uint32_t G;      // groups per sub-row (iterations of the CTA)
     uint32_t orig;   // caller's vertex id
@@ -74,6 +75,7 @@ struct GraphView {
     const PhaseRange* ranges;   // [n_phases][n_cta]
     uint32_t n_cta;             // CTAs the ranges were built for (== gridDim.x)
     uint32_t n_phases;
+    uint32_t hub_head;          // first hub head cell: group 0 of hub h sits at hub_head + h*256 + sub-row
 };
 
 struct SweepParams {

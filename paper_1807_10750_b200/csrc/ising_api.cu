@@ -151,7 +151,7 @@ struct ising_problem {
     SmallArrays sm{};
     DenseEngine* dense = nullptr;
     // host bookkeeping
-    uint32_t n_slices = 0, n_hubs = 0, n_phases = 1, n_cta = 1;
+    uint32_t n_slices = 0, n_hubs = 0, n_phases = 1, n_cta = 1, hub_head = 0;
     uint64_t cells = 0;
     size_t ws_used = 0;
     int cur = 0;
@@ -173,7 +173,7 @@ namespace {
 GraphView graph_view(const ising_problem* p) {
     GraphView g{};
     g.col4 = p->col4; g.w4 = p->w4; g.w4w = p->w4w; g.slices = p->slices; g.sorig = p->sorig; g.hubs = p->hubs;
-    g.ranges = p->ranges; g.n_cta = p->n_cta; g.n_phases = p->n_phases;
+    g.ranges = p->ranges; g.n_cta = p->n_cta; g.n_phases = p->n_phases; g.hub_head = p->hub_head;
     return g;
 }
 
@@ -448,8 +448,14 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         }
     }
 
-    // ---- static split of every colour phase over the CTAs of the persistent grid.  Cost unit: one
-    // CTA-wide step (16 warps x one group of gathers); a hub costs G + 3 steps, a slice (G + 2) / 16.
+    // ---- static split of every colour phase over the CTAs of the persistent grid.  Cost unit: executed
+    // warp instructions (ncu source counters, profiles/): a slice costs ~430 + 70 per group + 45 per
+    // butterfly level + 120 per dependent tail group, a hub 16 warps x (400 + 100 per group).
+    auto slice_cost = [](const SliceDesc& d) {
+        const double G = (double)d.G, l = (double)(d.meta & 0xffu);
+        return 430.0 + 70.0 * G + 45.0 * l + 120.0 * std::max(0.0, G - (double)kHeadGroups);
+    };
+    auto hub_cost = [](uint32_t G) { return (double)kWarpsPerCta * (400.0 + 100.0 * (double)G); };
     uint32_t n_cta = 1;
     for (int32_t c = 0; c < C; ++c)
         n_cta = std::max(n_cta, (slice_begin[c + 1] - slice_begin[c]) + (hub_begin[c + 1] - hub_begin[c]));
@@ -459,7 +465,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     hubs.reserve(hubs_sorted.size());
     {
         std::vector<double> load(n_cta);
-        uint64_t at = head_cells + tail_cells;
+        uint64_t at = head_cells + tail_cells + (uint64_t)hubs_sorted.size() * kHubSub;   // hub tails follow hub heads
         for (int32_t c = 0; c < C; ++c) {
             const uint32_t hb = hub_begin[c], hn = hub_begin[c + 1] - hb;
             double total = 0;
@@ -470,14 +476,14 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
                 for (uint32_t q = b; q < hn; q += n_cta) {   // round robin over degree-sorted hubs
                     HubDesc h = hubs_sorted[hb + q];
                     h.off = (uint32_t)at;
-                    at += (uint64_t)h.G * kHubSub;
-                    load[b] += (double)h.G + 3.0;
+                    at += (uint64_t)(h.G - 1) * kHubSub;
+                    load[b] += hub_cost(h.G);
                     hubs.push_back(h);
                 }
                 r.h1 = (uint32_t)hubs.size();
                 total += load[b];
             }
-            for (uint32_t q = slice_begin[c]; q < slice_begin[c + 1]; ++q) total += ((double)slices[q].G + 2.0) / kWarpsPerCta;
+            for (uint32_t q = slice_begin[c]; q < slice_begin[c + 1]; ++q) total += slice_cost(slices[q]);
             uint32_t pos = slice_begin[c];
             const uint32_t end = slice_begin[c + 1];
             double remaining = total;
@@ -487,10 +493,10 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
                 double mine = load[b];
                 r.s0 = pos;
                 if (b + 1 == n_cta) {
-                    while (pos < end) mine += ((double)slices[pos++].G + 2.0) / kWarpsPerCta;
+                    while (pos < end) mine += slice_cost(slices[pos++]);
                 } else {
                     while (pos < end) {
-                        const double cs = ((double)slices[pos].G + 2.0) / kWarpsPerCta;
+                        const double cs = slice_cost(slices[pos]);
                         if (mine + 0.5 * cs > target) break;
                         mine += cs;
                         ++pos;
@@ -512,7 +518,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     p->tiles_max = (max_replicas + kTile - 1) / kTile;
     p->W = rep.w_sum / 2; p->absw_max = rep.absw_max; p->wide = wide;
     p->n_slices = (uint32_t)slices.size(); p->n_hubs = (uint32_t)hubs.size(); p->cells = cells;
-    p->n_phases = (uint32_t)C; p->n_cta = n_cta; p->sm_count = sm_count; p->cooperative = coop != 0;
+    p->n_phases = (uint32_t)C; p->n_cta = n_cta; p->hub_head = (uint32_t)(head_cells + tail_cells); p->sm_count = sm_count; p->cooperative = coop != 0;
     p->flush_rows = wide ? 0x7fffffffu
                          : (uint32_t)std::max<int64_t>(1, ((1ll << 31) - 1) / std::max<int64_t>(1, 2 * rep.absw_max));
 
@@ -564,7 +570,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     }
     if (!hubs.empty()) {
         CKP(cudaMemcpyAsync(p->hubs, hubs.data(), sizeof(HubDesc) * hubs.size(), cudaMemcpyHostToDevice, st));
-        k_pack_hubs<<<(unsigned)hubs.size(), 256, 0, st>>>(p->hubs, (uint32_t)hubs.size(), p->inv, d_row_ptr, d_col,
+        k_pack_hubs<<<(unsigned)hubs.size(), 256, 0, st>>>(p->hubs, (uint32_t)hubs.size(), p->hub_head, p->inv, d_row_ptr, d_col,
                                                           d_w, wtype, p->col4, p->w4, p->w4w);
     }
     if (want_dense) {

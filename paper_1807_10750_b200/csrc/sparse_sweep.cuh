@@ -124,6 +124,31 @@ __device__ __forceinline__ void flush_acc(AccT (&acc)[16], long long* s_acc, int
     }
 }
 
+// Persistent kernel: a warp first reduces its lanes' increments into its own 32 shared slots
+// (plain adds by lanes 0 and 1, no atomics); the slots are folded per CTA at the end of the sweep.
+__device__ __forceinline__ void flush_warp(int (&acc)[16], long long* wacc, int lane) {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        int v = acc[k];
+        v += __shfl_xor_sync(0xffffffffu, v, 2);
+        v += __shfl_xor_sync(0xffffffffu, v, 4);
+        v += __shfl_xor_sync(0xffffffffu, v, 8);
+        v += __shfl_xor_sync(0xffffffffu, v, 16);
+        if (lane < 2) wacc[lane * 16 + k] += (long long)v;
+        acc[k] = 0;
+    }
+}
+// The warp moves on to another replica tile: hand its slots over to the CTA accumulator of the old tile.
+__device__ __forceinline__ void fold_warp(long long* wacc, long long* s_acc_tile, int lane) {
+    __syncwarp();
+    const long long v = wacc[lane];
+    if (v != 0) {
+        atomicAdd(reinterpret_cast<unsigned long long*>(s_acc_tile + lane), (unsigned long long)v);
+        wacc[lane] = 0;
+    }
+    __syncwarp();
+}
+
 // Per-unit context of a lane (tile-adjusted pointers already include the lane's half).
 struct PassCtx {
     const uint8_t* src;
@@ -177,8 +202,10 @@ __device__ __forceinline__ void row_update(const PassCtx& x, const int (&h)[16],
         if (KIND == kKindGS) {
             // a7: dE = (a - s) h; a - s is +-2 exactly where the byte changed (a ^ s == 0xfe)
             const uint32_t d2 = (a << 1) & (a ^ so[k]);
+            if (d2 != 0u) {   // at low temperature most words do not change
 #pragma unroll
-            for (int b = 0; b < 4; ++b) acc[4 * k + b] += (AccT)sbyte(d2, b) * (AccT)h[4 * k + b];
+                for (int b = 0; b < 4; ++b) acc[4 * k + b] += (AccT)sbyte(d2, b) * (AccT)h[4 * k + b];
+            }
         } else {
 #pragma unroll
             for (int b = 0; b < 4; ++b) acc[4 * k + b] += (AccT)sbyte(so[k], b) * (AccT)h[4 * k + b];
@@ -297,27 +324,45 @@ __device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x,
     if (owner) row_update<KIND>(x, h, so4, bold, finish_flip_mask(flip, x.rep_lane0), row_off, acc);
 }
 
+// Everything the CTA needs to start a hub, addressed by the hub index alone (prefetchable).
+struct HubHead {
+    HubDesc d;
+    int4 c;
+    uint32_t w;
+};
+
+template <bool WIDE>
+__device__ __forceinline__ HubHead fetch_hub_head(const GraphView& g, uint32_t hh, int warp, int sr) {
+    HubHead h;
+    const int4 v = ld_stream(reinterpret_cast<const int4*>(g.hubs + hh));
+    h.d.off = (uint32_t)v.x; h.d.row = (uint32_t)v.y; h.d.G = (uint32_t)v.z; h.d.orig = (uint32_t)v.w;
+    const size_t at = (size_t)g.hub_head + (size_t)hh * kHubSub + (size_t)(warp * kSubRows + sr);
+    h.c = ld_stream(g.col4 + at);
+    h.w = WIDE ? 0u : ld_stream(g.w4 + at);
+    return h;
+}
+
 // One (hub, tile) unit, whole CTA.  s_hub: [kWarpsPerCta][32] ints of the buffer of this hub's
 // parity (the caller alternates two buffers, so one __syncthreads per hub suffices).
 template <int KIND, bool WIDE, typename AccT>
-__device__ __forceinline__ void hub_pass(const GraphView& g, const PassCtx& x, const HubDesc& hd, int warp, int sr,
-                                         int half, int (*s_hub)[kTile], bool epi_warp, AccT (&acc)[16],
-                                         const PhiloxKeys& keys) {
+__device__ __forceinline__ void hub_pass(const GraphView& g, const PassCtx& x, const HubHead& head, uint32_t hh,
+                                         int warp, int sr, int half, int (*s_hub)[kTile], bool epi_warp,
+                                         AccT (&acc)[16], const PhiloxKeys& keys) {
+    const HubDesc hd = head.d;
     const bool owner = epi_warp && sr == 0;
     const size_t row_off = (size_t)hd.row * kTile;
-    const size_t j = (size_t)hd.off + (size_t)(warp * kSubRows + sr);
+    const size_t j = (size_t)hd.off + (size_t)(warp * kSubRows + sr);   // tail cells (groups >= 1)
     int h[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) h[k] = 0;
-    int4 c = ld_stream(g.col4 + j);
-    uint32_t w = 0;
+    int4 c = head.c;
+    uint32_t w = head.w;
     int4 ww = make_int4(0, 0, 0, 0);
-    if (WIDE) ww = ld_stream(g.w4w + j);
-    else w = ld_stream(g.w4 + j);
+    if (WIDE) ww = ld_stream(g.w4w + (size_t)g.hub_head + (size_t)hh * kHubSub + (size_t)(warp * kSubRows + sr));
+    uint4 e0 = ld_nbr(x.src, c.x), e1 = ld_nbr(x.src, c.y), e2 = ld_nbr(x.src, c.z), e3 = ld_nbr(x.src, c.w);
     uint4 so4 = make_uint4(0u, 0u, 0u, 0u);
     if (owner) so4 = ld_spin(x.src + row_off);
     const uint4 bold = ld_best_early<KIND>(x, owner, row_off);
-    uint4 e0 = ld_nbr(x.src, c.x), e1 = ld_nbr(x.src, c.y), e2 = ld_nbr(x.src, c.z), e3 = ld_nbr(x.src, c.w);
     uint32_t flip = 0;
     if (KIND != kKindEval && epi_warp)   // the 16 sub-row lane pairs of the epilogue warp share the Philox calls
         flip = flip_mask_part(hd.orig, x.T, x.rep_lane0, x.thr, (uint32_t)sr, (uint32_t)kSubRows, keys);
@@ -326,9 +371,9 @@ __device__ __forceinline__ void hub_pass(const GraphView& g, const PassCtx& x, c
         const int4 wwc = ww;
         const bool more = gi < hd.G;
         if (more) {
-            c = ld_stream(g.col4 + j + (size_t)gi * kHubSub);
-            if (WIDE) ww = ld_stream(g.w4w + j + (size_t)gi * kHubSub);
-            else w = ld_stream(g.w4 + j + (size_t)gi * kHubSub);
+            c = ld_stream(g.col4 + j + (size_t)(gi - 1) * kHubSub);
+            if (WIDE) ww = ld_stream(g.w4w + j + (size_t)(gi - 1) * kHubSub);
+            else w = ld_stream(g.w4 + j + (size_t)(gi - 1) * kHubSub);
         }
         if (WIDE) field_cell_wide(h, e0, e1, e2, e3, wwc);
         else field_cell(h, e0, e1, e2, e3, wc);
@@ -365,12 +410,6 @@ __device__ __forceinline__ PhaseRange ld_range(const PhaseRange* p) {
     const int4 v = ld_stream(reinterpret_cast<const int4*>(p));
     PhaseRange r;
     r.s0 = (uint32_t)v.x; r.s1 = (uint32_t)v.y; r.h0 = (uint32_t)v.z; r.h1 = (uint32_t)v.w;
-    return r;
-}
-__device__ __forceinline__ HubDesc ld_hub(const HubDesc* p) {
-    const int4 v = ld_stream(reinterpret_cast<const int4*>(p));
-    HubDesc r;
-    r.off = (uint32_t)v.x; r.row = (uint32_t)v.y; r.G = (uint32_t)v.z; r.orig = (uint32_t)v.w;
     return r;
 }
 
@@ -415,7 +454,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_sweep(const SweepParams p)
     for (uint32_t ph = p.phase_begin; ph < p.phase_end; ++ph) {
         const PhaseRange pr = ld_range(p.g.ranges + (size_t)ph * p.g.n_cta + blockIdx.x);
         for (uint32_t hh = pr.h0; hh < pr.h1; ++hh) {
-            const HubDesc hd = ld_hub(p.g.hubs + hh);
+            const HubHead hd = fetch_hub_head<WIDE>(p.g, hh, warp, sr);
             for (uint32_t tile = 0; tile < tiles; ++tile, ++hub_count) {
                 const bool epi = (hub_count % kWarpsPerCta) == (uint32_t)warp;
                 if (epi && tile != acc_tile) {
@@ -425,7 +464,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_sweep(const SweepParams p)
                 }
                 const PassCtx x = make_ctx(p.src, p.dst, nullptr, 0u, p.tile_stride, tile, half, p.rep0, p.thr, p.T,
                                            p.tie_rule);
-                hub_pass<KIND, WIDE>(p.g, x, hd, warp, sr, half, s_hub[hub_count & 1], epi, acc, p.keys);
+                hub_pass<KIND, WIDE>(p.g, x, hd, hh, warp, sr, half, s_hub[hub_count & 1], epi, acc, p.keys);
                 if (epi && !WIDE && ++rows_acc >= p.flush_rows) {
                     flush_acc(acc, s_acc + acc_tile * kTile, lane);
                     rows_acc = 0;
@@ -513,6 +552,8 @@ __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int
 
 __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealParams p) {
     __shared__ long long s_acc[kMaxPersistReplicas];
+    __shared__ long long s_wacc[kWarpsPerCta][kTile];
+    __shared__ uint32_t s_wtile[kWarpsPerCta];
     __shared__ long long s_E[kMaxPersistReplicas];
     __shared__ long long s_best[kMaxPersistReplicas];
     __shared__ int s_bsweep[kMaxPersistReplicas];
@@ -528,6 +569,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
         s_bsweep[i] = p.resume ? p.best_sweep_out[i] : 0;
     }
     if (threadIdx.x < kMaxPersistReplicas / kTile) s_mask[threadIdx.x] = 0u;
+    s_wacc[threadIdx.x >> 5][threadIdx.x & 31] = 0;
     __syncthreads();
 
     int acc[16];
@@ -539,7 +581,9 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     const PhaseRange* my_ranges = p.g.ranges + blockIdx.x;
     PhaseRange pr = ld_range(my_ranges);
     uint32_t nu = (pr.s1 - pr.s0) * tiles;
-    // one-slice lookahead of the static data, kept across the grid barrier
+    // one-unit lookahead of the static data (first hub, first slice), kept across the grid barrier
+    HubHead hub_nxt{};
+    if (pr.h0 < pr.h1) hub_nxt = fetch_hub_head<false>(p.g, pr.h0, warp, sr);
     bool have = (uint32_t)warp < nu;
     uint32_t nxt_s = 0, nxt_tile = 0;
     SliceHead nxt{};
@@ -558,19 +602,21 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             const PhaseRange prn = ld_range(my_ranges + (size_t)(last_phase ? 0u : ph + 1u) * n_cta);
 
             for (uint32_t hh = pr.h0; hh < pr.h1; ++hh) {
-                const HubDesc hd = ld_hub(p.g.hubs + hh);
+                const HubHead hd = hub_nxt;
+                if (hh + 1 < pr.h1) hub_nxt = fetch_hub_head<false>(p.g, hh + 1, warp, sr);
                 for (uint32_t tile = 0; tile < tiles; ++tile, ++hub_count) {
                     const bool epi = (hub_count % kWarpsPerCta) == (uint32_t)warp;
                     if (epi && tile != acc_tile) {
-                        flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                        flush_warp(acc, s_wacc[warp], lane);
+                        fold_warp(s_wacc[warp], s_acc + acc_tile * kTile, lane);
                         rows_acc = 0;
                         acc_tile = tile;
                     }
                     const PassCtx x = make_ctx(p.state, p.state, p.best, s_mask[tile], p.tile_stride, tile, half,
                                                p.rep0, thr, T, p.tie_rule);
-                    hub_pass<kKindGS, false>(p.g, x, hd, warp, sr, half, s_hub[hub_count & 1], epi, acc, p.keys);
+                    hub_pass<kKindGS, false>(p.g, x, hd, hh, warp, sr, half, s_hub[hub_count & 1], epi, acc, p.keys);
                     if (epi && ++rows_acc >= p.flush_rows) {
-                        flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                        flush_warp(acc, s_wacc[warp], lane);
                         rows_acc = 0;
                     }
                 }
@@ -588,7 +634,8 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                     nxt = fetch_head<false>(p.g, nxt_s, sr);
                 }
                 if (tile != acc_tile) {
-                    flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                    flush_warp(acc, s_wacc[warp], lane);
+                    fold_warp(s_wacc[warp], s_acc + acc_tile * kTile, lane);
                     rows_acc = 0;
                     acc_tile = tile;
                 }
@@ -596,7 +643,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                                            thr, T, p.tie_rule);
                 slice_pass<kKindGS, false>(p.g, x, cur, s, sr, acc, p.keys);
                 if (++rows_acc >= p.flush_rows) {
-                    flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                    flush_warp(acc, s_wacc[warp], lane);
                     rows_acc = 0;
                 }
             }
@@ -604,6 +651,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             // static data of this warp's first slice of the next phase: issued before the barrier
             pr = prn;
             nu = (pr.s1 - pr.s0) * tiles;
+            if (!very_last && pr.h0 < pr.h1) hub_nxt = fetch_hub_head<false>(p.g, pr.h0, warp, sr);
             have = !very_last && (uint32_t)warp < nu;
             if (have) {
                 nxt_s = pr.s0 + (uint32_t)warp / tiles;
@@ -612,11 +660,31 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             }
 
             if (last_phase) {   // a7: this sweep's energy increments -> accum slot t % 3
-                flush_acc(acc, s_acc + acc_tile * kTile, lane);
+                flush_warp(acc, s_wacc[warp], lane);
                 rows_acc = 0;
+                if (lane == 0) s_wtile[warp] = acc_tile;
                 __syncthreads();
                 long long* slot = p.accum + (size_t)(t % 3u) * nR;
-                for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {
+                if (threadIdx.x < kTile) {   // one add per replica and run of warps on the same tile
+                    long long run = 0;
+                    uint32_t run_tile = s_wtile[0];
+                    for (int wv = 0; wv < kWarpsPerCta; ++wv) {
+                        const uint32_t wt = s_wtile[wv];
+                        if (wt != run_tile) {
+                            if (run != 0)
+                                atomicAdd(reinterpret_cast<unsigned long long*>(slot + run_tile * kTile + threadIdx.x),
+                                          (unsigned long long)run);
+                            run = 0;
+                            run_tile = wt;
+                        }
+                        run += s_wacc[wv][threadIdx.x];
+                        s_wacc[wv][threadIdx.x] = 0;
+                    }
+                    if (run != 0)
+                        atomicAdd(reinterpret_cast<unsigned long long*>(slot + run_tile * kTile + threadIdx.x),
+                                  (unsigned long long)run);
+                }
+                for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {   // tile hand-overs (several tiles per warp)
                     const long long v = s_acc[i];
                     if (v != 0) {
                         atomicAdd(reinterpret_cast<unsigned long long*>(slot + i), (unsigned long long)v);
