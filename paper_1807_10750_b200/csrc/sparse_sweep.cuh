@@ -96,17 +96,37 @@ __device__ __forceinline__ uint32_t flip_mask_part(uint32_t orig, uint32_t T, ui
     const uint32_t cw = rep_lane0 >> 2;
     const uint32_t ncalls = (rep_lane0 & 3u) ? 5u : 4u;
     uint32_t m = 0;
-    if (spr == 1 && ncalls == 4) {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) m |= lt4(philox4x32_10(orig, T, cw + k, kDomainFlip, keys), thr) << (4 * k);
-    } else {
+    if (ncalls == 5) {   // rare: generic strided loop
         for (uint32_t k = q; k < ncalls; k += spr)
             m |= lt4(philox4x32_10(orig, T, cw + k, kDomainFlip, keys), thr) << (4 * k);
+    } else if (spr == 1) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) m |= lt4(philox4x32_10(orig, T, cw + k, kDomainFlip, keys), thr) << (4 * k);
+    } else if (spr == 2) {   // two independent calls per lane, straight-line so that they interleave
+        const uint4 u0 = philox4x32_10(orig, T, cw + q, kDomainFlip, keys);
+        const uint4 u1 = philox4x32_10(orig, T, cw + q + 2, kDomainFlip, keys);
+        m = (lt4(u0, thr) << (4 * q)) | (lt4(u1, thr) << (4 * q + 8));
+    } else if (q < 4) {      // one call per lane (parts 0..3 of the row)
+        m = lt4(philox4x32_10(orig, T, cw + q, kDomainFlip, keys), thr) << (4 * q);
     }
     return m;
 }
 __device__ __forceinline__ uint32_t finish_flip_mask(uint32_t m, uint32_t rep_lane0) {
     return (m >> (rep_lane0 & 3u)) & 0xffffu;
+}
+
+// Sum (or OR) over the 16 lanes of the same half (lane parity) with one REDUX per value: the even and the
+// odd lanes run their own redux.sync with their own member mask.
+__device__ __forceinline__ void half_reduce16(int (&v)[16], uint32_t& bits, int half) {
+    if (half) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) asm volatile("redux.sync.add.s32 %0, %0, 0xaaaaaaaa;" : "+r"(v[k]));
+        asm volatile("redux.sync.or.b32 %0, %0, 0xaaaaaaaa;" : "+r"(bits));
+    } else {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) asm volatile("redux.sync.add.s32 %0, %0, 0x55555555;" : "+r"(v[k]));
+        asm volatile("redux.sync.or.b32 %0, %0, 0x55555555;" : "+r"(bits));
+    }
 }
 
 template <typename AccT>
@@ -127,14 +147,11 @@ __device__ __forceinline__ void flush_acc(AccT (&acc)[16], long long* s_acc, int
 // Persistent kernel: a warp first reduces its lanes' increments into its own 32 shared slots
 // (plain adds by lanes 0 and 1, no atomics); the slots are folded per CTA at the end of the sweep.
 __device__ __forceinline__ void flush_warp(int (&acc)[16], long long* wacc, int lane) {
+    uint32_t none = 0;
+    half_reduce16(acc, none, lane & 1);
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-        int v = acc[k];
-        v += __shfl_xor_sync(0xffffffffu, v, 2);
-        v += __shfl_xor_sync(0xffffffffu, v, 4);
-        v += __shfl_xor_sync(0xffffffffu, v, 8);
-        v += __shfl_xor_sync(0xffffffffu, v, 16);
-        if (lane < 2) wacc[lane * 16 + k] += (long long)v;
+        if (lane < 2) wacc[lane * 16 + k] += (long long)acc[k];
         acc[k] = 0;
     }
 }
@@ -316,10 +333,14 @@ __device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x,
     }
 
     // warp-level segmented reduction over the sub-rows of one row (fields add, flip bits OR)
-    for (int lvl = 0; lvl < log_spr; ++lvl) {
+    if (log_spr == 4) {
+        half_reduce16(h, flip, (int)(threadIdx.x & 1));
+    } else {
+        for (int lvl = 0; lvl < log_spr; ++lvl) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) h[k] += __shfl_xor_sync(0xffffffffu, h[k], 2 << lvl);
-        flip |= __shfl_xor_sync(0xffffffffu, flip, 2 << lvl);
+            for (int k = 0; k < 16; ++k) h[k] += __shfl_xor_sync(0xffffffffu, h[k], 2 << lvl);
+            flip |= __shfl_xor_sync(0xffffffffu, flip, 2 << lvl);
+        }
     }
     if (owner) row_update<KIND>(x, h, so4, bold, finish_flip_mask(flip, x.rep_lane0), row_off, acc);
 }
@@ -380,12 +401,7 @@ __device__ __forceinline__ void hub_pass(const GraphView& g, const PassCtx& x, c
         if (!more) break;
         e0 = ld_nbr(x.src, c.x); e1 = ld_nbr(x.src, c.y); e2 = ld_nbr(x.src, c.z); e3 = ld_nbr(x.src, c.w);
     }
-#pragma unroll
-    for (int lvl = 0; lvl < 4; ++lvl) {
-#pragma unroll
-        for (int k = 0; k < 16; ++k) h[k] += __shfl_xor_sync(0xffffffffu, h[k], 2 << lvl);
-        flip |= __shfl_xor_sync(0xffffffffu, flip, 2 << lvl);
-    }
+    half_reduce16(h, flip, half);
     if (sr == 0) {
 #pragma unroll
         for (int k = 0; k < 16; k += 4)
