@@ -53,9 +53,9 @@ bool is_device_ptr(const void* p) {
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
-inline int spr_log2_for_degree(int64_t deg) {
+inline int spr_log2_for_degree(int64_t deg, int sub_row_edges) {
     int l = 0;
-    while (l < 4 && ((deg + (1ll << l) - 1) >> l) > kSubRowEdges) ++l;
+    while (l < 4 && ((deg + (1ll << l) - 1) >> l) > sub_row_edges) ++l;
     return l;
 }
 
@@ -399,7 +399,11 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     std::vector<uint32_t> slice_begin((size_t)C + 1, 0), hub_begin((size_t)C + 1, 0);
     uint64_t tail_cells = 0, hub_cells = 0;
     auto degree_of = [&](int32_t k) { return h_row_ptr[perm[k] + 1] - h_row_ptr[perm[k]]; };
-    {
+    // Edges per sub-row before a row is split over more sub-rows: 16 keeps the instruction count per edge low
+    // (throughput-bound graphs); 8 keeps every row of up to 128 edges inside the prefetched head cells, i.e. one
+    // gather round trip per phase (latency-bound graphs: fewer units in the largest phase than warps on the GPU).
+    auto build_units = [&](int sub_row_edges) {
+        slices.clear(); hubs_sorted.clear(); tail_cells = 0; hub_cells = 0;
         int32_t k = 0;
         for (int32_t c = 0; c < C; ++c) {
             slice_begin[c] = (uint32_t)slices.size();
@@ -417,10 +421,11 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
                     ++k;
                     continue;
                 }
-                const int l = spr_log2_for_degree(deg);
+                const int l = spr_log2_for_degree(deg, sub_row_edges);
                 const int rps = kSubRows >> l;
                 int nr = 1;
-                while (nr < rps && k + nr < n && h_colour[perm[k + nr]] == c && spr_log2_for_degree(degree_of(k + nr)) == l)
+                while (nr < rps && k + nr < n && h_colour[perm[k + nr]] == c &&
+                       spr_log2_for_degree(degree_of(k + nr), sub_row_edges) == l)
                     ++nr;
                 const int64_t groups = (deg + 3) / 4;
                 const int64_t G = std::max<int64_t>(1, (groups + (1ll << l) - 1) >> l);
@@ -436,7 +441,12 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         }
         slice_begin[C] = (uint32_t)slices.size();
         hub_begin[C] = (uint32_t)hubs_sorted.size();
-    }
+        uint64_t units = 0;
+        for (int32_t c = 0; c < C; ++c)
+            units = std::max<uint64_t>(units, (uint64_t)(slice_begin[c + 1] - slice_begin[c]) + (hub_begin[c + 1] - hub_begin[c]));
+        return units * (uint64_t)((max_replicas + kTile - 1) / kTile);
+    };
+    if (build_units(kSubRowEdges) < (uint64_t)sm_count * kWarpsPerCta) build_units(kHeadGroups * 4);
     const uint64_t head_cells = (uint64_t)slices.size() * kSubRows * kHeadGroups;
     const uint64_t cells = head_cells + tail_cells + hub_cells;
     if (cells > 0xffffffffull) return ISING_ERR_BAD_SHAPE;
@@ -456,10 +466,18 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         return 430.0 + 70.0 * G + 45.0 * l + 120.0 * std::max(0.0, G - (double)kHeadGroups);
     };
     auto hub_cost = [](uint32_t G) { return (double)kWarpsPerCta * (400.0 + 100.0 * (double)G); };
+    // Grid size: small graphs are latency-bound (one dependent gather chain per phase), so every (slice, tile)
+    // unit and every hub of the largest phase gets its own CTA, up to one CTA per SM (measured on configs 1-3:
+    // spreading the units beats the cheaper barrier of a smaller grid).
     uint32_t n_cta = 1;
-    for (int32_t c = 0; c < C; ++c)
-        n_cta = std::max(n_cta, (slice_begin[c + 1] - slice_begin[c]) + (hub_begin[c + 1] - hub_begin[c]));
-    n_cta = std::min<uint32_t>(n_cta, (uint32_t)std::min<int>(sm_count, (int)kMaxCtas));
+    {
+        const uint64_t tiles_max = (uint64_t)(max_replicas + kTile - 1) / kTile;
+        uint64_t units = 1;
+        for (int32_t c = 0; c < C; ++c)
+            units = std::max<uint64_t>(units, ((uint64_t)(slice_begin[c + 1] - slice_begin[c]) +
+                                               (uint64_t)(hub_begin[c + 1] - hub_begin[c])) * tiles_max);
+        n_cta = (uint32_t)std::min<uint64_t>(units, (uint64_t)std::min<int>(sm_count, (int)kMaxCtas));
+    }
     std::vector<PhaseRange> ranges((size_t)C * n_cta);
     std::vector<HubDesc> hubs;
     hubs.reserve(hubs_sorted.size());
