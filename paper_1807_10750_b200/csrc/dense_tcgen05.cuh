@@ -7,7 +7,7 @@
 // replica-major [R][n] so that K = the neighbour index is contiguous), fed by TMA
 // (cp.async.bulk.tensor, 128-byte swizzle) through an mbarrier ring, int32 accumulators in TMEM.
 // The epilogue reads the accumulators with tcgen05.ld (one thread = one spin i, 16 replicas at a time)
-// and fuses a4-a7: energy-minimising value, Philox flip, int8 store of the next state (synchronous
+// and fuses a4-a7 (16 epilogue warps: 4 lane quarters x 4 groups of 64 replicas): energy-minimising value, Philox flip, int8 store of the next state (synchronous
 // Jacobi: into the other buffer) and sum_i s_i h_i = 2 E(s) per replica.
 //
 // One launch = one Jacobi sweep (every sweep needs the complete previous state); one CTA = one
@@ -26,7 +26,8 @@ constexpr int kDM = 128;        // spins per tile (UMMA M)
 constexpr int kDN = 256;        // replicas per tile (UMMA N)
 constexpr int kDK = 128;        // K bytes per pipeline stage (one 128-byte swizzle row)
 constexpr int kDStages = 4;
-constexpr int kDThreads = 192;  // warp 0 TMA, warp 1 MMA, warps 2-5 epilogue
+constexpr int kDEpiWarps = 16;   // 4 TMEM lane quarters x 4 column groups of 64 replicas
+constexpr int kDThreads = 64 + 32 * kDEpiWarps;   // warp 0 TMA, warp 1 MMA, warps 2.. epilogue
 constexpr uint32_t kDStageBytesA = kDM * kDK, kDStageBytesB = kDN * kDK;
 constexpr uint32_t kDSmemBytes = kDStages * (kDStageBytesA + kDStageBytesB) + 1024 /*align*/ + 256 /*barriers*/;
 
@@ -162,7 +163,8 @@ k_dense_sweep(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ 
             umma_commit(acc_full);        // accumulators complete (arrives even after a time-out)
         }
     } else {
-        // ---- epilogue: warp q = warp & 3 owns TMEM lanes [32 q, +32) = spins m0 + 32 q + lane
+        // ---- epilogue: a warp may only read the TMEM lane quarter q = warp id & 3, i.e. spins m0 + 32 q + lane;
+        // the four warps that share a quarter split the 256 replicas of the tile
         const uint32_t q = (uint32_t)warp & 3u;
         const uint32_t row = m0 + q * 32u + (uint32_t)lane;   // caller's vertex id (dense layout keeps caller order)
         const bool live = row < p.n;
@@ -170,8 +172,10 @@ k_dense_sweep(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ 
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         if (ok) {
             long long colsum = 0;   // this lane's column (c & 31 == lane) of the current block of 32 replicas
+            const uint32_t cg = ((uint32_t)warp - 2u) >> 2;                      // column group of this warp
+            constexpr uint32_t kColsPerWarp = (uint32_t)kDN / (kDEpiWarps / 4);  // 64
 #pragma unroll 1
-            for (uint32_t c0 = 0; c0 < (uint32_t)kDN; c0 += 16) {
+            for (uint32_t c0 = cg * kColsPerWarp; c0 < (cg + 1u) * kColsPerWarp; c0 += 16) {
                 uint32_t hreg[16];
                 tmem_ld16(tmem_base + ((q * 32u) << 16) + c0, hreg);
                 int sold[16];
