@@ -517,6 +517,8 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_sweep(const SweepParams p)
 // k_anneal_gs: the persistent Gauss-Seidel annealer (int8 weights).  Cooperative launch,
 // grid = g.n_cta CTAs (one per SM at most), all co-resident.
 // ---------------------------------------------------------------------------------------------
+constexpr int kRangeCache = 128;   // phases whose per-CTA ranges are kept in shared memory
+
 struct AnnealParams {
     GraphView g;
     uint8_t* state;                 // [tiles][n][32], updated in place
@@ -570,6 +572,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     __shared__ long long s_acc[kMaxPersistReplicas];
     __shared__ long long s_wacc[kWarpsPerCta][kTile];
     __shared__ uint32_t s_wtile[kWarpsPerCta];
+    __shared__ PhaseRange s_ranges[kRangeCache];
     __shared__ long long s_E[kMaxPersistReplicas];
     __shared__ long long s_best[kMaxPersistReplicas];
     __shared__ int s_bsweep[kMaxPersistReplicas];
@@ -594,8 +597,15 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     uint32_t rows_acc = 0, acc_tile = 0, hub_count = 0;
     unsigned int epoch = 0;
 
+    // this CTA's work ranges of all phases: staged once in shared memory (first kRangeCache phases)
     const PhaseRange* my_ranges = p.g.ranges + blockIdx.x;
-    PhaseRange pr = ld_range(my_ranges);
+    for (uint32_t i = threadIdx.x; i < min(C, (uint32_t)kRangeCache); i += blockDim.x)
+        s_ranges[i] = ld_range(my_ranges + (size_t)i * n_cta);
+    __syncthreads();
+    auto range_of = [&](uint32_t ph_) {
+        return ph_ < (uint32_t)kRangeCache ? s_ranges[ph_] : ld_range(my_ranges + (size_t)ph_ * n_cta);
+    };
+    PhaseRange pr = range_of(0u);
     uint32_t nu = (pr.s1 - pr.s0) * tiles;
     // one-unit lookahead of the static data (first hub, first slice), kept across the grid barrier
     HubHead hub_nxt{};
@@ -615,7 +625,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
         for (uint32_t ph = 0; ph < C; ++ph) {
             const bool last_phase = ph + 1 == C;
             const bool very_last = last_phase && t + 1 == p.n_sweeps;
-            const PhaseRange prn = ld_range(my_ranges + (size_t)(last_phase ? 0u : ph + 1u) * n_cta);
+            const PhaseRange prn = range_of(last_phase ? 0u : ph + 1u);
 
             for (uint32_t hh = pr.h0; hh < pr.h1; ++hh) {
                 const HubHead hd = hub_nxt;
