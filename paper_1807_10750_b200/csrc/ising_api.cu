@@ -595,6 +595,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         p->dense = dense_create(n, max_replicas, dense_mem, dense_bytes, d_row_ptr, d_col, d_w, wtype, st);
         if (!p->dense) return fail(ISING_ERR_CUDA);
     }
+    CKP(cudaFuncSetAttribute(k_anneal_gs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
     CKP(cudaStreamSynchronize(st));   // the host vectors die at return
     CKP(cudaGetLastError());
 #undef CKP
@@ -734,7 +735,8 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
                 a.timing_sweep = p->timing_sweep;
                 a.keys = keys;
                 void* args[] = {&a};
-                CK(cudaLaunchCooperativeKernel((const void*)k_anneal_gs, dim3(p->n_cta), dim3(kSweepThreads), args, 0, st));
+                CK(cudaLaunchCooperativeKernel((const void*)k_anneal_gs, dim3(p->n_cta), dim3(kSweepThreads), args,
+                                               kAnnealDynSmem, st));
                 p->launches++;
             }
         }

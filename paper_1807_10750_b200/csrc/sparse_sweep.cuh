@@ -115,6 +115,21 @@ __device__ __forceinline__ uint32_t finish_flip_mask(uint32_t m, uint32_t rep_la
     return (m >> (rep_lane0 & 3u)) & 0xffffu;
 }
 
+// Where a lane keeps its 16 per-replica energy increments: registers (launch-per-sweep kernels), or a private
+// column of shared memory (persistent kernel: the increments are touched only where a spin changed, which is rare
+// at low temperature, and 16 registers per thread are worth more there).
+template <typename T>
+struct RegAcc {
+    using value_type = T;
+    T (&a)[16];
+    __device__ __forceinline__ void add(int i, T v) const { a[i] += v; }
+};
+struct SmemAcc {
+    using value_type = int;
+    int* p;   // &s_dE[0][thread]; element i at p[i * kSweepThreads]
+    __device__ __forceinline__ void add(int i, int v) const { p[i * kSweepThreads] += v; }
+};
+
 // Sum (or OR) over the 16 lanes of the same half (lane parity) with one REDUX per value: the even and the
 // odd lanes run their own redux.sync with their own member mask.
 __device__ __forceinline__ void half_reduce16(int (&v)[16], uint32_t& bits, int half) {
@@ -155,6 +170,12 @@ __device__ __forceinline__ void flush_warp(int (&acc)[16], long long* wacc, int 
         acc[k] = 0;
     }
 }
+__device__ __forceinline__ void flush_warp(const SmemAcc& acc, long long* wacc, int lane) {
+    int v[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { v[k] = acc.p[k * kSweepThreads]; acc.p[k * kSweepThreads] = 0; }
+    flush_warp(v, wacc, lane);
+}
 // The warp moves on to another replica tile: hand its slots over to the CTA accumulator of the old tile.
 __device__ __forceinline__ void fold_warp(long long* wacc, long long* s_acc_tile, int lane) {
     __syncwarp();
@@ -190,15 +211,16 @@ __device__ __forceinline__ uint32_t sign_bytes(int v0, int v1, int v2, int v3) {
 }
 
 // a4-a7 for one row and this lane's 16 replicas, four replicas (one word of spin bytes) at a time.
-template <int KIND, typename AccT>
+template <int KIND, typename Acc>
 __device__ __forceinline__ void row_update(const PassCtx& x, const int (&h)[16], const uint4& so4, uint4 bold,
-                                           uint32_t flip16, size_t row_off, AccT (&acc)[16]) {
+                                           uint32_t flip16, size_t row_off, const Acc& acc) {
+    using AccT = typename Acc::value_type;
     const uint32_t so[4] = {so4.x, so4.y, so4.z, so4.w};
     if (KIND == kKindEval) {
 #pragma unroll
         for (int k = 0; k < 4; ++k)
 #pragma unroll
-            for (int b = 0; b < 4; ++b) acc[4 * k + b] += (AccT)sbyte(so[k], b) * (AccT)h[4 * k + b];
+            for (int b = 0; b < 4; ++b) acc.add(4 * k + b, (AccT)sbyte(so[k], b) * (AccT)h[4 * k + b]);
         return;
     }
     uint32_t nv[4];
@@ -221,11 +243,11 @@ __device__ __forceinline__ void row_update(const PassCtx& x, const int (&h)[16],
             const uint32_t d2 = (a << 1) & (a ^ so[k]);
             if (d2 != 0u) {   // at low temperature most words do not change
 #pragma unroll
-                for (int b = 0; b < 4; ++b) acc[4 * k + b] += (AccT)sbyte(d2, b) * (AccT)h[4 * k + b];
+                for (int b = 0; b < 4; ++b) acc.add(4 * k + b, (AccT)sbyte(d2, b) * (AccT)h[4 * k + b]);
             }
         } else {
 #pragma unroll
-            for (int b = 0; b < 4; ++b) acc[4 * k + b] += (AccT)sbyte(so[k], b) * (AccT)h[4 * k + b];
+            for (int b = 0; b < 4; ++b) acc.add(4 * k + b, (AccT)sbyte(so[k], b) * (AccT)h[4 * k + b]);
         }
     }
     *reinterpret_cast<uint4*>(x.dst + row_off) = make_uint4(nv[0], nv[1], nv[2], nv[3]);
@@ -279,9 +301,9 @@ __device__ __forceinline__ SliceHead fetch_head(const GraphView& g, uint32_t s, 
 }
 
 // One (slice, tile) unit, whole warp.
-template <int KIND, bool WIDE, typename AccT>
+template <int KIND, bool WIDE, typename Acc>
 __device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x, const SliceHead& hd, uint32_t s,
-                                           int sr, AccT (&acc)[16], const PhiloxKeys& keys) {
+                                           int sr, const Acc& acc, const PhiloxKeys& keys) {
     const SliceDesc d = hd.d;
     const int log_spr = (int)(d.meta & 0xffu);
     const int nrows = (int)(d.meta >> 8);
@@ -365,10 +387,10 @@ __device__ __forceinline__ HubHead fetch_hub_head(const GraphView& g, uint32_t h
 
 // One (hub, tile) unit, whole CTA.  s_hub: [kWarpsPerCta][32] ints of the buffer of this hub's
 // parity (the caller alternates two buffers, so one __syncthreads per hub suffices).
-template <int KIND, bool WIDE, typename AccT>
+template <int KIND, bool WIDE, typename Acc>
 __device__ __forceinline__ void hub_pass(const GraphView& g, const PassCtx& x, const HubHead& head, uint32_t hh,
                                          int warp, int sr, int half, int (*s_hub)[kTile], bool epi_warp,
-                                         AccT (&acc)[16], const PhiloxKeys& keys) {
+                                         const Acc& acc, const PhiloxKeys& keys) {
     const HubDesc hd = head.d;
     const bool owner = epi_warp && sr == 0;
     const size_t row_off = (size_t)hd.row * kTile;
@@ -480,7 +502,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_sweep(const SweepParams p)
                 }
                 const PassCtx x = make_ctx(p.src, p.dst, nullptr, 0u, p.tile_stride, tile, half, p.rep0, p.thr, p.T,
                                            p.tie_rule);
-                hub_pass<KIND, WIDE>(p.g, x, hd, hh, warp, sr, half, s_hub[hub_count & 1], epi, acc, p.keys);
+                hub_pass<KIND, WIDE>(p.g, x, hd, hh, warp, sr, half, s_hub[hub_count & 1], epi, RegAcc<AccT>{acc}, p.keys);
                 if (epi && !WIDE && ++rows_acc >= p.flush_rows) {
                     flush_acc(acc, s_acc + acc_tile * kTile, lane);
                     rows_acc = 0;
@@ -498,7 +520,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_sweep(const SweepParams p)
             }
             const PassCtx x = make_ctx(p.src, p.dst, nullptr, 0u, p.tile_stride, tile, half, p.rep0, p.thr, p.T,
                                        p.tie_rule);
-            slice_pass<KIND, WIDE>(p.g, x, hd, s, sr, acc, p.keys);
+            slice_pass<KIND, WIDE>(p.g, x, hd, s, sr, RegAcc<AccT>{acc}, p.keys);
             if (!WIDE && ++rows_acc >= p.flush_rows) {
                 flush_acc(acc, s_acc + acc_tile * kTile, lane);
                 rows_acc = 0;
@@ -517,6 +539,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_sweep(const SweepParams p)
 // k_anneal_gs: the persistent Gauss-Seidel annealer (int8 weights).  Cooperative launch,
 // grid = g.n_cta CTAs (one per SM at most), all co-resident.
 // ---------------------------------------------------------------------------------------------
+constexpr size_t kAnnealDynSmem = 16 * kSweepThreads * sizeof(int);   // s_dE
 constexpr int kRangeCache = 128;   // phases whose per-CTA ranges are kept in shared memory
 
 struct AnnealParams {
@@ -573,6 +596,8 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     __shared__ long long s_wacc[kWarpsPerCta][kTile];
     __shared__ uint32_t s_wtile[kWarpsPerCta];
     __shared__ PhaseRange s_ranges[kRangeCache];
+    extern __shared__ int s_dE_raw[];         // dynamic: [16][kSweepThreads] per-thread energy increments (SmemAcc)
+    int (*s_dE)[kSweepThreads] = reinterpret_cast<int (*)[kSweepThreads]>(s_dE_raw);
     __shared__ long long s_E[kMaxPersistReplicas];
     __shared__ long long s_best[kMaxPersistReplicas];
     __shared__ int s_bsweep[kMaxPersistReplicas];
@@ -591,9 +616,9 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     s_wacc[threadIdx.x >> 5][threadIdx.x & 31] = 0;
     __syncthreads();
 
-    int acc[16];
+    const SmemAcc acc{&s_dE[0][threadIdx.x]};
 #pragma unroll
-    for (int k = 0; k < 16; ++k) acc[k] = 0;
+    for (int k = 0; k < 16; ++k) s_dE[k][threadIdx.x] = 0;
     uint32_t rows_acc = 0, acc_tile = 0, hub_count = 0;
     unsigned int epoch = 0;
 
