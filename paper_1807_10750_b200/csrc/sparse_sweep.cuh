@@ -321,15 +321,18 @@ __device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x,
     const uint4 bold = ld_best_early<KIND>(x, owner, row_off);
     int4 ww0 = make_int4(0, 0, 0, 0), ww1 = ww0;
     if (WIDE) { ww0 = ld_stream(g.w4w + head_at); ww1 = ld_stream(g.w4w + head_at + kSubRows); }
-    // tail cells (groups >= 2, rows of more than 128 edges only)
-    const int4* cp = g.col4 + d.off + sr;
-    const uint32_t* wp = g.w4 + d.off + sr;
-    const int4* wwp = g.w4w + d.off + sr;
-    int4 c = make_int4(-1, -1, -1, -1), ww = make_int4(0, 0, 0, 0);
-    uint32_t w = 0;
-    if (d.G > kHeadGroups) {
-        c = ld_stream(cp);
-        if (WIDE) ww = ld_stream(wwp); else w = ld_stream(wp);
+    // tail cells: groups 2 and 3 (a sub-row never holds more than 16 edges, so G <= 4); their indices are
+    // requested right away so that both tail gathers can follow the head groups back to back
+    const size_t tail_at = (size_t)d.off + sr;
+    int4 c2 = make_int4(0, 0, 0, 0), c3 = c2, ww2 = c2, ww3 = c2;
+    uint32_t w2 = 0, w3 = 0;
+    if (d.G > 2) {
+        c2 = ld_stream(g.col4 + tail_at);
+        if (WIDE) ww2 = ld_stream(g.w4w + tail_at); else w2 = ld_stream(g.w4 + tail_at);
+        if (d.G > 3) {
+            c3 = ld_stream(g.col4 + tail_at + kSubRows);
+            if (WIDE) ww3 = ld_stream(g.w4w + tail_at + kSubRows); else w3 = ld_stream(g.w4 + tail_at + kSubRows);
+        }
     }
     uint32_t flip = 0;
     if (KIND != kKindEval && hd.orig != 0xffffffffu)
@@ -339,19 +342,16 @@ __device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x,
 #pragma unroll
     for (int k = 0; k < 16; ++k) h[k] = 0;
     if (WIDE) field_cell_wide(h, e0, e1, e2, e3, ww0); else field_cell(h, e0, e1, e2, e3, hd.w0);
+    if (d.G > 2) { e0 = ld_nbr(x.src, c2.x); e1 = ld_nbr(x.src, c2.y); e2 = ld_nbr(x.src, c2.z); e3 = ld_nbr(x.src, c2.w); }
     if (d.G > 1) {
         if (WIDE) field_cell_wide(h, f0, f1, f2, f3, ww1); else field_cell(h, f0, f1, f2, f3, hd.w1);
     }
-    for (uint32_t gi = kHeadGroups; gi < d.G; ++gi) {
-        e0 = ld_nbr(x.src, c.x); e1 = ld_nbr(x.src, c.y); e2 = ld_nbr(x.src, c.z); e3 = ld_nbr(x.src, c.w);
-        const uint32_t wc = w;
-        const int4 wwc = ww;
-        if (gi + 1 < d.G) {   // indices of the next group while the gathers fly
-            c = ld_stream(cp + (size_t)(gi + 1 - kHeadGroups) * kSubRows);
-            if (WIDE) ww = ld_stream(wwp + (size_t)(gi + 1 - kHeadGroups) * kSubRows);
-            else w = ld_stream(wp + (size_t)(gi + 1 - kHeadGroups) * kSubRows);
+    if (d.G > 2) {
+        if (d.G > 3) { f0 = ld_nbr(x.src, c3.x); f1 = ld_nbr(x.src, c3.y); f2 = ld_nbr(x.src, c3.z); f3 = ld_nbr(x.src, c3.w); }
+        if (WIDE) field_cell_wide(h, e0, e1, e2, e3, ww2); else field_cell(h, e0, e1, e2, e3, w2);
+        if (d.G > 3) {
+            if (WIDE) field_cell_wide(h, f0, f1, f2, f3, ww3); else field_cell(h, f0, f1, f2, f3, w3);
         }
-        if (WIDE) field_cell_wide(h, e0, e1, e2, e3, wwc); else field_cell(h, e0, e1, e2, e3, wc);
     }
 
     // warp-level segmented reduction over the sub-rows of one row (fields add, flip bits OR)
