@@ -84,7 +84,7 @@ __global__ void k_validate(int32_t n, const long long* row_ptr, const int32_t* c
 }
 
 // One warp per slice: fill the cells of the slice (head cells for groups 0 and 1, tail cells for
-// the rest) and the per-sub-row caller ids.  Cell (g, sr) holds group q = g * SPR + part of row
+// the rest) and the per-sub-row caller ids (hub parts: caller id, hub id, part index).  Cell (g, sr) holds group q = g * SPR + part of row
 // row0 + (sr >> log_spr), part = sr & (SPR - 1); edges 4q .. 4q+3.
 __device__ __forceinline__ void store_cell(int4* col4, uint32_t* w4, int4* w4w, size_t at, const int (&cc)[4],
                                            const int (&ww)[4]) {
@@ -109,15 +109,39 @@ __device__ __forceinline__ void fetch_group(const int32_t* inv, const int32_t* c
     }
 }
 
-__global__ void k_pack(const SliceDesc* slices, uint32_t n_slices, const int32_t* perm, const int32_t* inv,
-                       const long long* row_ptr, const int32_t* col, const void* w, int wtype, int4* col4,
-                       uint32_t* w4, int4* w4w, uint32_t* sorig) {
+__global__ void k_pack(const SliceDesc* slices, const uint32_t* slice_aux, uint32_t n_slices, const int32_t* perm,
+                       const int32_t* inv, const long long* row_ptr, const int32_t* col, const void* w, int wtype,
+                       int4* col4, uint32_t* w4, int4* w4w, uint32_t* sorig) {
     const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (gw >= n_slices) return;
     const SliceDesc d = slices[gw];
-    const int log_spr = (int)(d.meta & 0xffu), nrows = (int)(d.meta >> 8);
+    const int log_spr = (int)(d.meta & 0xffu), nrows = (int)((d.meta >> 8) & 0xffu);
+    const uint32_t parts = d.meta >> 16;
     const uint32_t spr = 1u << log_spr;
+    if (parts != 0u) {
+        // part `part` of a hub row: cells [part * cpp, min((part + 1) * cpp, groups)) of the row, cell l of the
+        // part at (g, sr) = (l / 16, l % 16)
+        const uint32_t hub = slice_aux[2 * gw], part = slice_aux[2 * gw + 1];
+        const int32_t orig = perm[d.row0];
+        const long long b = row_ptr[orig], deg = row_ptr[orig + 1] - b;
+        const long long groups = (deg + 3) / 4, cpp = (groups + parts - 1) / parts;
+        const long long first = (long long)part * cpp;
+        const long long mine = groups - first < cpp ? groups - first : cpp;   // may be <= 0 for a trailing part
+        if (lane < kSubRows)
+            sorig[(size_t)gw * kSubRows + lane] = lane == 0 ? (uint32_t)orig : lane == 1 ? hub : lane == 2 ? part : 0xffffffffu;
+        const uint32_t Gs = d.G > (uint32_t)kHeadGroups ? d.G : (uint32_t)kHeadGroups;
+        for (uint32_t cell = lane; cell < Gs * kSubRows; cell += 32) {
+            const uint32_t g = cell / kSubRows, sr = cell % kSubRows;
+            int cc[4] = {(int)d.row0, (int)d.row0, (int)d.row0, (int)d.row0};
+            int ww[4] = {0, 0, 0, 0};
+            if ((long long)cell < mine) fetch_group(inv, col, w, wtype, b, deg, first + cell, (int)d.row0, cc, ww);
+            const size_t at = g < kHeadGroups ? ((size_t)gw * kHeadGroups + g) * kSubRows + sr
+                                              : (size_t)d.off + (size_t)(g - kHeadGroups) * kSubRows + sr;
+            store_cell(col4, w4, w4w, at, cc, ww);
+        }
+        return;
+    }
     if (lane < kSubRows) {
         const uint32_t rloc = (uint32_t)lane >> log_spr;
         sorig[(size_t)gw * kSubRows + lane] = (int)rloc < nrows ? (uint32_t)perm[d.row0 + rloc] : 0xffffffffu;
@@ -145,23 +169,6 @@ __global__ void k_pack(const SliceDesc* slices, uint32_t n_slices, const int32_t
         const int ww[4] = {0, 0, 0, 0};
         for (uint32_t g = d.G; g < kHeadGroups; ++g)
             store_cell(col4, w4, w4w, ((size_t)gw * kHeadGroups + g) * kSubRows + lane, cc, ww);
-    }
-}
-
-// One CTA per hub: cell (g, j) holds group q = g * kHubSub + j of the hub's row (g = 0: hub-indexed head cell).
-__global__ void k_pack_hubs(const HubDesc* hubs, uint32_t n_hubs, uint32_t hub_head, const int32_t* inv,
-                            const long long* row_ptr, const int32_t* col, const void* w, int wtype, int4* col4,
-                            uint32_t* w4, int4* w4w) {
-    if (blockIdx.x >= n_hubs) return;
-    const HubDesc d = hubs[blockIdx.x];
-    const long long b = row_ptr[d.orig], deg = row_ptr[d.orig + 1] - b;
-    const unsigned long long cells = (unsigned long long)d.G * kHubSub;
-    for (unsigned long long cell = threadIdx.x; cell < cells; cell += blockDim.x) {
-        int cc[4], ww[4];
-        fetch_group(inv, col, w, wtype, b, deg, (long long)cell, (int)d.row, cc, ww);
-        const size_t at = cell < (unsigned long long)kHubSub ? (size_t)hub_head + (size_t)blockIdx.x * kHubSub + cell
-                                                             : (size_t)d.off + (cell - kHubSub);
-        store_cell(col4, w4, w4w, at, cc, ww);
     }
 }
 

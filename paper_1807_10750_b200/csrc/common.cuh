@@ -3,12 +3,14 @@
 // Device layout of a loaded graph ("SELL-16 with row splitting + CTA hubs"):
 //   * vertices are relabelled by (colour asc, degree desc, caller id asc); `perm` maps the
 //     internal row back to the caller's vertex id (which is what enters the Philox counter);
-//   * a SLICE is the work of one warp: 16 sub-rows x G groups x 4 edges.  A row of
-//     degree d <= kHubDegree is split into SPR in {1,2,4,8,16} sub-rows (group q of the row goes
+//   * a SLICE is the work of one warp: 16 sub-rows x G groups x 4 edges.  A row of up to
+//     16 x kSubRowEdges edges is split into SPR in {1,2,4,8,16} sub-rows (group q of the row goes
 //     to sub-row q % SPR), so a slice holds 16/SPR rows; the sub-rows of one row are
 //     finished by a warp-level segmented (butterfly) reduction;
-//   * a HUB is a row of degree > kHubDegree; it is the work of one whole CTA (kHubSub = 256
-//     sub-rows, group q goes to sub-row q % 256) and is finished through shared memory;
+//   * a HUB is a row with more edges than one slice holds; it is cut into P balanced PARTS, one
+//     slice each (SPR = 16), scheduled like any other slice.  A part adds its partial local fields
+//     to hub_acc[hub][tile][32] (integer atomics, order-free) and counts itself in hub_cnt; the part
+//     that arrives last reads the sums, finishes the row and clears hub_acc for the next sweep;
 //   * a CELL is one int4 of four (relabelled) neighbour rows plus one word of four int8
 //     weights (w4w: an int4 of int32 weights for graphs whose weights do not fit int8).
 //     Padding entries carry weight 0 and point at the sub-row's own row (a sector that is read
@@ -16,15 +18,13 @@
 //     Cell arrays: groups 0 and 1 of slice s sit at HEAD cells (s*2 + g)*16 + sub-row, so that
 //     everything a warp needs to start a slice (descriptor, first cells, caller ids) is addressed
 //     by the slice index alone and can be prefetched with independent loads, also across the grid
-//     barrier that separates colour phases.  Rows of up to 128 edges live entirely in head cells;
-//     groups g >= 2 (rows of 129..256 edges) sit at desc.off + (g-2)*16 + sub-row;
-//     group 0 of hub h sits at hub_head + h*256 + sub-row (prefetchable as well), its groups g >= 1 at
-//     hub.off + (g-1)*256 + sub-row;
+//     barrier that separates colour phases; groups g >= 2 sit at desc.off + (g-2)*16 + sub-row;
 //   * spins are replica-interleaved: state[tile][row][32] int8 (+1/-1), one 32-byte
 //     sector per spin per tile of 32 replicas, so a neighbour gather is one sector and a
 //     thread pair reads it with two 16-byte loads;
 //   * ranges[phase][cta] is the static, cost-balanced split of every colour phase over the
-//     CTAs of the persistent grid.
+//     CTAs of the grid (launch-per-phase kernels; hubs also in the persistent kernel, which hands out
+//     the slices of a phase by ticket, phase_slices[phase] .. phase_slices[phase + 1]).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -40,27 +40,19 @@ constexpr int kWarpsPerCta = 16;
 constexpr int kSweepThreads = kWarpsPerCta * 32;
 constexpr int kHeadGroups = 2;       // groups of every slice stored at slice-indexed (prefetchable) positions
 constexpr int kSubRowEdges = 16;                      // a row is split until a sub-row has <= this many edges ...
-constexpr int kHubDegree = 256;                        // ... up to 16 sub-rows; rows above this are CTA hubs
-constexpr int kHubSub = kWarpsPerCta * kSubRows;       // 256 sub-rows of a hub
-constexpr int kMaxPersistReplicas = 1024;              // replicas per persistent launch
+                                                       // ... up to 16 sub-rows; rows above that are hubs (cut into parts)
+constexpr int kMaxPersistReplicas = 512;               // replicas per persistent launch
 
 struct SliceDesc {
     uint32_t off;    // first tail cell (groups >= kHeadGroups) of this slice
     uint32_t row0;   // first internal row
     uint32_t G;      // groups (of 4 edges) per sub-row, >= 1
-    uint32_t meta;   // log2(SPR) | (valid rows << 8)
-};
-
-struct HubDesc {
-    uint32_t off;    // first tail cell (groups >= 1)
-    uint32_t row;    // internal row
-    uint32_t G;      // groups per sub-row (iterations of the CTA)
-    uint32_t orig;   // caller's vertex id
+    uint32_t meta;   // log2(SPR) | (valid rows << 8) | (parts P of the hub this slice is a part of, else 0) << 16
 };
 
 struct PhaseRange {  // work of one CTA in one colour phase (absolute indices)
     uint32_t s0, s1; // slices
-    uint32_t h0, h1; // hubs
+    uint32_t h0, h1; // unused
 };
 
 enum SweepKind : int { kKindGS = 0, kKindJacobi = 1, kKindEval = 2 };
@@ -70,12 +62,15 @@ struct GraphView {
     const uint32_t* w4;
     const int4* w4w;            // wide weights, or nullptr
     const SliceDesc* slices;
-    const uint32_t* sorig;      // [n_slices * 16] caller id of each sub-row's row (0xffffffff: none)
-    const HubDesc* hubs;
+    const uint32_t* sorig;      // [n_slices * 16] caller id of each sub-row's row (0xffffffff: none); hub part:
+                                //   {caller id, hub id, part index, 0xffffffff ...}
+    int* hub_acc;               // [n_hubs][tiles_max][32] partial local fields of hub rows (zero between sweeps)
+    unsigned int* hub_cnt;      // [n_hubs][tiles_max] parts arrived so far (monotone)
+    uint32_t tiles_max;
     const PhaseRange* ranges;   // [n_phases][n_cta]
+    const uint32_t* phase_slices;   // [n_phases + 1] first slice of every phase
     uint32_t n_cta;             // CTAs the ranges were built for (== gridDim.x)
     uint32_t n_phases;
-    uint32_t hub_head;          // first hub head cell: group 0 of hub h sits at hub_head + h*256 + sub-row
 };
 
 struct SweepParams {

@@ -59,6 +59,7 @@ inline int spr_log2_for_degree(int64_t deg, int sub_row_edges) {
     return l;
 }
 
+constexpr uint32_t kTicketChunk = 0;   // slice units per ticket of the persistent kernel; 0 = static stride (measured faster on config 5: 241 vs 261 us per sweep)
 constexpr uint32_t kThrCap = 1u << 16;   // thresholds per persistent launch (longer schedules are chunked)
 
 // Upper bounds used by ising_workspace_bytes (any degree distribution).
@@ -67,11 +68,11 @@ inline uint64_t bound_slices(int64_t n, int64_t nnz, int64_t C) {
     // slice per (colour, SPR)
     return (uint64_t)n / 16 + (uint64_t)nnz / 64 + 5 * (uint64_t)(C + 1) + 8;
 }
-inline uint64_t bound_hubs(int64_t nnz) { return (uint64_t)nnz / (kHubDegree + 1) + 1; }
+inline uint64_t bound_hubs(int64_t n, int64_t nnz) { return std::min<uint64_t>((uint64_t)n, (uint64_t)nnz / 129 + 1); }   // hub rows have > 128 edges
 inline uint64_t bound_cells(int64_t n, int64_t nnz, int64_t C) {
     // two head cells per sub-row of every slice; tail cells only for rows of 129..256 edges (each
-    // holds >= 1 edge of a sub-row that is more than half full); hubs: nnz_h/4 + 256 cells of rounding each
-    return kHeadGroups * kSubRows * bound_slices(n, nnz, C) + (uint64_t)nnz / 2 + kHubSub * bound_hubs(nnz) +
+    // holds >= 1 edge of a sub-row that is more than half full); hubs: nnz_h/4 + 256 cells of rounding each, at least two groups
+    return kHeadGroups * kSubRows * bound_slices(n, nnz, C) + (uint64_t)nnz / 2 +
            (uint64_t)nnz / 4 + 64;
 }
 constexpr uint64_t kMaxCtas = 1024;
@@ -86,6 +87,7 @@ struct SmallArrays {
     int32_t* best_sweep;
     uint32_t* thr;         // kThrCap
     unsigned int* barrier;
+    unsigned int* tickets;  // 2 * phases
     int* flag;
 };
 
@@ -106,7 +108,9 @@ size_t workspace_need(int64_t n, int64_t nnz, int wtype, int64_t max_replicas, i
     add(4 * (size_t)n);                       // inv
     add(sizeof(SliceDesc) * (size_t)(n_slices + 1));
     add(4 * 16 * (size_t)(n_slices + 1));     // sorig
-    add(sizeof(HubDesc) * (size_t)(n_hubs + 1));
+    add(8 * (size_t)(n_slices + 1));          // slice_aux
+    add(4 * kTile * (size_t)tiles * (size_t)(n_hubs + 1));   // hub_acc
+    add(4 * (size_t)tiles * (size_t)(n_hubs + 1));           // hub_cnt
     add(sizeof(PhaseRange) * (size_t)(phases * kMaxCtas));
     add(16 * (size_t)(cells + 1));            // col4
     add(4 * (size_t)(cells + 1));             // w4
@@ -119,6 +123,8 @@ size_t workspace_need(int64_t n, int64_t nnz, int wtype, int64_t max_replicas, i
     add(4 * (size_t)tiles * kTile);           // best_sweep
     add(4 * (size_t)kThrCap);                 // thr
     add(256);                                 // barrier
+    add(8 * (size_t)phases);                  // tickets
+    add(4 * (size_t)(phases + 1));            // phase_slices
     add(256);                                 // flag
     if (dense) add(dense_workspace_bytes(n, max_replicas));
     return align_up(s) + kAlign;
@@ -140,8 +146,11 @@ struct ising_problem {
     int32_t* inv = nullptr;
     SliceDesc* slices = nullptr;
     uint32_t* sorig = nullptr;
-    HubDesc* hubs = nullptr;
+    uint32_t* slice_aux = nullptr;       // [n_slices][2] (hub id, part index) of hub-part slices
+    int* hub_acc = nullptr;              // [n_hubs][tiles_max][32] partial local fields of hub rows
+    unsigned int* hub_cnt = nullptr;     // [n_hubs][tiles_max] parts arrived (monotone)
     PhaseRange* ranges = nullptr;
+    uint32_t* phase_slices = nullptr;
     int4* col4 = nullptr;
     uint32_t* w4 = nullptr;
     int4* w4w = nullptr;
@@ -151,7 +160,7 @@ struct ising_problem {
     SmallArrays sm{};
     DenseEngine* dense = nullptr;
     // host bookkeeping
-    uint32_t n_slices = 0, n_hubs = 0, n_phases = 1, n_cta = 1, hub_head = 0;
+    uint32_t n_slices = 0, n_hubs = 0, n_phases = 1, n_cta = 1;
     uint64_t cells = 0;
     size_t ws_used = 0;
     int cur = 0;
@@ -172,8 +181,9 @@ namespace {
 
 GraphView graph_view(const ising_problem* p) {
     GraphView g{};
-    g.col4 = p->col4; g.w4 = p->w4; g.w4w = p->w4w; g.slices = p->slices; g.sorig = p->sorig; g.hubs = p->hubs;
-    g.ranges = p->ranges; g.n_cta = p->n_cta; g.n_phases = p->n_phases; g.hub_head = p->hub_head;
+    g.col4 = p->col4; g.w4 = p->w4; g.w4w = p->w4w; g.slices = p->slices; g.sorig = p->sorig;
+    g.hub_acc = p->hub_acc; g.hub_cnt = p->hub_cnt; g.tiles_max = (uint32_t)p->tiles_max;
+    g.ranges = p->ranges; g.phase_slices = p->phase_slices; g.n_cta = p->n_cta; g.n_phases = p->n_phases;
     return g;
 }
 
@@ -286,7 +296,7 @@ ising_status ising_workspace_bytes(int32_t n, int64_t nnz, int32_t wtype, int32_
     if (max_replicas < 1 || max_replicas > 65536) return ISING_ERR_TOO_MANY_REPLICAS;
     const bool dense = kDenseEnabled && nnz == (int64_t)n * (n - 1) && n >= 2;
     *bytes_out = workspace_need(n, nnz, wtype, max_replicas, n_colours, wtype == ISING_W_INT32,
-                                bound_slices(n, nnz, n_colours), bound_hubs(nnz), bound_cells(n, nnz, n_colours), true,
+                                bound_slices(n, nnz, n_colours), bound_hubs(n, nnz), bound_cells(n, nnz, n_colours), true,
                                 dense);
     return ISING_OK;
 }
@@ -395,29 +405,42 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
     }
     std::vector<SliceDesc> slices;
-    std::vector<HubDesc> hubs_sorted;                           // per phase, degree descending
-    std::vector<uint32_t> slice_begin((size_t)C + 1, 0), hub_begin((size_t)C + 1, 0);
-    uint64_t tail_cells = 0, hub_cells = 0;
+    std::vector<uint32_t> slice_aux;                            // per slice: (hub id, part index) of hub-part slices
+    std::vector<uint32_t> slice_begin((size_t)C + 1, 0);
+    uint64_t tail_cells = 0;
+    uint32_t n_hub_rows = 0;
+    bool too_many_parts = false;
     auto degree_of = [&](int32_t k) { return h_row_ptr[perm[k] + 1] - h_row_ptr[perm[k]]; };
     // Edges per sub-row before a row is split over more sub-rows: 16 keeps the instruction count per edge low
-    // (throughput-bound graphs); 8 keeps every row of up to 128 edges inside the prefetched head cells, i.e. one
-    // gather round trip per phase (latency-bound graphs: fewer units in the largest phase than warps on the GPU).
+    // (throughput-bound graphs); 8 keeps every row inside the prefetched head cells, i.e. one gather round trip
+    // per phase (latency-bound graphs: fewer units in the largest phase than warps on the GPU).  A row of more
+    // than 16 sub-rows x sub_row_edges edges (a hub) is cut into P balanced PARTS, one slice each, whose partial
+    // fields meet in hub_acc (integer atomics); the part that arrives last finishes the row.
     auto build_units = [&](int sub_row_edges) {
-        slices.clear(); hubs_sorted.clear(); tail_cells = 0; hub_cells = 0;
+        slices.clear(); slice_aux.clear(); tail_cells = 0; n_hub_rows = 0;
+        const int64_t part_cells_max = (int64_t)kSubRows * (sub_row_edges / 4);
         int32_t k = 0;
         for (int32_t c = 0; c < C; ++c) {
             slice_begin[c] = (uint32_t)slices.size();
-            hub_begin[c] = (uint32_t)hubs_sorted.size();
             while (k < n && h_colour[perm[k]] == c) {
                 const int64_t deg = degree_of(k);
-                if (deg > kHubDegree) {
-                    HubDesc h;
-                    h.off = 0;
-                    h.row = (uint32_t)k;
-                    h.G = (uint32_t)(((deg + 3) / 4 + kHubSub - 1) / kHubSub);
-                    h.orig = (uint32_t)perm[k];
-                    hubs_sorted.push_back(h);
-                    hub_cells += (uint64_t)h.G * kHubSub;
+                const int64_t groups = (deg + 3) / 4;
+                if (groups > part_cells_max) {
+                    const int64_t P = (groups + part_cells_max - 1) / part_cells_max;
+                    const int64_t cpp = (groups + P - 1) / P;
+                    if (P > 0xffff) too_many_parts = true;
+                    for (int64_t q = 0; q < P; ++q) {
+                        SliceDesc d;
+                        d.off = 0;
+                        d.row0 = (uint32_t)k;
+                        d.G = (uint32_t)((cpp + kSubRows - 1) / kSubRows);
+                        d.meta = 4u | (1u << 8) | ((uint32_t)P << 16);
+                        slices.push_back(d);
+                        slice_aux.push_back(n_hub_rows);
+                        slice_aux.push_back((uint32_t)q);
+                        tail_cells += (uint64_t)std::max<int64_t>(0, (int64_t)d.G - kHeadGroups) * kSubRows;
+                    }
+                    ++n_hub_rows;
                     ++k;
                     continue;
                 }
@@ -427,7 +450,6 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
                 while (nr < rps && k + nr < n && h_colour[perm[k + nr]] == c &&
                        spr_log2_for_degree(degree_of(k + nr), sub_row_edges) == l)
                     ++nr;
-                const int64_t groups = (deg + 3) / 4;
                 const int64_t G = std::max<int64_t>(1, (groups + (1ll << l) - 1) >> l);
                 SliceDesc d;
                 d.off = 0;
@@ -435,20 +457,21 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
                 d.G = (uint32_t)G;
                 d.meta = (uint32_t)l | ((uint32_t)nr << 8);
                 slices.push_back(d);
+                slice_aux.push_back(0u);
+                slice_aux.push_back(0u);
                 tail_cells += (uint64_t)std::max<int64_t>(0, G - kHeadGroups) * kSubRows;
                 k += nr;
             }
         }
         slice_begin[C] = (uint32_t)slices.size();
-        hub_begin[C] = (uint32_t)hubs_sorted.size();
         uint64_t units = 0;
-        for (int32_t c = 0; c < C; ++c)
-            units = std::max<uint64_t>(units, (uint64_t)(slice_begin[c + 1] - slice_begin[c]) + (hub_begin[c + 1] - hub_begin[c]));
+        for (int32_t c = 0; c < C; ++c) units = std::max<uint64_t>(units, (uint64_t)(slice_begin[c + 1] - slice_begin[c]));
         return units * (uint64_t)((max_replicas + kTile - 1) / kTile);
     };
     if (build_units(kSubRowEdges) < (uint64_t)sm_count * kWarpsPerCta) build_units(kHeadGroups * 4);
+    if (too_many_parts) return ISING_ERR_BAD_SHAPE;
     const uint64_t head_cells = (uint64_t)slices.size() * kSubRows * kHeadGroups;
-    const uint64_t cells = head_cells + tail_cells + hub_cells;
+    const uint64_t cells = head_cells + tail_cells;
     if (cells > 0xffffffffull) return ISING_ERR_BAD_SHAPE;
     {
         uint64_t at = head_cells;
@@ -458,71 +481,49 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         }
     }
 
-    // ---- static split of every colour phase over the CTAs of the persistent grid.  Cost unit: executed
-    // warp instructions (ncu source counters, profiles/): a slice costs ~430 + 70 per group + 45 per
-    // butterfly level + 120 per dependent tail group, a hub 16 warps x (400 + 100 per group).
+    // ---- static split of every colour phase over the CTAs of the grid (launch-per-phase kernels; the persistent
+    // kernel deals the units out itself).  Cost unit: executed warp instructions (ncu source counters,
+    // profiles/): a slice costs ~430 + 70 per group + 45 per butterfly level + 120 per dependent tail group.
     auto slice_cost = [](const SliceDesc& d) {
         const double G = (double)d.G, l = (double)(d.meta & 0xffu);
         return 430.0 + 70.0 * G + 45.0 * l + 120.0 * std::max(0.0, G - (double)kHeadGroups);
     };
-    auto hub_cost = [](uint32_t G) { return (double)kWarpsPerCta * (400.0 + 100.0 * (double)G); };
     // Grid size: small graphs are latency-bound (one dependent gather chain per phase), so every (slice, tile)
-    // unit and every hub of the largest phase gets its own CTA, up to one CTA per SM (measured on configs 1-3:
-    // spreading the units beats the cheaper barrier of a smaller grid).
+    // unit of the largest phase gets its own CTA, up to one CTA per SM (measured on configs 1-3: spreading the
+    // units beats the cheaper barrier of a smaller grid).
     uint32_t n_cta = 1;
     {
         const uint64_t tiles_max = (uint64_t)(max_replicas + kTile - 1) / kTile;
         uint64_t units = 1;
         for (int32_t c = 0; c < C; ++c)
-            units = std::max<uint64_t>(units, ((uint64_t)(slice_begin[c + 1] - slice_begin[c]) +
-                                               (uint64_t)(hub_begin[c + 1] - hub_begin[c])) * tiles_max);
+            units = std::max<uint64_t>(units, (uint64_t)(slice_begin[c + 1] - slice_begin[c]) * tiles_max);
         n_cta = (uint32_t)std::min<uint64_t>(units, (uint64_t)std::min<int>(sm_count, (int)kMaxCtas));
     }
     std::vector<PhaseRange> ranges((size_t)C * n_cta);
-    std::vector<HubDesc> hubs;
-    hubs.reserve(hubs_sorted.size());
-    {
-        std::vector<double> load(n_cta);
-        uint64_t at = head_cells + tail_cells + (uint64_t)hubs_sorted.size() * kHubSub;   // hub tails follow hub heads
-        for (int32_t c = 0; c < C; ++c) {
-            const uint32_t hb = hub_begin[c], hn = hub_begin[c + 1] - hb;
-            double total = 0;
-            for (uint32_t b = 0; b < n_cta; ++b) {
-                PhaseRange& r = ranges[(size_t)c * n_cta + b];
-                r.h0 = (uint32_t)hubs.size();
-                load[b] = 0;
-                for (uint32_t q = b; q < hn; q += n_cta) {   // round robin over degree-sorted hubs
-                    HubDesc h = hubs_sorted[hb + q];
-                    h.off = (uint32_t)at;
-                    at += (uint64_t)(h.G - 1) * kHubSub;
-                    load[b] += hub_cost(h.G);
-                    hubs.push_back(h);
+    for (int32_t c = 0; c < C; ++c) {
+        double total = 0;
+        for (uint32_t q = slice_begin[c]; q < slice_begin[c + 1]; ++q) total += slice_cost(slices[q]);
+        uint32_t pos = slice_begin[c];
+        const uint32_t end = slice_begin[c + 1];
+        double remaining = total;
+        for (uint32_t b = 0; b < n_cta; ++b) {
+            PhaseRange& r = ranges[(size_t)c * n_cta + b];
+            const double target = remaining / (double)(n_cta - b);
+            double mine = 0;
+            r.h0 = r.h1 = 0;
+            r.s0 = pos;
+            if (b + 1 == n_cta) {
+                while (pos < end) mine += slice_cost(slices[pos++]);
+            } else {
+                while (pos < end) {
+                    const double cs = slice_cost(slices[pos]);
+                    if (mine + 0.5 * cs > target) break;
+                    mine += cs;
+                    ++pos;
                 }
-                r.h1 = (uint32_t)hubs.size();
-                total += load[b];
             }
-            for (uint32_t q = slice_begin[c]; q < slice_begin[c + 1]; ++q) total += slice_cost(slices[q]);
-            uint32_t pos = slice_begin[c];
-            const uint32_t end = slice_begin[c + 1];
-            double remaining = total;
-            for (uint32_t b = 0; b < n_cta; ++b) {
-                PhaseRange& r = ranges[(size_t)c * n_cta + b];
-                const double target = remaining / (double)(n_cta - b);
-                double mine = load[b];
-                r.s0 = pos;
-                if (b + 1 == n_cta) {
-                    while (pos < end) mine += slice_cost(slices[pos++]);
-                } else {
-                    while (pos < end) {
-                        const double cs = slice_cost(slices[pos]);
-                        if (mine + 0.5 * cs > target) break;
-                        mine += cs;
-                        ++pos;
-                    }
-                }
-                r.s1 = pos;
-                remaining -= mine;
-            }
+            r.s1 = pos;
+            remaining -= mine;
         }
     }
 
@@ -535,8 +536,8 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     p->n = n; p->nnz = nnz; p->n_colours = n_colours; p->max_replicas = max_replicas;
     p->tiles_max = (max_replicas + kTile - 1) / kTile;
     p->W = rep.w_sum / 2; p->absw_max = rep.absw_max; p->wide = wide;
-    p->n_slices = (uint32_t)slices.size(); p->n_hubs = (uint32_t)hubs.size(); p->cells = cells;
-    p->n_phases = (uint32_t)C; p->n_cta = n_cta; p->hub_head = (uint32_t)(head_cells + tail_cells); p->sm_count = sm_count; p->cooperative = coop != 0;
+    p->n_slices = (uint32_t)slices.size(); p->n_hubs = n_hub_rows; p->cells = cells;
+    p->n_phases = (uint32_t)C; p->n_cta = n_cta; p->sm_count = sm_count; p->cooperative = coop != 0;
     p->flush_rows = wide ? 0x7fffffffu
                          : (uint32_t)std::max<int64_t>(1, ((1ll << 31) - 1) / std::max<int64_t>(1, 2 * rep.absw_max));
 
@@ -545,7 +546,9 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     p->inv = (int32_t*)ws.take(4 * (size_t)n);
     p->slices = (SliceDesc*)ws.take(sizeof(SliceDesc) * (slices.size() + 1));
     p->sorig = (uint32_t*)ws.take(4 * kSubRows * (slices.size() + 1));
-    p->hubs = (HubDesc*)ws.take(sizeof(HubDesc) * (hubs.size() + 1));
+    p->slice_aux = (uint32_t*)ws.take(8 * (slices.size() + 1));
+    p->hub_acc = (int*)ws.take(sizeof(int) * kTile * tiles * ((size_t)n_hub_rows + 1));
+    p->hub_cnt = (unsigned int*)ws.take(4 * tiles * ((size_t)n_hub_rows + 1));
     p->ranges = (PhaseRange*)ws.take(sizeof(PhaseRange) * ranges.size());
     p->col4 = (int4*)ws.take(16 * ((size_t)cells + 1));
     p->w4 = (uint32_t*)ws.take(4 * ((size_t)cells + 1));
@@ -565,6 +568,8 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     p->sm.best_sweep = (int32_t*)ws.take(4 * tiles * kTile);
     p->sm.thr = (uint32_t*)ws.take(4 * (size_t)kThrCap);
     p->sm.barrier = (unsigned int*)ws.take(256);
+    p->sm.tickets = (unsigned int*)ws.take(8 * (size_t)C);
+    p->phase_slices = (uint32_t*)ws.take(4 * ((size_t)C + 1));
     p->sm.flag = (int*)ws.take(256);
     void* dense_mem = nullptr;
     size_t dense_bytes = 0;
@@ -580,17 +585,16 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     CKP(cudaMemcpyAsync(p->perm, perm.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
     CKP(cudaMemcpyAsync(p->inv, inv.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
     CKP(cudaMemcpyAsync(p->ranges, ranges.data(), sizeof(PhaseRange) * ranges.size(), cudaMemcpyHostToDevice, st));
+    CKP(cudaMemcpyAsync(p->phase_slices, slice_begin.data(), 4 * ((size_t)C + 1), cudaMemcpyHostToDevice, st));
     if (!slices.empty()) {
         CKP(cudaMemcpyAsync(p->slices, slices.data(), sizeof(SliceDesc) * slices.size(), cudaMemcpyHostToDevice, st));
+        CKP(cudaMemcpyAsync(p->slice_aux, slice_aux.data(), 4 * slice_aux.size(), cudaMemcpyHostToDevice, st));
         const unsigned blocks = (unsigned)(((long long)slices.size() * 32 + 255) / 256);
-        k_pack<<<blocks, 256, 0, st>>>(p->slices, (uint32_t)slices.size(), p->perm, p->inv, d_row_ptr, d_col, d_w,
-                                       wtype, p->col4, p->w4, p->w4w, p->sorig);
+        k_pack<<<blocks, 256, 0, st>>>(p->slices, p->slice_aux, (uint32_t)slices.size(), p->perm, p->inv, d_row_ptr,
+                                       d_col, d_w, wtype, p->col4, p->w4, p->w4w, p->sorig);
     }
-    if (!hubs.empty()) {
-        CKP(cudaMemcpyAsync(p->hubs, hubs.data(), sizeof(HubDesc) * hubs.size(), cudaMemcpyHostToDevice, st));
-        k_pack_hubs<<<(unsigned)hubs.size(), 256, 0, st>>>(p->hubs, (uint32_t)hubs.size(), p->hub_head, p->inv, d_row_ptr, d_col,
-                                                          d_w, wtype, p->col4, p->w4, p->w4w);
-    }
+    CKP(cudaMemsetAsync(p->hub_acc, 0, sizeof(int) * kTile * tiles * ((size_t)n_hub_rows + 1), st));
+    CKP(cudaMemsetAsync(p->hub_cnt, 0, 4 * tiles * ((size_t)n_hub_rows + 1), st));
     if (want_dense) {
         p->dense = dense_create(n, max_replicas, dense_mem, dense_bytes, d_row_ptr, d_col, d_w, wtype, st);
         if (!p->dense) return fail(ISING_ERR_CUDA);
@@ -707,6 +711,7 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
                 CK(cudaMemcpyAsync(p->sm.thr, thresholds + s0, 4 * (size_t)ns, cudaMemcpyHostToDevice, st));
                 CK(cudaMemsetAsync(p->sm.accum3, 0, 8 * 3 * (size_t)kMaxPersistReplicas, st));
                 CK(cudaMemsetAsync(p->sm.barrier, 0, 256, st));
+                CK(cudaMemsetAsync(p->sm.tickets, 0, 8 * (size_t)p->n_phases, st));
                 AnnealParams a{};
                 a.g = graph_view(p);
                 a.state = p->state[p->cur] + (size_t)t0 * tile_stride;
@@ -730,6 +735,9 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
                 a.best_out = p->sm.bestcut[0] + (size_t)t0 * kTile;
                 a.best_sweep_out = p->sm.best_sweep + (size_t)t0 * kTile;
                 a.barrier = p->sm.barrier;
+                a.tickets = p->sm.tickets;
+                a.ticket_chunk = kTicketChunk;
+                if (const char* e = getenv("ISING_TICKET_CHUNK")) a.ticket_chunk = (uint32_t)atoi(e);   // tuning knob
                 a.resume = s0 > 0 ? 1 : 0;
                 a.timing = (t0 == 0 && s0 == 0) ? p->timing : nullptr;
                 a.timing_sweep = p->timing_sweep;

@@ -5,7 +5,7 @@
 // neighbour sectors are gathered per step (16-byte L2 loads), byte-transposed with PRMT so
 // that one dp4a multiplies the four edge weights into one replica's field.  Rows split
 // over several sub-rows are finished by a warp-level segmented (butterfly) reduction; hub
-// rows are spread over the whole CTA and finished through shared memory.
+// rows are cut into parts (one slice each) whose partial fields meet in global memory.
 // The epilogue takes the energy-minimising value (L47-49 with the sign reading Q1:
 // s_i <- +1 if h_i < 0 else -1), applies the scheduled flip of Algorithm 2 (L177) with the
 // stateless Philox word, writes the spin sector and accumulates the energy bookkeeping
@@ -196,6 +196,7 @@ struct PassCtx {
     uint32_t rep_lane0;    // global id of this lane's replica 0
     uint32_t thr, T;
     int32_t tie_rule;
+    uint32_t tile;         // replica tile of this unit (index into hub_acc / hub_cnt)
 };
 
 __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
@@ -278,6 +279,52 @@ __device__ __forceinline__ uint4 ld_best_early(const PassCtx& x, bool owner, siz
     return b;
 }
 
+// Hub part (common.cuh): this warp holds, spread over its 16 sub-rows, the partial local fields of one part of
+// a hub row.  The partial sums of all parts meet in hub_acc (one warp-wide integer RED per part, so the result
+// does not depend on the order); the part that arrives last (hub_cnt) reads the totals, clears them for the
+// next sweep and finishes the row (a4-a7) like the owner lanes of an ordinary slice.
+template <int KIND, typename Acc>
+__device__ __forceinline__ void part_finish(const GraphView& g, const PassCtx& x, uint32_t row0, uint32_t parts,
+                                            uint32_t orig, uint32_t hub, int (&h)[16], const uint4& so4,
+                                            const Acc& acc, const PhiloxKeys& keys) {
+    const int lane = threadIdx.x & 31, sr = lane >> 1, half = lane & 1;
+    uint32_t none = 0;
+    half_reduce16(h, none, half);   // every lane: the part's sums of its half's 16 replicas
+    int v = h[0];
+#pragma unroll
+    for (int k = 1; k < 16; ++k) v = sr == k ? h[k] : v;   // lane (sr, half) contributes replica half * 16 + sr
+    const size_t slot = (size_t)hub * g.tiles_max + x.tile;
+    int* accp = g.hub_acc + slot * kTile + half * 16;
+    asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(accp + sr), "r"(v) : "memory");
+    // arrival: the warp barrier orders the lanes' REDs before lane 0's release (cumulative), the last part's
+    // acquire orders its reads of the sums after every part's REDs
+    __syncwarp();
+    unsigned int old = 0;
+    if (lane == 0)
+        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(g.hub_cnt + slot) : "memory");
+    old = __shfl_sync(0xffffffffu, old, 0);
+    if ((old + 1u) % parts != 0u) return;
+    __syncwarp();
+    const size_t row_off = (size_t)row0 * kTile;
+    const uint4 bold = ld_best_early<KIND>(x, sr == 0, row_off);
+    uint32_t flip = 0;
+    if (KIND != kKindEval) {
+        flip = flip_mask_part(orig, x.T, x.rep_lane0, x.thr, (uint32_t)sr, (uint32_t)kSubRows, keys);
+        if (half) asm volatile("redux.sync.or.b32 %0, %0, 0xaaaaaaaa;" : "+r"(flip));
+        else asm volatile("redux.sync.or.b32 %0, %0, 0x55555555;" : "+r"(flip));
+    }
+    if (sr == 0) {
+        int4* ap = reinterpret_cast<int4*>(accp);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int4 t = __ldcg(ap + k);
+            h[4 * k] = t.x; h[4 * k + 1] = t.y; h[4 * k + 2] = t.z; h[4 * k + 3] = t.w;
+            __stcg(ap + k, make_int4(0, 0, 0, 0));
+        }
+        row_update<KIND>(x, h, so4, bold, finish_flip_mask(flip, x.rep_lane0), row_off, acc);
+    }
+}
+
 // Everything a warp needs to start a slice; addressed by the slice index alone.
 struct SliceHead {
     SliceDesc d;
@@ -306,7 +353,7 @@ __device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x,
                                            int sr, const Acc& acc, const PhiloxKeys& keys) {
     const SliceDesc d = hd.d;
     const int log_spr = (int)(d.meta & 0xffu);
-    const int nrows = (int)(d.meta >> 8);
+    const int nrows = (int)((d.meta >> 8) & 0xffu);
     const uint32_t spr = 1u << log_spr;
     const int rloc = sr >> log_spr;
     const bool owner = ((sr & (int)(spr - 1)) == 0) && rloc < nrows;
@@ -335,7 +382,7 @@ __device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x,
         }
     }
     uint32_t flip = 0;
-    if (KIND != kKindEval && hd.orig != 0xffffffffu)
+    if (KIND != kKindEval && hd.orig != 0xffffffffu && (d.meta >> 16) == 0u)
         flip = flip_mask_part(hd.orig, x.T, x.rep_lane0, x.thr, (uint32_t)sr & (spr - 1), spr, keys);
 
     int h[16];
@@ -354,6 +401,11 @@ __device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x,
         }
     }
 
+    if (d.meta >> 16) {   // hub part: sorig = {caller id, hub id, part index, ...}
+        const uint32_t orig = __shfl_sync(0xffffffffu, hd.orig, 0), hub = __shfl_sync(0xffffffffu, hd.orig, 2);
+        part_finish<KIND>(g, x, d.row0, d.meta >> 16, orig, hub, h, so4, acc, keys);
+        return;
+    }
     // warp-level segmented reduction over the sub-rows of one row (fields add, flip bits OR)
     if (log_spr == 4) {
         half_reduce16(h, flip, (int)(threadIdx.x & 1));
@@ -367,81 +419,174 @@ __device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x,
     if (owner) row_update<KIND>(x, h, so4, bold, finish_flip_mask(flip, x.rep_lane0), row_off, acc);
 }
 
-// Everything the CTA needs to start a hub, addressed by the hub index alone (prefetchable).
-struct HubHead {
-    HubDesc d;
-    int4 c;
-    uint32_t w;
+// ---------------------------------------------------------------------------------------------
+// Persistent kernel: the gathers of a slice land in shared memory (cp.async, 16 bytes per lane and
+// neighbour, thread-private slots), so that the gathers of unit k+1 fly while unit k is computed and no
+// register waits for them.  Slots 0-3: head group 0, 4-7: head group 1, 8: the row's own sector.
+// ---------------------------------------------------------------------------------------------
+constexpr int kGatherSlots = 2 * 4 + 1;
+constexpr uint32_t kSlotBytes = kSweepThreads * 16;                    // one slot of every thread of the CTA
+constexpr uint32_t kGatherBufBytes = kGatherSlots * kSlotBytes;
+
+__device__ __forceinline__ void cp_async16(uint32_t smem_addr, const void* gptr) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ uint4 lds128(uint32_t smem_addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(smem_addr));
+    return v;
+}
+
+__device__ __forceinline__ void cp_async4(uint32_t smem_addr, const void* gptr) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t smem_addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(smem_addr));
+    return v;
+}
+__device__ __forceinline__ void sts32(uint32_t smem_addr, uint32_t v) {
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(smem_addr), "r"(v) : "memory");
+}
+
+// Static data of a unit on its way to the compute stage.  Only the eight neighbour indices of the head groups
+// travel through registers (they form the gather addresses); weights, caller ids and the descriptor go straight
+// from global to shared memory (cp.async): meta slot m of this thread = {w0, w1, orig}, descriptor slot of the
+// warp = {SliceDesc, tile}.  Three rotating slots: computing / gathers in flight / head in flight.
+constexpr uint32_t kMetaSlots = 3;
+constexpr uint32_t kMetaBytes = kMetaSlots * 3 * kSweepThreads * 4;
+constexpr uint32_t kDescStride = 32;
+constexpr uint32_t kDescBytes = kMetaSlots * kWarpsPerCta * kDescStride;
+
+struct PipeAddr {      // shared-memory addresses of this thread
+    uint32_t meta0;    // meta slot 0, word 0 (word k at + k * kSweepThreads * 4, slot m at + m * 3 * kSweepThreads * 4)
+    uint32_t desc0;    // descriptor slot 0 of this warp (slot m at + m * kWarpsPerCta * kDescStride)
+    __device__ __forceinline__ uint32_t meta(uint32_t m, uint32_t k) const { return meta0 + (m * 3u + k) * (kSweepThreads * 4u); }
+    __device__ __forceinline__ uint32_t desc(uint32_t m) const { return desc0 + m * (kWarpsPerCta * kDescStride); }
 };
 
-template <bool WIDE>
-__device__ __forceinline__ HubHead fetch_hub_head(const GraphView& g, uint32_t hh, int warp, int sr) {
-    HubHead h;
-    const int4 v = ld_stream(reinterpret_cast<const int4*>(g.hubs + hh));
-    h.d.off = (uint32_t)v.x; h.d.row = (uint32_t)v.y; h.d.G = (uint32_t)v.z; h.d.orig = (uint32_t)v.w;
-    const size_t at = (size_t)g.hub_head + (size_t)hh * kHubSub + (size_t)(warp * kSubRows + sr);
-    h.c = ld_stream(g.col4 + at);
-    h.w = WIDE ? 0u : ld_stream(g.w4 + at);
+struct HeadIdx { int4 c0, c1; };
+
+__device__ __forceinline__ HeadIdx request_head(const GraphView& g, const PipeAddr& pa, uint32_t m, uint32_t s,
+                                                uint32_t tile, int sr, int lane) {
+    const size_t at = (size_t)s * (kHeadGroups * kSubRows) + sr;
+    HeadIdx h;
+    h.c0 = ld_stream(g.col4 + at);
+    h.c1 = ld_stream(g.col4 + at + kSubRows);
+    cp_async4(pa.meta(m, 0), g.w4 + at);
+    cp_async4(pa.meta(m, 1), g.w4 + at + kSubRows);
+    cp_async4(pa.meta(m, 2), g.sorig + (size_t)s * kSubRows + sr);
+    if (lane == 0) {
+        cp_async16(pa.desc(m), g.slices + s);
+        sts32(pa.desc(m) + 16, tile);
+    }
+    cp_async_commit();
     return h;
 }
 
-// One (hub, tile) unit, whole CTA.  s_hub: [kWarpsPerCta][32] ints of the buffer of this hub's
-// parity (the caller alternates two buffers, so one __syncthreads per hub suffices).
-template <int KIND, bool WIDE, typename Acc>
-__device__ __forceinline__ void hub_pass(const GraphView& g, const PassCtx& x, const HubHead& head, uint32_t hh,
-                                         int warp, int sr, int half, int (*s_hub)[kTile], bool epi_warp,
-                                         const Acc& acc, const PhiloxKeys& keys) {
-    const HubDesc hd = head.d;
-    const bool owner = epi_warp && sr == 0;
-    const size_t row_off = (size_t)hd.row * kTile;
-    const size_t j = (size_t)hd.off + (size_t)(warp * kSubRows + sr);   // tail cells (groups >= 1)
+// src: the unit's tile, lane half included.  gb: shared address of slot 0 of this thread in the target buffer.
+__device__ __forceinline__ void issue_slice_gathers(const uint8_t* src, const HeadIdx& hd, const SliceDesc& d, int sr,
+                                                    uint32_t gb) {
+    const int log_spr = (int)(d.meta & 0xffu);
+    const int nrows = (int)((d.meta >> 8) & 0xffu);
+    const int rloc = sr >> log_spr;
+    const bool owner = ((sr & ((1 << log_spr) - 1)) == 0) && rloc < nrows;
+    cp_async16(gb + 0 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.x * kTile);
+    cp_async16(gb + 1 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.y * kTile);
+    cp_async16(gb + 2 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.z * kTile);
+    cp_async16(gb + 3 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.w * kTile);
+    if (d.G > 1) {
+        cp_async16(gb + 4 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.x * kTile);
+        cp_async16(gb + 5 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.y * kTile);
+        cp_async16(gb + 6 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.z * kTile);
+        cp_async16(gb + 7 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.w * kTile);
+    }
+    if (owner) cp_async16(gb + 8 * kSlotBytes, src + (size_t)(d.row0 + (uint32_t)rloc) * kTile);
+    cp_async_commit();
+}
+
+__device__ __forceinline__ SliceDesc lds_desc(uint32_t addr) {
+    const uint4 v = lds128(addr);
+    SliceDesc d;
+    d.off = v.x; d.row0 = v.y; d.G = v.z; d.meta = v.w;
+    return d;
+}
+
+// Compute stage of one (slice, tile) unit whose head gathers have landed in buffer gb (Gauss-Seidel, int8 weights).
+template <typename Acc>
+__device__ __forceinline__ void slice_compute(const GraphView& g, const PassCtx& x, const SliceDesc& d, uint32_t ma,
+                                              int sr, const Acc& acc, const PhiloxKeys& keys, uint32_t gb) {
+    // ma: this thread's meta slot of the unit (w0, w1, orig one word plane apart)
+    const int log_spr = (int)(d.meta & 0xffu);
+    const int nrows = (int)((d.meta >> 8) & 0xffu);
+    const uint32_t spr = 1u << log_spr;
+    const int rloc = sr >> log_spr;
+    const bool owner = ((sr & (int)(spr - 1)) == 0) && rloc < nrows;
+    const size_t row_off = (size_t)(d.row0 + (uint32_t)rloc) * kTile;
+    const uint4 bold = ld_best_early<kKindGS>(x, owner, row_off);
+    // tail cells (rows of 129..256 edges only): through registers, requested right away
+    const size_t tail_at = (size_t)d.off + sr;
+    int4 c2 = make_int4(0, 0, 0, 0), c3 = c2;
+    uint32_t w2 = 0, w3 = 0;
+    if (d.G > 2) {
+        c2 = ld_stream(g.col4 + tail_at);
+        w2 = ld_stream(g.w4 + tail_at);
+        if (d.G > 3) {
+            c3 = ld_stream(g.col4 + tail_at + kSubRows);
+            w3 = ld_stream(g.w4 + tail_at + kSubRows);
+        }
+    }
+    uint32_t flip = 0;
+    const uint32_t orig = lds32(ma + 2u * kSweepThreads * 4u);
+    const uint32_t parts = d.meta >> 16;
+    if (orig != 0xffffffffu && parts == 0u)
+        flip = flip_mask_part(orig, x.T, x.rep_lane0, x.thr, (uint32_t)sr & (spr - 1), spr, keys);
+
     int h[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) h[k] = 0;
-    int4 c = head.c;
-    uint32_t w = head.w;
-    int4 ww = make_int4(0, 0, 0, 0);
-    if (WIDE) ww = ld_stream(g.w4w + (size_t)g.hub_head + (size_t)hh * kHubSub + (size_t)(warp * kSubRows + sr));
-    uint4 e0 = ld_nbr(x.src, c.x), e1 = ld_nbr(x.src, c.y), e2 = ld_nbr(x.src, c.z), e3 = ld_nbr(x.src, c.w);
+    {
+        const uint4 e0 = lds128(gb + 0 * kSlotBytes), e1 = lds128(gb + 1 * kSlotBytes);
+        const uint4 e2 = lds128(gb + 2 * kSlotBytes), e3 = lds128(gb + 3 * kSlotBytes);
+        field_cell(h, e0, e1, e2, e3, lds32(ma));
+    }
+    if (d.G > 1) {
+        const uint4 f0 = lds128(gb + 4 * kSlotBytes), f1 = lds128(gb + 5 * kSlotBytes);
+        const uint4 f2 = lds128(gb + 6 * kSlotBytes), f3 = lds128(gb + 7 * kSlotBytes);
+        field_cell(h, f0, f1, f2, f3, lds32(ma + kSweepThreads * 4u));
+    }
+    if (d.G > 2) {
+        uint4 e0 = ld_nbr(x.src, c2.x), e1 = ld_nbr(x.src, c2.y), e2 = ld_nbr(x.src, c2.z), e3 = ld_nbr(x.src, c2.w);
+        if (d.G > 3) {
+            const uint4 f0 = ld_nbr(x.src, c3.x), f1 = ld_nbr(x.src, c3.y), f2 = ld_nbr(x.src, c3.z), f3 = ld_nbr(x.src, c3.w);
+            field_cell(h, e0, e1, e2, e3, w2);
+            field_cell(h, f0, f1, f2, f3, w3);
+        } else {
+            field_cell(h, e0, e1, e2, e3, w2);
+        }
+    }
     uint4 so4 = make_uint4(0u, 0u, 0u, 0u);
-    if (owner) so4 = ld_spin(x.src + row_off);
-    const uint4 bold = ld_best_early<KIND>(x, owner, row_off);
-    uint32_t flip = 0;
-    if (KIND != kKindEval && epi_warp)   // the 16 sub-row lane pairs of the epilogue warp share the Philox calls
-        flip = flip_mask_part(hd.orig, x.T, x.rep_lane0, x.thr, (uint32_t)sr, (uint32_t)kSubRows, keys);
-    for (uint32_t gi = 1;; ++gi) {
-        const uint32_t wc = w;
-        const int4 wwc = ww;
-        const bool more = gi < hd.G;
-        if (more) {
-            c = ld_stream(g.col4 + j + (size_t)(gi - 1) * kHubSub);
-            if (WIDE) ww = ld_stream(g.w4w + j + (size_t)(gi - 1) * kHubSub);
-            else w = ld_stream(g.w4 + j + (size_t)(gi - 1) * kHubSub);
+    if (owner) so4 = lds128(gb + 8 * kSlotBytes);
+
+    if (parts != 0u) {   // hub part: sorig = {caller id, hub id, part index, ...}
+        const uint32_t orig0 = __shfl_sync(0xffffffffu, orig, 0), hub = __shfl_sync(0xffffffffu, orig, 2);
+        part_finish<kKindGS>(g, x, d.row0, parts, orig0, hub, h, so4, acc, keys);
+        return;
+    }
+    // warp-level segmented reduction over the sub-rows of one row (fields add, flip bits OR)
+    if (log_spr == 4) {
+        half_reduce16(h, flip, (int)(threadIdx.x & 1));
+    } else {
+        for (int lvl = 0; lvl < log_spr; ++lvl) {
+#pragma unroll
+            for (int k = 0; k < 16; ++k) h[k] += __shfl_xor_sync(0xffffffffu, h[k], 2 << lvl);
+            flip |= __shfl_xor_sync(0xffffffffu, flip, 2 << lvl);
         }
-        if (WIDE) field_cell_wide(h, e0, e1, e2, e3, wwc);
-        else field_cell(h, e0, e1, e2, e3, wc);
-        if (!more) break;
-        e0 = ld_nbr(x.src, c.x); e1 = ld_nbr(x.src, c.y); e2 = ld_nbr(x.src, c.z); e3 = ld_nbr(x.src, c.w);
     }
-    half_reduce16(h, flip, half);
-    if (sr == 0) {
-#pragma unroll
-        for (int k = 0; k < 16; k += 4)
-            *reinterpret_cast<int4*>(&s_hub[warp][half * 16 + k]) = make_int4(h[k], h[k + 1], h[k + 2], h[k + 3]);
-    }
-    __syncthreads();
-    if (owner) {
-#pragma unroll
-        for (int k = 0; k < 16; ++k) h[k] = 0;
-        for (int wv = 0; wv < kWarpsPerCta; ++wv) {
-#pragma unroll
-            for (int k = 0; k < 16; k += 4) {
-                const int4 v = *reinterpret_cast<const int4*>(&s_hub[wv][half * 16 + k]);
-                h[k] += v.x; h[k + 1] += v.y; h[k + 2] += v.z; h[k + 3] += v.w;
-            }
-        }
-        row_update<KIND>(x, h, so4, bold, finish_flip_mask(flip, x.rep_lane0), row_off, acc);
-    }
+    if (owner) row_update<kKindGS>(x, h, so4, bold, finish_flip_mask(flip, x.rep_lane0), row_off, acc);
 }
 
 __device__ __forceinline__ PhaseRange ld_range(const PhaseRange* p) {
@@ -464,6 +609,7 @@ __device__ __forceinline__ PassCtx make_ctx(const uint8_t* src, uint8_t* dst, ui
     x.thr = thr;
     x.T = T;
     x.tie_rule = tie_rule;
+    x.tile = tile;
     return x;
 }
 
@@ -477,7 +623,6 @@ template <int KIND, bool WIDE>
 __global__ void __launch_bounds__(kSweepThreads, 1) k_sweep(const SweepParams p) {
     using AccT = typename std::conditional<WIDE, long long, int>::type;
     __shared__ long long s_acc[kMaxPersistReplicas];
-    __shared__ __align__(16) int s_hub[2][kWarpsPerCta][kTile];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int sr = lane >> 1, half = lane & 1;
     const uint32_t tiles = p.tiles;
@@ -487,28 +632,10 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_sweep(const SweepParams p)
     AccT acc[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) acc[k] = 0;
-    uint32_t rows_acc = 0, acc_tile = 0, hub_count = 0;
+    uint32_t rows_acc = 0, acc_tile = 0;
 
     for (uint32_t ph = p.phase_begin; ph < p.phase_end; ++ph) {
         const PhaseRange pr = ld_range(p.g.ranges + (size_t)ph * p.g.n_cta + blockIdx.x);
-        for (uint32_t hh = pr.h0; hh < pr.h1; ++hh) {
-            const HubHead hd = fetch_hub_head<WIDE>(p.g, hh, warp, sr);
-            for (uint32_t tile = 0; tile < tiles; ++tile, ++hub_count) {
-                const bool epi = (hub_count % kWarpsPerCta) == (uint32_t)warp;
-                if (epi && tile != acc_tile) {
-                    flush_acc(acc, s_acc + acc_tile * kTile, lane);
-                    rows_acc = 0;
-                    acc_tile = tile;
-                }
-                const PassCtx x = make_ctx(p.src, p.dst, nullptr, 0u, p.tile_stride, tile, half, p.rep0, p.thr, p.T,
-                                           p.tie_rule);
-                hub_pass<KIND, WIDE>(p.g, x, hd, hh, warp, sr, half, s_hub[hub_count & 1], epi, RegAcc<AccT>{acc}, p.keys);
-                if (epi && !WIDE && ++rows_acc >= p.flush_rows) {
-                    flush_acc(acc, s_acc + acc_tile * kTile, lane);
-                    rows_acc = 0;
-                }
-            }
-        }
         const uint32_t nu = (pr.s1 - pr.s0) * tiles;
         for (uint32_t u = warp; u < nu; u += kWarpsPerCta) {
             const uint32_t s = pr.s0 + u / tiles, tile = u % tiles;
@@ -539,7 +666,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_sweep(const SweepParams p)
 // k_anneal_gs: the persistent Gauss-Seidel annealer (int8 weights).  Cooperative launch,
 // grid = g.n_cta CTAs (one per SM at most), all co-resident.
 // ---------------------------------------------------------------------------------------------
-constexpr size_t kAnnealDynSmem = 16 * kSweepThreads * sizeof(int);   // s_dE
+constexpr size_t kAnnealDynSmem = 16 * kSweepThreads * sizeof(int) + 2 * (size_t)kGatherBufBytes + kMetaBytes + kDescBytes;   // s_dE, two gather buffers, meta / descriptor slots
 constexpr int kRangeCache = 128;   // phases whose per-CTA ranges are kept in shared memory
 
 struct AnnealParams {
@@ -564,6 +691,8 @@ struct AnnealParams {
     long long* best_out;            // [tiles*32]
     int32_t* best_sweep_out;        // [tiles*32]
     unsigned int* barrier;          // zero at launch
+    unsigned int* tickets;          // [2][n_phases] slice-ticket counters (sweep parity x phase), zero at launch
+    uint32_t ticket_chunk;          // units per ticket (0: no tickets, unit k of a warp = its static unit + k * n_static)
     int32_t resume;                 // 1: best_out / best_sweep_out hold the bests of the sweeps before this chunk
     unsigned long long* timing;     // diagnostics: [n_phases][n_cta][2] SM-clock stamps of sweep timing_sweep, or nullptr
     uint32_t timing_sweep;
@@ -598,11 +727,17 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     __shared__ PhaseRange s_ranges[kRangeCache];
     extern __shared__ int s_dE_raw[];         // dynamic: [16][kSweepThreads] per-thread energy increments (SmemAcc)
     int (*s_dE)[kSweepThreads] = reinterpret_cast<int (*)[kSweepThreads]>(s_dE_raw);
+    // two gather buffers behind s_dE; gbuf0 / gbuf0 ^ gbuf_flip: this thread's slot 0 in buffer 0 / 1
+    const uint32_t gbuf_base = (uint32_t)__cvta_generic_to_shared(s_dE_raw) + 16u * kSweepThreads * (uint32_t)sizeof(int);
+    const uint32_t gbuf0 = gbuf_base + threadIdx.x * 16u;
+    const uint32_t gbuf_flip = gbuf0 ^ (gbuf0 + kGatherBufBytes);
+    PipeAddr pa;
+    pa.meta0 = gbuf_base + 2u * kGatherBufBytes + threadIdx.x * 4u;
+    pa.desc0 = gbuf_base + 2u * kGatherBufBytes + kMetaBytes + (uint32_t)(threadIdx.x >> 5) * kDescStride;
     __shared__ long long s_E[kMaxPersistReplicas];
     __shared__ long long s_best[kMaxPersistReplicas];
     __shared__ int s_bsweep[kMaxPersistReplicas];
     __shared__ uint32_t s_mask[kMaxPersistReplicas / kTile];
-    __shared__ __align__(16) int s_hub[2][kWarpsPerCta][kTile];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int sr = lane >> 1, half = lane & 1;
     const uint32_t tiles = p.tiles, nR = p.tiles * kTile, n_cta = p.g.n_cta, C = p.g.n_phases;
@@ -619,30 +754,33 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     const SmemAcc acc{&s_dE[0][threadIdx.x]};
 #pragma unroll
     for (int k = 0; k < 16; ++k) s_dE[k][threadIdx.x] = 0;
-    uint32_t rows_acc = 0, acc_tile = 0, hub_count = 0;
+    uint32_t rows_acc = 0, acc_tile = 0;
     unsigned int epoch = 0;
 
-    // this CTA's work ranges of all phases: staged once in shared memory (first kRangeCache phases)
+    // work of all phases, staged once in shared memory (first kRangeCache phases): the slices of the whole phase
+    // (shared by all CTAs, see below)
     const PhaseRange* my_ranges = p.g.ranges + blockIdx.x;
-    for (uint32_t i = threadIdx.x; i < min(C, (uint32_t)kRangeCache); i += blockDim.x)
-        s_ranges[i] = ld_range(my_ranges + (size_t)i * n_cta);
-    __syncthreads();
-    auto range_of = [&](uint32_t ph_) {
-        return ph_ < (uint32_t)kRangeCache ? s_ranges[ph_] : ld_range(my_ranges + (size_t)ph_ * n_cta);
+    auto load_range = [&](uint32_t ph_) {
+        PhaseRange r = ld_range(my_ranges + (size_t)ph_ * n_cta);
+        r.s0 = __ldg(p.g.phase_slices + ph_);
+        r.s1 = __ldg(p.g.phase_slices + ph_ + 1);
+        return r;
     };
+    for (uint32_t i = threadIdx.x; i < min(C, (uint32_t)kRangeCache); i += blockDim.x) s_ranges[i] = load_range(i);
+    __syncthreads();
+    auto range_of = [&](uint32_t ph_) { return ph_ < (uint32_t)kRangeCache ? s_ranges[ph_] : load_range(ph_); };
+    // Slice units of a phase (heaviest first): the first n_cta * 16 are static, unit warp * n_cta + cta belongs to
+    // this warp, so its static data can be prefetched across the grid barrier; the rest are handed out by a ticket
+    // counter (one atomic per unit, requested one unit ahead), which evens out cache luck.
+    const uint32_t n_static = n_cta * (uint32_t)kWarpsPerCta;
+    const uint32_t u_static = (uint32_t)warp * n_cta + blockIdx.x;
     PhaseRange pr = range_of(0u);
     uint32_t nu = (pr.s1 - pr.s0) * tiles;
-    // one-unit lookahead of the static data (first hub, first slice), kept across the grid barrier
-    HubHead hub_nxt{};
-    if (pr.h0 < pr.h1) hub_nxt = fetch_hub_head<false>(p.g, pr.h0, warp, sr);
-    bool have = (uint32_t)warp < nu;
-    uint32_t nxt_s = 0, nxt_tile = 0;
-    SliceHead nxt{};
-    if (have) {
-        nxt_s = pr.s0 + (uint32_t)warp / tiles;
-        nxt_tile = (uint32_t)warp % tiles;
-        nxt = fetch_head<false>(p.g, nxt_s, sr);
-    }
+    // one-unit lookahead of the static data, kept across the grid barrier
+    bool have = u_static < nu;
+    HeadIdx nxt{};
+    uint32_t mslot = 0;   // meta slot of the unit whose head is in flight (`nxt`)
+    if (have) nxt = request_head(p.g, pa, mslot, pr.s0 + u_static / tiles, u_static % tiles, sr, lane);
 
     for (uint32_t t = 0; t < p.n_sweeps; ++t) {
         const uint32_t thr = __ldg(p.thr + t);
@@ -651,63 +789,85 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             const bool last_phase = ph + 1 == C;
             const bool very_last = last_phase && t + 1 == p.n_sweeps;
             const PhaseRange prn = range_of(last_phase ? 0u : ph + 1u);
+            const bool dyn = nu > n_static;   // then every warp of the grid owns a static unit
+            unsigned int* ticket_ctr = p.tickets + (size_t)(t & 1u) * C + ph;
+            if (blockIdx.x == 0 && threadIdx.x == 0) p.tickets[(size_t)((t + 1u) & 1u) * C + ph] = 0u;   // last used a sweep ago
+            unsigned int tk = 0;
+            uint32_t u_pos = u_static, chunk_left = 0;
+            if (dyn && p.ticket_chunk != 0u && lane == 0) tk = atomicAdd(ticket_ctr, 1u);
 
-            for (uint32_t hh = pr.h0; hh < pr.h1; ++hh) {
-                const HubHead hd = hub_nxt;
-                if (hh + 1 < pr.h1) hub_nxt = fetch_hub_head<false>(p.g, hh + 1, warp, sr);
-                for (uint32_t tile = 0; tile < tiles; ++tile, ++hub_count) {
-                    const bool epi = (hub_count % kWarpsPerCta) == (uint32_t)warp;
-                    if (epi && tile != acc_tile) {
+            if (have) {
+                // software pipeline: unit k is computed from gather buffer gb while the gathers of unit k+1 fly
+                // into the other buffer and the head of unit k+2 is on its way (indices -> `nxt`, the rest -> its
+                // meta slot); with tickets, the ticket of the unit after that is being drawn
+                SliceDesc pend_d{};
+                uint32_t pend_tile = 0;
+                auto stage_next = [&](uint32_t gb_) {   // needs: head of `nxt` landed (cp.async.wait_group 0 + __syncwarp)
+                    pend_d = lds_desc(pa.desc(mslot));
+                    pend_tile = lds32(pa.desc(mslot) + 16);
+                    issue_slice_gathers(p.state + (size_t)pend_tile * p.tile_stride + (size_t)half * 16, nxt, pend_d, sr, gb_);
+                    have = false;
+                    if (dyn) {
+                        uint32_t u;
+                        if (p.ticket_chunk == 0u) {
+                            u = (u_pos += n_static);
+                        } else {
+                            if (chunk_left == 0u) {   // the ticket drawn a chunk ago names the next chunk; draw the one after it
+                                u_pos = n_static + __shfl_sync(0xffffffffu, tk, 0) * p.ticket_chunk;
+                                chunk_left = p.ticket_chunk;
+                                if (u_pos < nu && lane == 0) tk = atomicAdd(ticket_ctr, 1u);
+                            }
+                            u = u_pos++;
+                            --chunk_left;
+                        }
+                        have = u < nu;
+                        if (have) {
+                            mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
+                            nxt = request_head(p.g, pa, mslot, pr.s0 + u / tiles, u % tiles, sr, lane);
+                        }
+                    }
+                };
+                uint32_t gb = gbuf0;
+                cp_async_wait<0>();
+                __syncwarp();
+                uint32_t cur_m = mslot;
+                stage_next(gb);
+                while (true) {
+                    const SliceDesc cur_d = pend_d;
+                    const uint32_t tile = pend_tile;
+                    const bool more = have;
+                    const uint32_t nxt_m = mslot;
+                    cp_async_wait<0>();   // gathers of the current unit and, if any, the head of the next one
+                    if (more) {
+                        __syncwarp();
+                        stage_next(gb ^ gbuf_flip);
+                    }
+                    if (tile != acc_tile) {
                         flush_warp(acc, s_wacc[warp], lane);
                         fold_warp(s_wacc[warp], s_acc + acc_tile * kTile, lane);
                         rows_acc = 0;
                         acc_tile = tile;
                     }
-                    const PassCtx x = make_ctx(p.state, p.state, p.best, s_mask[tile], p.tile_stride, tile, half,
-                                               p.rep0, thr, T, p.tie_rule);
-                    hub_pass<kKindGS, false>(p.g, x, hd, hh, warp, sr, half, s_hub[hub_count & 1], epi, acc, p.keys);
-                    if (epi && ++rows_acc >= p.flush_rows) {
+                    const PassCtx x = make_ctx(p.state, p.state, p.best, s_mask[tile], p.tile_stride, tile, half, p.rep0,
+                                               thr, T, p.tie_rule);
+                    slice_compute(p.g, x, cur_d, pa.meta(cur_m, 0), sr, acc, p.keys, gb);
+                    if (++rows_acc >= p.flush_rows) {
                         flush_warp(acc, s_wacc[warp], lane);
                         rows_acc = 0;
                     }
-                }
-            }
-
-            uint32_t u = (uint32_t)warp;
-            while (have) {
-                const SliceHead cur = nxt;
-                const uint32_t s = nxt_s, tile = nxt_tile;
-                u += kWarpsPerCta;
-                have = u < nu;
-                if (have) {
-                    nxt_s = pr.s0 + u / tiles;
-                    nxt_tile = u % tiles;
-                    nxt = fetch_head<false>(p.g, nxt_s, sr);
-                }
-                if (tile != acc_tile) {
-                    flush_warp(acc, s_wacc[warp], lane);
-                    fold_warp(s_wacc[warp], s_acc + acc_tile * kTile, lane);
-                    rows_acc = 0;
-                    acc_tile = tile;
-                }
-                const PassCtx x = make_ctx(p.state, p.state, p.best, s_mask[tile], p.tile_stride, tile, half, p.rep0,
-                                           thr, T, p.tie_rule);
-                slice_pass<kKindGS, false>(p.g, x, cur, s, sr, acc, p.keys);
-                if (++rows_acc >= p.flush_rows) {
-                    flush_warp(acc, s_wacc[warp], lane);
-                    rows_acc = 0;
+                    if (!more) break;
+                    gb ^= gbuf_flip;
+                    cur_m = nxt_m;
                 }
             }
 
             // static data of this warp's first slice of the next phase: issued before the barrier
             pr = prn;
             nu = (pr.s1 - pr.s0) * tiles;
-            if (!very_last && pr.h0 < pr.h1) hub_nxt = fetch_hub_head<false>(p.g, pr.h0, warp, sr);
-            have = !very_last && (uint32_t)warp < nu;
+            have = !very_last && u_static < nu;
             if (have) {
-                nxt_s = pr.s0 + (uint32_t)warp / tiles;
-                nxt_tile = (uint32_t)warp % tiles;
-                nxt = fetch_head<false>(p.g, nxt_s, sr);
+                mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
+                nxt = request_head(p.g, pa, mslot, pr.s0 + u_static / tiles, u_static % tiles, sr, lane);
             }
 
             if (last_phase) {   // a7: this sweep's energy increments -> accum slot t % 3
