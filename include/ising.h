@@ -195,7 +195,9 @@ ising_status ising_problem_info(const ising_problem* p, int32_t what, int64_t* v
  * Diagnostics of the persistent Gauss-Seidel kernel: the next ising_anneal calls record, for sweep
  * `sweep` of the call, the SM clock of every CTA when it arrives at and when it leaves the grid
  * barrier that ends each colour phase.
- *   stamps   uint64 [n_colours][n_cta][2] (arrive, leave), DEVICE; n_cta = ising_problem_info(12);
+ *   stamps   uint64 [n_colours][n_cta][8] (0 arrive, 1 leave, 2-6 stages of the first unit of warp 0: pipeline
+ *            start, gathers landed, fields done, hub part arrived, row finished; 7 unused), DEVICE;
+ *            n_cta = ising_problem_info(12);
  *            NULL switches the recording off
  * Stamps of different CTAs come from different SM clocks: compare differences within one CTA.
  */

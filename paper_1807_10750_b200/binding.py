@@ -151,10 +151,11 @@ class Problem:
         return self.info(6)
 
     def phase_timing(self, sweep: int = 0):
-        """Diagnostics: record barrier arrive/leave SM clocks of sweep `sweep` of the next GS anneal.
-        Returns the int64 device tensor [n_colours][n_cta][2] the kernel will fill."""
+        """Diagnostics: record SM clocks of sweep `sweep` of the next GS anneal (per colour phase and CTA:
+        0/1 barrier arrive / leave, 2-6 stages of the first unit of warp 0).
+        Returns the int64 device tensor [n_colours][n_cta][8] the kernel will fill."""
         t = _torch()
-        buf = t.zeros((max(1, self.n_colours), self.info(12), 2), dtype=t.int64, device="cuda")
+        buf = t.zeros((max(1, self.n_colours), self.info(12), 8), dtype=t.int64, device="cuda")
         _check(lib().ising_debug_phase_timing(self.handle, buf.data_ptr(), sweep), "ising_debug_phase_timing")
         self._keep.append(buf)
         return buf

@@ -64,7 +64,7 @@ struct GraphView {
     const SliceDesc* slices;
     const uint32_t* sorig;      // [n_slices * 16] caller id of each sub-row's row (0xffffffff: none); hub part:
                                 //   {caller id, hub id, part index, 0xffffffff ...}
-    int* hub_acc;               // [n_hubs][tiles_max][32] partial local fields of hub rows (zero between sweeps)
+    unsigned long long* hub_acc;   // [n_hubs][tiles_max][32] partial local fields of hub rows (zero between sweeps)
     unsigned int* hub_cnt;      // [n_hubs][tiles_max] parts arrived so far (monotone)
     uint32_t tiles_max;
     const PhaseRange* ranges;   // [n_phases][n_cta]

@@ -109,7 +109,7 @@ size_t workspace_need(int64_t n, int64_t nnz, int wtype, int64_t max_replicas, i
     add(sizeof(SliceDesc) * (size_t)(n_slices + 1));
     add(4 * 16 * (size_t)(n_slices + 1));     // sorig
     add(8 * (size_t)(n_slices + 1));          // slice_aux
-    add(4 * kTile * (size_t)tiles * (size_t)(n_hubs + 1));   // hub_acc
+    add(8 * kTile * (size_t)tiles * (size_t)(n_hubs + 1));   // hub_acc
     add(4 * (size_t)tiles * (size_t)(n_hubs + 1));           // hub_cnt
     add(sizeof(PhaseRange) * (size_t)(phases * kMaxCtas));
     add(16 * (size_t)(cells + 1));            // col4
@@ -147,7 +147,7 @@ struct ising_problem {
     SliceDesc* slices = nullptr;
     uint32_t* sorig = nullptr;
     uint32_t* slice_aux = nullptr;       // [n_slices][2] (hub id, part index) of hub-part slices
-    int* hub_acc = nullptr;              // [n_hubs][tiles_max][32] partial local fields of hub rows
+    unsigned long long* hub_acc = nullptr;   // [n_hubs][tiles_max][32] partial local fields of hub rows
     unsigned int* hub_cnt = nullptr;     // [n_hubs][tiles_max] parts arrived (monotone)
     PhaseRange* ranges = nullptr;
     uint32_t* phase_slices = nullptr;
@@ -412,63 +412,71 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     bool too_many_parts = false;
     auto degree_of = [&](int32_t k) { return h_row_ptr[perm[k] + 1] - h_row_ptr[perm[k]]; };
     // Edges per sub-row before a row is split over more sub-rows: 16 keeps the instruction count per edge low
-    // (throughput-bound graphs); 8 keeps every row inside the prefetched head cells, i.e. one gather round trip
-    // per phase (latency-bound graphs: fewer units in the largest phase than warps on the GPU).  A row of more
-    // than 16 sub-rows x sub_row_edges edges (a hub) is cut into P balanced PARTS, one slice each, whose partial
-    // fields meet in hub_acc (integer atomics); the part that arrives last finishes the row.
-    auto build_units = [&](int sub_row_edges) {
-        slices.clear(); slice_aux.clear(); tail_cells = 0; n_hub_rows = 0;
+    // (throughput-bound colour phases); 8 keeps every row inside the prefetched head cells, i.e. one gather round
+    // trip per phase (latency-bound phases: fewer units than warps on the GPU).  Chosen per colour phase.
+    // A row of more than 16 sub-rows x sub_row_edges edges (a hub) is cut into P balanced PARTS, one slice each,
+    // whose partial fields meet in hub_acc (integer atomics); the part that arrives last finishes the row.
+    const uint64_t tiles_all = (uint64_t)((max_replicas + kTile - 1) / kTile);
+    auto emit_colour = [&](int32_t c, int32_t k, int sub_row_edges) {   // rows k.. of colour c -> slices; returns the next row
         const int64_t part_cells_max = (int64_t)kSubRows * (sub_row_edges / 4);
+        while (k < n && h_colour[perm[k]] == c) {
+            const int64_t deg = degree_of(k);
+            const int64_t groups = (deg + 3) / 4;
+            if (groups > part_cells_max) {
+                const int64_t P = (groups + part_cells_max - 1) / part_cells_max;
+                const int64_t cpp = (groups + P - 1) / P;
+                if (P > 0x7fff) too_many_parts = true;   // packed arrival count / biased sum of part_finish
+                for (int64_t q = 0; q < P; ++q) {
+                    SliceDesc d;
+                    d.off = 0;
+                    d.row0 = (uint32_t)k;
+                    d.G = (uint32_t)((cpp + kSubRows - 1) / kSubRows);
+                    d.meta = 4u | (1u << 8) | ((uint32_t)P << 16);
+                    slices.push_back(d);
+                    slice_aux.push_back(n_hub_rows);
+                    slice_aux.push_back((uint32_t)q);
+                }
+                ++n_hub_rows;
+                ++k;
+                continue;
+            }
+            const int l = spr_log2_for_degree(deg, sub_row_edges);
+            const int rps = kSubRows >> l;
+            int nr = 1;
+            while (nr < rps && k + nr < n && h_colour[perm[k + nr]] == c &&
+                   spr_log2_for_degree(degree_of(k + nr), sub_row_edges) == l)
+                ++nr;
+            const int64_t G = std::max<int64_t>(1, (groups + (1ll << l) - 1) >> l);
+            SliceDesc d;
+            d.off = 0;
+            d.row0 = (uint32_t)k;
+            d.G = (uint32_t)G;
+            d.meta = (uint32_t)l | ((uint32_t)nr << 8);
+            slices.push_back(d);
+            slice_aux.push_back(0u);
+            slice_aux.push_back(0u);
+            k += nr;
+        }
+        return k;
+    };
+    {
         int32_t k = 0;
         for (int32_t c = 0; c < C; ++c) {
             slice_begin[c] = (uint32_t)slices.size();
-            while (k < n && h_colour[perm[k]] == c) {
-                const int64_t deg = degree_of(k);
-                const int64_t groups = (deg + 3) / 4;
-                if (groups > part_cells_max) {
-                    const int64_t P = (groups + part_cells_max - 1) / part_cells_max;
-                    const int64_t cpp = (groups + P - 1) / P;
-                    if (P > 0xffff) too_many_parts = true;
-                    for (int64_t q = 0; q < P; ++q) {
-                        SliceDesc d;
-                        d.off = 0;
-                        d.row0 = (uint32_t)k;
-                        d.G = (uint32_t)((cpp + kSubRows - 1) / kSubRows);
-                        d.meta = 4u | (1u << 8) | ((uint32_t)P << 16);
-                        slices.push_back(d);
-                        slice_aux.push_back(n_hub_rows);
-                        slice_aux.push_back((uint32_t)q);
-                        tail_cells += (uint64_t)std::max<int64_t>(0, (int64_t)d.G - kHeadGroups) * kSubRows;
-                    }
-                    ++n_hub_rows;
-                    ++k;
-                    continue;
-                }
-                const int l = spr_log2_for_degree(deg, sub_row_edges);
-                const int rps = kSubRows >> l;
-                int nr = 1;
-                while (nr < rps && k + nr < n && h_colour[perm[k + nr]] == c &&
-                       spr_log2_for_degree(degree_of(k + nr), sub_row_edges) == l)
-                    ++nr;
-                const int64_t G = std::max<int64_t>(1, (groups + (1ll << l) - 1) >> l);
-                SliceDesc d;
-                d.off = 0;
-                d.row0 = (uint32_t)k;
-                d.G = (uint32_t)G;
-                d.meta = (uint32_t)l | ((uint32_t)nr << 8);
-                slices.push_back(d);
-                slice_aux.push_back(0u);
-                slice_aux.push_back(0u);
-                tail_cells += (uint64_t)std::max<int64_t>(0, G - kHeadGroups) * kSubRows;
-                k += nr;
+            const size_t mark = slices.size();
+            const uint32_t hub_mark = n_hub_rows;
+            const int32_t k_end = emit_colour(c, k, kSubRowEdges);
+            if ((uint64_t)(slices.size() - mark) * tiles_all < (uint64_t)sm_count * kWarpsPerCta) {   // latency-bound phase
+                slices.resize(mark);
+                slice_aux.resize(2 * mark);
+                n_hub_rows = hub_mark;
+                emit_colour(c, k, kHeadGroups * 4);
             }
+            k = k_end;
         }
         slice_begin[C] = (uint32_t)slices.size();
-        uint64_t units = 0;
-        for (int32_t c = 0; c < C; ++c) units = std::max<uint64_t>(units, (uint64_t)(slice_begin[c + 1] - slice_begin[c]));
-        return units * (uint64_t)((max_replicas + kTile - 1) / kTile);
-    };
-    if (build_units(kSubRowEdges) < (uint64_t)sm_count * kWarpsPerCta) build_units(kHeadGroups * 4);
+        for (const SliceDesc& d : slices) tail_cells += (uint64_t)(d.G > (uint32_t)kHeadGroups ? d.G - kHeadGroups : 0u) * kSubRows;
+    }
     if (too_many_parts) return ISING_ERR_BAD_SHAPE;
     const uint64_t head_cells = (uint64_t)slices.size() * kSubRows * kHeadGroups;
     const uint64_t cells = head_cells + tail_cells;
@@ -547,7 +555,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     p->slices = (SliceDesc*)ws.take(sizeof(SliceDesc) * (slices.size() + 1));
     p->sorig = (uint32_t*)ws.take(4 * kSubRows * (slices.size() + 1));
     p->slice_aux = (uint32_t*)ws.take(8 * (slices.size() + 1));
-    p->hub_acc = (int*)ws.take(sizeof(int) * kTile * tiles * ((size_t)n_hub_rows + 1));
+    p->hub_acc = (unsigned long long*)ws.take(8 * kTile * tiles * ((size_t)n_hub_rows + 1));
     p->hub_cnt = (unsigned int*)ws.take(4 * tiles * ((size_t)n_hub_rows + 1));
     p->ranges = (PhaseRange*)ws.take(sizeof(PhaseRange) * ranges.size());
     p->col4 = (int4*)ws.take(16 * ((size_t)cells + 1));
@@ -593,7 +601,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         k_pack<<<blocks, 256, 0, st>>>(p->slices, p->slice_aux, (uint32_t)slices.size(), p->perm, p->inv, d_row_ptr,
                                        d_col, d_w, wtype, p->col4, p->w4, p->w4w, p->sorig);
     }
-    CKP(cudaMemsetAsync(p->hub_acc, 0, sizeof(int) * kTile * tiles * ((size_t)n_hub_rows + 1), st));
+    CKP(cudaMemsetAsync(p->hub_acc, 0, 8 * kTile * tiles * ((size_t)n_hub_rows + 1), st));
     CKP(cudaMemsetAsync(p->hub_cnt, 0, 4 * tiles * ((size_t)n_hub_rows + 1), st));
     if (want_dense) {
         p->dense = dense_create(n, max_replicas, dense_mem, dense_bytes, d_row_ptr, d_col, d_w, wtype, st);

@@ -197,7 +197,11 @@ struct PassCtx {
     uint32_t thr, T;
     int32_t tie_rule;
     uint32_t tile;         // replica tile of this unit (index into hub_acc / hub_cnt)
+    unsigned long long* stamp;   // diagnostics: SM-clock stamps of this unit's stages (one lane of one warp), or nullptr
 };
+__device__ __forceinline__ void dbg_stamp(const PassCtx& x, int k) {
+    if (x.stamp) x.stamp[k] = (unsigned long long)clock64();
+}
 
 __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
     uint32_t r;
@@ -280,10 +284,17 @@ __device__ __forceinline__ uint4 ld_best_early(const PassCtx& x, bool owner, siz
 }
 
 // Hub part (common.cuh): this warp holds, spread over its 16 sub-rows, the partial local fields of one part of
-// a hub row.  The partial sums of all parts meet in hub_acc (one warp-wide integer RED per part, so the result
-// does not depend on the order); the part that arrives last (hub_cnt) reads the totals, clears them for the
-// next sweep and finishes the row (a4-a7) like the owner lanes of an ordinary slice.
-template <int KIND, typename Acc>
+// a hub row.  The partial sums of all parts meet in hub_acc by integer atomics (the result does not depend on
+// their order); the part that arrives last reads the totals, clears them for the next sweep and finishes the
+// row (a4-a7) like the owner lanes of an ordinary slice.
+//   PACKED (int8 weights: a part's sum fits 16 bits): one 64-bit atomic per lane adds (1 << 32) + sum + 2^16 to
+//   the replica's slot and returns what the slot held: arrivals in the high word, biased sum in the low one.
+//   The warp whose lane 0 arrives last finishes the row; a lane whose own slot is not complete yet polls it
+//   (the missing atomics are in flight: they were issued together with the ones lane 0 has seen).
+//   Otherwise (int32 weights): 32-bit RED per lane, then an acq_rel arrival counter (hub_cnt).
+constexpr int kPartBias = 1 << 16;
+
+template <int KIND, bool PACKED, typename Acc>
 __device__ __forceinline__ void part_finish(const GraphView& g, const PassCtx& x, uint32_t row0, uint32_t parts,
                                             uint32_t orig, uint32_t hub, int (&h)[16], const uint4& so4,
                                             const Acc& acc, const PhiloxKeys& keys) {
@@ -294,18 +305,36 @@ __device__ __forceinline__ void part_finish(const GraphView& g, const PassCtx& x
 #pragma unroll
     for (int k = 1; k < 16; ++k) v = sr == k ? h[k] : v;   // lane (sr, half) contributes replica half * 16 + sr
     const size_t slot = (size_t)hub * g.tiles_max + x.tile;
-    int* accp = g.hub_acc + slot * kTile + half * 16;
-    asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(accp + sr), "r"(v) : "memory");
-    // arrival: the warp barrier orders the lanes' REDs before lane 0's release (cumulative), the last part's
-    // acquire orders its reads of the sums after every part's REDs
-    __syncwarp();
-    unsigned int old = 0;
-    if (lane == 0)
-        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(g.hub_cnt + slot) : "memory");
-    old = __shfl_sync(0xffffffffu, old, 0);
-    if ((old + 1u) % parts != 0u) return;
-    __syncwarp();
     const size_t row_off = (size_t)row0 * kTile;
+    int total = 0;
+    if (PACKED) {
+        unsigned long long* sp = g.hub_acc + slot * kTile + half * 16 + sr;
+        const unsigned long long mine = (1ull << 32) + (unsigned long long)(uint32_t)(v + kPartBias);
+        unsigned long long now;
+        asm volatile("atom.relaxed.gpu.global.add.u64 %0, [%1], %2;" : "=l"(now) : "l"(sp), "l"(mine) : "memory");
+        now += mine;
+        dbg_stamp(x, 5);
+        if ((uint32_t)(__shfl_sync(0xffffffffu, now, 0) >> 32) != parts) return;
+        while ((uint32_t)(now >> 32) != parts)
+            asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(now) : "l"(sp) : "memory");
+        asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(sp), "l"(0ull) : "memory");
+        total = (int)((uint32_t)now - parts * (uint32_t)kPartBias);
+    } else {
+        int* accp = reinterpret_cast<int*>(g.hub_acc + slot * kTile) + half * 16 + sr;
+        asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(accp), "r"(v) : "memory");
+        // arrival: the warp barrier orders the lanes' REDs before lane 0's release (cumulative), the last
+        // part's acquire orders its reads of the sums after every part's REDs
+        __syncwarp();
+        unsigned int old = 0;
+        if (lane == 0)
+            asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(g.hub_cnt + slot) : "memory");
+        old = __shfl_sync(0xffffffffu, old, 0);
+        dbg_stamp(x, 5);
+        if ((old + 1u) % parts != 0u) return;
+        __syncwarp();
+        total = __ldcg(accp);
+        __stcg(accp, 0);
+    }
     const uint4 bold = ld_best_early<KIND>(x, sr == 0, row_off);
     uint32_t flip = 0;
     if (KIND != kKindEval) {
@@ -313,15 +342,11 @@ __device__ __forceinline__ void part_finish(const GraphView& g, const PassCtx& x
         if (half) asm volatile("redux.sync.or.b32 %0, %0, 0xaaaaaaaa;" : "+r"(flip));
         else asm volatile("redux.sync.or.b32 %0, %0, 0x55555555;" : "+r"(flip));
     }
-    if (sr == 0) {
-        int4* ap = reinterpret_cast<int4*>(accp);
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const int4 t = __ldcg(ap + k);
-            h[4 * k] = t.x; h[4 * k + 1] = t.y; h[4 * k + 2] = t.z; h[4 * k + 3] = t.w;
-            __stcg(ap + k, make_int4(0, 0, 0, 0));
-        }
+    for (int k = 0; k < 16; ++k) h[k] = __shfl_sync(0xffffffffu, total, 2 * k + half);   // replica half * 16 + k
+    if (sr == 0) {
         row_update<KIND>(x, h, so4, bold, finish_flip_mask(flip, x.rep_lane0), row_off, acc);
+        dbg_stamp(x, 6);
     }
 }
 
@@ -403,7 +428,7 @@ __device__ __forceinline__ void slice_pass(const GraphView& g, const PassCtx& x,
 
     if (d.meta >> 16) {   // hub part: sorig = {caller id, hub id, part index, ...}
         const uint32_t orig = __shfl_sync(0xffffffffu, hd.orig, 0), hub = __shfl_sync(0xffffffffu, hd.orig, 2);
-        part_finish<KIND>(g, x, d.row0, d.meta >> 16, orig, hub, h, so4, acc, keys);
+        part_finish<KIND, !WIDE>(g, x, d.row0, d.meta >> 16, orig, hub, h, so4, acc, keys);
         return;
     }
     // warp-level segmented reduction over the sub-rows of one row (fields add, flip bits OR)
@@ -571,9 +596,10 @@ __device__ __forceinline__ void slice_compute(const GraphView& g, const PassCtx&
     uint4 so4 = make_uint4(0u, 0u, 0u, 0u);
     if (owner) so4 = lds128(gb + 8 * kSlotBytes);
 
+    dbg_stamp(x, 4);
     if (parts != 0u) {   // hub part: sorig = {caller id, hub id, part index, ...}
         const uint32_t orig0 = __shfl_sync(0xffffffffu, orig, 0), hub = __shfl_sync(0xffffffffu, orig, 2);
-        part_finish<kKindGS>(g, x, d.row0, parts, orig0, hub, h, so4, acc, keys);
+        part_finish<kKindGS, true>(g, x, d.row0, parts, orig0, hub, h, so4, acc, keys);
         return;
     }
     // warp-level segmented reduction over the sub-rows of one row (fields add, flip bits OR)
@@ -610,6 +636,7 @@ __device__ __forceinline__ PassCtx make_ctx(const uint8_t* src, uint8_t* dst, ui
     x.T = T;
     x.tie_rule = tie_rule;
     x.tile = tile;
+    x.stamp = nullptr;
     return x;
 }
 
@@ -694,7 +721,8 @@ struct AnnealParams {
     unsigned int* tickets;          // [2][n_phases] slice-ticket counters (sweep parity x phase), zero at launch
     uint32_t ticket_chunk;          // units per ticket (0: no tickets, unit k of a warp = its static unit + k * n_static)
     int32_t resume;                 // 1: best_out / best_sweep_out hold the bests of the sweeps before this chunk
-    unsigned long long* timing;     // diagnostics: [n_phases][n_cta][2] SM-clock stamps of sweep timing_sweep, or nullptr
+    unsigned long long* timing;     // diagnostics: [n_phases][n_cta][8] SM-clock stamps of sweep timing_sweep (0/1: barrier
+                                    // arrive / leave, 2-6: stages of the first unit of warp 0), or nullptr
     uint32_t timing_sweep;
     PhiloxKeys keys;
 };
@@ -831,6 +859,9 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 cp_async_wait<0>();
                 __syncwarp();
                 uint32_t cur_m = mslot;
+                bool first_unit = true;
+                unsigned long long* ts = (p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + blockIdx.x) * 8 : nullptr;
+                if (ts && threadIdx.x == 0) ts[2] = (unsigned long long)clock64();
                 stage_next(gb);
                 while (true) {
                     const SliceDesc cur_d = pend_d;
@@ -848,8 +879,10 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                         rows_acc = 0;
                         acc_tile = tile;
                     }
-                    const PassCtx x = make_ctx(p.state, p.state, p.best, s_mask[tile], p.tile_stride, tile, half, p.rep0,
-                                               thr, T, p.tie_rule);
+                    PassCtx x = make_ctx(p.state, p.state, p.best, s_mask[tile], p.tile_stride, tile, half, p.rep0,
+                                         thr, T, p.tie_rule);
+                    if (first_unit && ts && threadIdx.x == 0) { x.stamp = ts; ts[3] = (unsigned long long)clock64(); }
+                    first_unit = false;
                     slice_compute(p.g, x, cur_d, pa.meta(cur_m, 0), sr, acc, p.keys, gb);
                     if (++rows_acc >= p.flush_rows) {
                         flush_warp(acc, s_wacc[warp], lane);
@@ -904,7 +937,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 }
             }
             grid_barrier(p.barrier, epoch, n_cta,
-                         (p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + blockIdx.x) * 2 : nullptr);
+                         (p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + blockIdx.x) * 8 : nullptr);
         }
 
         // sweep end (every CTA redundantly): E, cut = (W - E)/2 (eq. 4), improved mask

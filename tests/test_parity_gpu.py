@@ -335,7 +335,7 @@ def test_phase_timing_diagnostics_do_not_change_results():
     o = oracle_anneal(wl)
     assert_same(g, o)
     t = stamps.cpu().numpy()
-    assert t.shape == (wl.n_colours, p.info(12), 2)
+    assert t.shape == (wl.n_colours, p.info(12), 8)   # 0/1: barrier arrive / leave, 2-6: stages of one unit
     assert (t[:, :, 1] >= t[:, :, 0]).all() and (t[:, :, 0] > 0).all()
 
 
