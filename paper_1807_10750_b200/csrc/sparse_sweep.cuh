@@ -307,11 +307,24 @@ __device__ __forceinline__ void part_finish(const GraphView& g, const PassCtx& x
     const size_t slot = (size_t)hub * g.tiles_max + x.tile;
     const size_t row_off = (size_t)row0 * kTile;
     int total = 0;
+    uint4 bold = make_uint4(0u, 0u, 0u, 0u);
+    uint32_t flip = 0;
+    // what only the finishing part needs (captured row, Philox flips) is computed by every part while its atomic
+    // is in flight: it shortens the chain of the part that turns out to be last
+    auto speculate = [&]() {
+        bold = ld_best_early<KIND>(x, sr == 0, row_off);
+        if (KIND != kKindEval) {
+            flip = flip_mask_part(orig, x.T, x.rep_lane0, x.thr, (uint32_t)sr, (uint32_t)kSubRows, keys);
+            if (half) asm volatile("redux.sync.or.b32 %0, %0, 0xaaaaaaaa;" : "+r"(flip));
+            else asm volatile("redux.sync.or.b32 %0, %0, 0x55555555;" : "+r"(flip));
+        }
+    };
     if (PACKED) {
         unsigned long long* sp = g.hub_acc + slot * kTile + half * 16 + sr;
         const unsigned long long mine = (1ull << 32) + (unsigned long long)(uint32_t)(v + kPartBias);
         unsigned long long now;
         asm volatile("atom.relaxed.gpu.global.add.u64 %0, [%1], %2;" : "=l"(now) : "l"(sp), "l"(mine) : "memory");
+        speculate();
         now += mine;
         dbg_stamp(x, 5);
         if ((uint32_t)(__shfl_sync(0xffffffffu, now, 0) >> 32) != parts) return;
@@ -328,19 +341,13 @@ __device__ __forceinline__ void part_finish(const GraphView& g, const PassCtx& x
         unsigned int old = 0;
         if (lane == 0)
             asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(g.hub_cnt + slot) : "memory");
+        speculate();
         old = __shfl_sync(0xffffffffu, old, 0);
         dbg_stamp(x, 5);
         if ((old + 1u) % parts != 0u) return;
         __syncwarp();
         total = __ldcg(accp);
         __stcg(accp, 0);
-    }
-    const uint4 bold = ld_best_early<KIND>(x, sr == 0, row_off);
-    uint32_t flip = 0;
-    if (KIND != kKindEval) {
-        flip = flip_mask_part(orig, x.T, x.rep_lane0, x.thr, (uint32_t)sr, (uint32_t)kSubRows, keys);
-        if (half) asm volatile("redux.sync.or.b32 %0, %0, 0xaaaaaaaa;" : "+r"(flip));
-        else asm volatile("redux.sync.or.b32 %0, %0, 0x55555555;" : "+r"(flip));
     }
 #pragma unroll
     for (int k = 0; k < 16; ++k) h[k] = __shfl_sync(0xffffffffu, total, 2 * k + half);   // replica half * 16 + k
@@ -455,6 +462,9 @@ constexpr uint32_t kGatherBufBytes = kGatherSlots * kSlotBytes;
 
 __device__ __forceinline__ void cp_async16(uint32_t smem_addr, const void* gptr) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void prefetch_l2(const void* gptr) {
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(gptr));
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
@@ -808,7 +818,8 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     bool have = u_static < nu;
     HeadIdx nxt{};
     uint32_t mslot = 0;   // meta slot of the unit whose head is in flight (`nxt`)
-    if (have) nxt = request_head(p.g, pa, mslot, pr.s0 + u_static / tiles, u_static % tiles, sr, lane);
+    if (have) nxt = tiles == 1u ? request_head(p.g, pa, mslot, pr.s0 + u_static, 0u, sr, lane)
+                              : request_head(p.g, pa, mslot, pr.s0 + u_static / tiles, u_static % tiles, sr, lane);
 
     for (uint32_t t = 0; t < p.n_sweeps; ++t) {
         const uint32_t thr = __ldg(p.thr + t);
@@ -834,6 +845,12 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                     pend_d = lds_desc(pa.desc(mslot));
                     pend_tile = lds32(pa.desc(mslot) + 16);
                     issue_slice_gathers(p.state + (size_t)pend_tile * p.tile_stride + (size_t)half * 16, nxt, pend_d, sr, gb_);
+                    if (pend_d.G > (uint32_t)kHeadGroups) {   // tail cells: towards L2 now, read when the unit is computed
+                        const size_t tail_at = (size_t)pend_d.off + sr;
+                        if (half == 0) prefetch_l2(p.g.col4 + tail_at);
+                        else if (pend_d.G > (uint32_t)kHeadGroups + 1u) prefetch_l2(p.g.col4 + tail_at + kSubRows);
+                        if (lane == 0) prefetch_l2(p.g.w4 + tail_at);
+                    }
                     have = false;
                     if (dyn) {
                         uint32_t u;
@@ -851,7 +868,8 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                         have = u < nu;
                         if (have) {
                             mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
-                            nxt = request_head(p.g, pa, mslot, pr.s0 + u / tiles, u % tiles, sr, lane);
+                            nxt = tiles == 1u ? request_head(p.g, pa, mslot, pr.s0 + u, 0u, sr, lane)
+                                              : request_head(p.g, pa, mslot, pr.s0 + u / tiles, u % tiles, sr, lane);
                         }
                     }
                 };
@@ -898,9 +916,17 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             pr = prn;
             nu = (pr.s1 - pr.s0) * tiles;
             have = !very_last && u_static < nu;
+            if (have && p.ticket_chunk == 0u && u_static + n_static < nu) {   // this warp's second unit: head towards L2
+                const uint32_t u2 = u_static + n_static;
+                const uint32_t s2 = pr.s0 + (tiles == 1u ? u2 : u2 / tiles);
+                const size_t at2 = (size_t)s2 * (kHeadGroups * kSubRows) + sr;
+                prefetch_l2(half == 0 ? p.g.col4 + at2 : p.g.col4 + at2 + kSubRows);
+                if (lane == 0) { prefetch_l2(p.g.w4 + at2); prefetch_l2(p.g.sorig + (size_t)s2 * kSubRows); prefetch_l2(p.g.slices + s2); }
+            }
             if (have) {
                 mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
-                nxt = request_head(p.g, pa, mslot, pr.s0 + u_static / tiles, u_static % tiles, sr, lane);
+                nxt = tiles == 1u ? request_head(p.g, pa, mslot, pr.s0 + u_static, 0u, sr, lane)
+                              : request_head(p.g, pa, mslot, pr.s0 + u_static / tiles, u_static % tiles, sr, lane);
             }
 
             if (last_phase) {   // a7: this sweep's energy increments -> accum slot t % 3
