@@ -76,9 +76,8 @@ __device__ __forceinline__ void field_cell_wide(int (&h)[16], const uint4& e0, c
 }
 
 __device__ __forceinline__ uint32_t nibble_to_bytemask(uint32_t nib) {
-    // bit b of nib -> byte b = 0xff
-    uint32_t m = (nib & 1u) | ((nib & 2u) << 7) | ((nib & 4u) << 14) | ((nib & 8u) << 21);
-    return m * 0xffu;
+    // bit b of nib -> byte b = 0xff (the four copies of nib at shifts 0, 7, 14, 21 do not overlap)
+    return ((nib * 0x00204081u) & 0x01010101u) * 0xffu;
 }
 
 __device__ __forceinline__ uint32_t lt4(const uint4& u, uint32_t thr) {
@@ -897,8 +896,9 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                         rows_acc = 0;
                         acc_tile = tile;
                     }
-                    PassCtx x = make_ctx(p.state, p.state, p.best, s_mask[tile], p.tile_stride, tile, half, p.rep0,
-                                         thr, T, p.tie_rule);
+                    PassCtx x = tiles == 1u ? make_ctx(p.state, p.state, p.best, s_mask[0], 0ull, 0u, half, p.rep0, thr, T, p.tie_rule)
+                                            : make_ctx(p.state, p.state, p.best, s_mask[tile], p.tile_stride, tile, half, p.rep0,
+                                                       thr, T, p.tie_rule);
                     if (first_unit && ts && threadIdx.x == 0) { x.stamp = ts; ts[3] = (unsigned long long)clock64(); }
                     first_unit = false;
                     slice_compute(p.g, x, cur_d, pa.meta(cur_m, 0), sr, acc, p.keys, gb);
