@@ -301,14 +301,82 @@ def test_run_twice_is_bit_identical():
 def test_hub_rows_with_several_tiles_and_ragged_replicas():
     wl = W.config5(n=12000, sweeps=12, replicas=75)
     deg = np.diff(wl.row_ptr)
-    assert (deg > 256).sum() > 5 and deg.max() > 1024     # CTA-wide hub rows, several groups each
+    assert (deg > 256).sum() > 5 and deg.max() > 1024     # hub rows cut into several parts each
     g = gpu_anneal(wl)
     o = oracle_anneal(wl)
     assert_same(g, o)
-    # Jacobi and evaluation share the hub pass
+    # Jacobi and evaluation share the part logic
     g = gpu_anneal(wl, mode=P.ISING_MODE_JACOBI, thr=wl.thr[:5], n_replicas=40)
     o = oracle_anneal(wl, mode=1, thr=wl.thr[:5], n_replicas=40)
     assert_same(g, o)
+
+
+def hub_graph(n, p, gseed, hub_degrees):
+    """Sparse Erdos-Renyi background plus a few hub vertices (ids 0, 1, ...) of the given degrees."""
+    u, v = W.erdos_renyi_edges(n, p, gseed)
+    us, vs = [u], [v]
+    for hid, d in enumerate(hub_degrees):
+        others = np.arange(len(hub_degrees), n, dtype=np.int64)
+        order = np.argsort(W.hash_pairs(gseed + 7 * hid + 1, np.full(others.size, hid, dtype=np.int64), others), kind="stable")
+        us.append(np.full(d, hid, dtype=np.int64))
+        vs.append(np.sort(others[order[:d]]))
+    key = np.unique(np.concatenate(us) * n + np.concatenate(vs))
+    return key // n, key % n
+
+
+def test_hub_parts_with_wide_weights_gs_and_jacobi():
+    """Hub rows cut into parts on the int32-weight path (32-bit RED + arrival counter instead of the packed
+    64-bit atomic of the int8 path), Gauss-Seidel (launch per phase) and Jacobi, three replica tiles."""
+    n = 4000
+    u, v = hub_graph(n, 0.002, 71, [1500, 700, 300, 130])
+    h = W.hash_pairs(71, u, v)
+    wt = ((h >> np.uint64(8)) % np.uint64(60001)).astype(np.int64) - 30000
+    wt[wt == 0] = 1
+    csr = W.csr_from_edges(n, u, v, wt, np.int32)
+    colour, nc = W.greedy_colouring(n, csr[0], csr[1], "ldf")
+    wl = wl_from_csr(n, csr, colour, nc, 70, W.linear_schedule(0.2, 0.0, 12), seed=5)
+    assert_same(gpu_anneal(wl), oracle_anneal(wl))
+    wlj = wl_from_csr(n, csr, None, 0, 70, W.linear_schedule(0.2, 0.0, 8), mode="jacobi", seed=5)
+    assert_same(gpu_anneal(wlj), oracle_anneal(wlj))
+
+
+@pytest.mark.parametrize("sign", [1, -1])
+def test_hub_parts_extreme_int8_partial_sums(sign):
+    """All weights +-127 and all spins +1: every hub part adds the largest partial sum the packed arrival
+    word has to hold (128 edges x 127 in latency-bound phases); zero-temperature sweeps from there."""
+    n = 3000
+    u, v = hub_graph(n, 0.001, 73, [2900, 2000, 515, 129])
+    wt = np.full(u.size, 127 * sign, dtype=np.int64)
+    csr = W.csr_from_edges(n, u, v, wt, np.int8)
+    colour, nc = W.greedy_colouring(n, csr[0], csr[1], "index")
+    thr = np.zeros(4, dtype=np.uint32)
+    wl = wl_from_csr(n, csr, colour, nc, 33, thr, seed=2)
+    init = np.ones((33, n), dtype=np.int8)
+    g = gpu_anneal(wl, init_spins=init)
+    o = oracle_anneal(wl, init_spins=init)
+    assert_same(g, o)
+
+
+def test_config5_midsize_uses_both_sub_row_lengths():
+    """300k spins: the big colour phases take 16-edge sub-rows with tail cells and 256-edge hub parts, the small
+    ones 8-edge sub-rows and 128-edge parts (chosen per phase at load)."""
+    wl = W.config5(n=300000, sweeps=5, replicas=32)
+    g = gpu_anneal(wl, want_best_spins=False)
+    assert g["problem"].info(9) > 148 * 16            # more slice units than warps on the GPU
+    o = oracle_anneal(wl)
+    assert_same(g, o, best_spins=False)
+
+
+@pytest.mark.parametrize("chunk", ["1", "3"])
+def test_ticket_scheduling_knob_gives_identical_results(chunk, monkeypatch):
+    """ISING_TICKET_CHUNK (tuning knob of the persistent kernel: units handed out by a grid-wide ticket counter
+    instead of the static stride) must not change any result."""
+    wl = W.config5(n=300000, sweeps=4, replicas=32)
+    monkeypatch.setenv("ISING_TICKET_CHUNK", chunk)
+    g = gpu_anneal(wl, want_best_spins=False)
+    monkeypatch.delenv("ISING_TICKET_CHUNK")
+    o = oracle_anneal(wl)
+    assert_same(g, o, best_spins=False)
 
 
 def test_more_replicas_than_one_persistent_launch():
