@@ -126,7 +126,7 @@ struct RegAcc {
 struct SmemAcc {
     using value_type = int;
     int* p;   // &s_dE[0][thread]; element i at p[i * kSweepThreads]
-    __device__ __forceinline__ void add(int i, int v) const { p[i * kSweepThreads] += v; }
+    __device__ __forceinline__ void add(int i, int v) const { atomicAdd(p + i * kSweepThreads, v); }   // one ATOMS instead of LDS + IADD + STS (the slot is this thread's own)
 };
 
 // Sum (or OR) over the 16 lanes of the same half (lane parity) with one REDUX per value: the even and the
