@@ -143,9 +143,9 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
  * After every sweep the cut of every replica is evaluated (eq. 4) and the best state seen
  * in THIS call is captured (strictly greater cut wins, so the earliest sweep wins ties).
  * Asynchronous on `stream`.  n_sweeps == 0 only (re)initialises the state.
- * Tuning knob (results never depend on it): environment variable ISING_TICKET_CHUNK = k > 0 makes the
- * persistent Gauss-Seidel kernel hand out its work units k at a time by a grid-wide ticket counter
- * instead of the default strided assignment.
+ * Tuning knob (results never depend on it): environment variable ISING_TICKET_MODE = 1 / 2 makes the
+ * persistent Gauss-Seidel kernel hand out its work units by a CTA-local / grid-wide ticket counter
+ * instead of the default strided assignment (0).
  */
 ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int32_t n_replicas,
                           int32_t first_replica, uint64_t seed, const uint32_t* thresholds,

@@ -59,7 +59,7 @@ inline int spr_log2_for_degree(int64_t deg, int sub_row_edges) {
     return l;
 }
 
-constexpr uint32_t kTicketChunk = 0;   // slice units per ticket of the persistent kernel; 0 = static stride (measured faster on config 5: 241 vs 261 us per sweep)
+constexpr uint32_t kTicketMode = 0;   // unit hand-out of the persistent kernel: 0 static stride, 1 CTA-local tickets, 2 grid-wide tickets
 constexpr uint32_t kThrCap = 1u << 16;   // thresholds per persistent launch (longer schedules are chunked)
 
 // Upper bounds used by ising_workspace_bytes (any degree distribution).
@@ -744,8 +744,8 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
                 a.best_sweep_out = p->sm.best_sweep + (size_t)t0 * kTile;
                 a.barrier = p->sm.barrier;
                 a.tickets = p->sm.tickets;
-                a.ticket_chunk = kTicketChunk;
-                if (const char* e = getenv("ISING_TICKET_CHUNK")) a.ticket_chunk = (uint32_t)atoi(e);   // tuning knob
+                a.ticket_mode = kTicketMode;
+                if (const char* e = getenv("ISING_TICKET_MODE")) a.ticket_mode = (uint32_t)atoi(e) % 3u;   // tuning knob
                 a.resume = s0 > 0 ? 1 : 0;
                 a.timing = (t0 == 0 && s0 == 0) ? p->timing : nullptr;
                 a.timing_sweep = p->timing_sweep;

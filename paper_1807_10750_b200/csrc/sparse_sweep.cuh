@@ -728,7 +728,9 @@ struct AnnealParams {
     int32_t* best_sweep_out;        // [tiles*32]
     unsigned int* barrier;          // zero at launch
     unsigned int* tickets;          // [2][n_phases] slice-ticket counters (sweep parity x phase), zero at launch
-    uint32_t ticket_chunk;          // units per ticket (0: no tickets, unit k of a warp = its static unit + k * n_static)
+    uint32_t ticket_mode;           // how a warp gets its units after the static first one: 0 static stride (unit k of a warp =
+                                    // its static unit + k * n_static), 1 CTA-local tickets (shared-memory counter over the CTA's
+                                    // stride set), 2 grid-wide tickets (global counter)
     int32_t resume;                 // 1: best_out / best_sweep_out hold the bests of the sweeps before this chunk
     unsigned long long* timing;     // diagnostics: [n_phases][n_cta][8] SM-clock stamps of sweep timing_sweep (0/1: barrier
                                     // arrive / leave, 2-6: stages of the first unit of warp 0), or nullptr
@@ -740,20 +742,21 @@ struct AnnealParams {
 // release-add per CTA on a monotone counter, acquire-polled by thread 0; bar.sync on both sides
 // extends the ordering to the whole CTA (PTX memory model: causality order is cumulative).
 __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& epoch, unsigned int n_cta,
-                                             unsigned long long* stamp) {
+                                             unsigned long long* stamp, unsigned int* s_next) {
     __syncthreads();
     epoch += n_cta;
     if (stamp && threadIdx.x == 0) stamp[0] = (unsigned long long)clock64();
-    if (n_cta > 1) {
-        if (threadIdx.x == 0) {
+    if (threadIdx.x == 0) {
+        *s_next = (unsigned int)kWarpsPerCta;   // CTA-local unit tickets of the next phase (no warp draws one right now)
+        if (n_cta > 1) {
             asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
             unsigned int v;
             do {
                 asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
             } while ((int)(v - epoch) < 0);
         }
-        __syncthreads();
     }
+    __syncthreads();
     if (stamp && threadIdx.x == 0) stamp[1] = (unsigned long long)clock64();
 }
 
@@ -761,8 +764,11 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     __shared__ long long s_acc[kMaxPersistReplicas];
     __shared__ long long s_wacc[kWarpsPerCta][kTile];
     __shared__ uint32_t s_wtile[kWarpsPerCta];
+    __shared__ unsigned int s_next;           // CTA-local unit tickets (ticket_mode 1)
     __shared__ PhaseRange s_ranges[kRangeCache];
-    extern __shared__ int s_dE_raw[];         // dynamic: [16][kSweepThreads] per-thread energy increments (SmemAcc)
+    // 128-byte alignment matters: a warp's 512-byte row of 16-byte slots must not straddle a fifth 128-byte line
+    // (measured: +18 % time when the static arrays happened to end 16 bytes past a line)
+    extern __shared__ __align__(128) int s_dE_raw[];         // dynamic: [16][kSweepThreads] per-thread energy increments (SmemAcc)
     int (*s_dE)[kSweepThreads] = reinterpret_cast<int (*)[kSweepThreads]>(s_dE_raw);
     // two gather buffers behind s_dE; gbuf0 / gbuf0 ^ gbuf_flip: this thread's slot 0 in buffer 0 / 1
     const uint32_t gbuf_base = (uint32_t)__cvta_generic_to_shared(s_dE_raw) + 16u * kSweepThreads * (uint32_t)sizeof(int);
@@ -785,6 +791,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
         s_bsweep[i] = p.resume ? p.best_sweep_out[i] : 0;
     }
     if (threadIdx.x < kMaxPersistReplicas / kTile) s_mask[threadIdx.x] = 0u;
+    if (threadIdx.x == 0) s_next = (unsigned int)kWarpsPerCta;
     s_wacc[threadIdx.x >> 5][threadIdx.x & 31] = 0;
     __syncthreads();
 
@@ -831,8 +838,11 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             unsigned int* ticket_ctr = p.tickets + (size_t)(t & 1u) * C + ph;
             if (blockIdx.x == 0 && threadIdx.x == 0) p.tickets[(size_t)((t + 1u) & 1u) * C + ph] = 0u;   // last used a sweep ago
             unsigned int tk = 0;
-            uint32_t u_pos = u_static, chunk_left = 0;
-            if (dyn && p.ticket_chunk != 0u && lane == 0) tk = atomicAdd(ticket_ctr, 1u);
+            uint32_t u_pos = u_static;
+            if (dyn && lane == 0) {   // ticket of this warp's second unit (drawn one unit ahead from here on)
+                if (p.ticket_mode == 1u) tk = atomicAdd(&s_next, 1u);
+                else if (p.ticket_mode == 2u) tk = atomicAdd(ticket_ctr, 1u);
+            }
 
             if (have) {
                 // software pipeline: unit k is computed from gather buffer gb while the gathers of unit k+1 fly
@@ -853,22 +863,18 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                     have = false;
                     if (dyn) {
                         uint32_t u;
-                        if (p.ticket_chunk == 0u) {
-                            u = (u_pos += n_static);
-                        } else {
-                            if (chunk_left == 0u) {   // the ticket drawn a chunk ago names the next chunk; draw the one after it
-                                u_pos = n_static + __shfl_sync(0xffffffffu, tk, 0) * p.ticket_chunk;
-                                chunk_left = p.ticket_chunk;
-                                if (u_pos < nu && lane == 0) tk = atomicAdd(ticket_ctr, 1u);
-                            }
-                            u = u_pos++;
-                            --chunk_left;
-                        }
+                        if (p.ticket_mode == 0u) u = (u_pos += n_static);
+                        else if (p.ticket_mode == 1u) u = __shfl_sync(0xffffffffu, tk, 0) * n_cta + blockIdx.x;
+                        else u = n_static + __shfl_sync(0xffffffffu, tk, 0);
                         have = u < nu;
                         if (have) {
                             mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
                             nxt = tiles == 1u ? request_head(p.g, pa, mslot, pr.s0 + u, 0u, sr, lane)
                                               : request_head(p.g, pa, mslot, pr.s0 + u / tiles, u % tiles, sr, lane);
+                            if (lane == 0) {
+                                if (p.ticket_mode == 1u) tk = atomicAdd(&s_next, 1u);
+                                else if (p.ticket_mode == 2u) tk = atomicAdd(ticket_ctr, 1u);
+                            }
                         }
                     }
                 };
@@ -916,7 +922,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             pr = prn;
             nu = (pr.s1 - pr.s0) * tiles;
             have = !very_last && u_static < nu;
-            if (have && p.ticket_chunk == 0u && u_static + n_static < nu) {   // this warp's second unit: head towards L2
+            if (have && p.ticket_mode != 2u && u_static + n_static < nu) {   // this warp's second unit: head towards L2
                 const uint32_t u2 = u_static + n_static;
                 const uint32_t s2 = pr.s0 + (tiles == 1u ? u2 : u2 / tiles);
                 const size_t at2 = (size_t)s2 * (kHeadGroups * kSubRows) + sr;
@@ -963,7 +969,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 }
             }
             grid_barrier(p.barrier, epoch, n_cta,
-                         (p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + blockIdx.x) * 8 : nullptr);
+                         (p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + blockIdx.x) * 8 : nullptr, &s_next);
         }
 
         // sweep end (every CTA redundantly): E, cut = (W - E)/2 (eq. 4), improved mask

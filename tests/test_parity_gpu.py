@@ -367,14 +367,14 @@ def test_config5_midsize_uses_both_sub_row_lengths():
     assert_same(g, o, best_spins=False)
 
 
-@pytest.mark.parametrize("chunk", ["1", "3"])
-def test_ticket_scheduling_knob_gives_identical_results(chunk, monkeypatch):
-    """ISING_TICKET_CHUNK (tuning knob of the persistent kernel: units handed out by a grid-wide ticket counter
-    instead of the static stride) must not change any result."""
+@pytest.mark.parametrize("ticket_mode", ["1", "2"])
+def test_ticket_scheduling_knob_gives_identical_results(ticket_mode, monkeypatch):
+    """ISING_TICKET_MODE (tuning knob of the persistent kernel: units handed out by a CTA-local or a grid-wide
+    ticket counter instead of the static stride) must not change any result."""
     wl = W.config5(n=300000, sweeps=4, replicas=32)
-    monkeypatch.setenv("ISING_TICKET_CHUNK", chunk)
+    monkeypatch.setenv("ISING_TICKET_MODE", ticket_mode)
     g = gpu_anneal(wl, want_best_spins=False)
-    monkeypatch.delenv("ISING_TICKET_CHUNK")
+    monkeypatch.delenv("ISING_TICKET_MODE")
     o = oracle_anneal(wl)
     assert_same(g, o, best_spins=False)
 
