@@ -315,6 +315,38 @@ def config5(n: int = 1_000_000, sweeps: int = 500, replicas: int = 32,
                    exponential_schedule(0.2, 1e-4, sweeps), "gs", "power-law sparse, %s colouring" % colouring)
 
 
+def load_edge_list(path: str, replicas: int = 32, sweeps: int = 1000, p0: float = 0.10, p_end: float = 0.0,
+                   colouring: str = "ldf", seed: int = 0, name: Optional[str] = None) -> Workload:
+    """Weighted graph from a text file in the edge-list layout the paper's benchmark files use (PAPER.md L190,
+    SURVEY 8(f) rank 4; the files themselves are not in this repo): first line `n m`, then m lines `i j w` with
+    1-based vertex ids and an integer weight.  Duplicate pairs are summed, self loops dropped, zero weights dropped.
+    Returns a Gauss-Seidel workload with a greedy colouring and a linear flip schedule p0 -> p_end."""
+    with open(path, "r") as f:
+        head = f.readline().split()
+        n, m = int(head[0]), int(head[1])
+        data = np.loadtxt(f, dtype=np.int64, ndmin=2) if m > 0 else np.zeros((0, 3), dtype=np.int64)
+    if data.shape[0] != m or (m > 0 and data.shape[1] != 3):
+        raise ValueError("%s: expected %d lines 'i j w'" % (path, m))
+    i, j, w = data[:, 0] - 1, data[:, 1] - 1, data[:, 2]
+    if m > 0 and (i.min() < 0 or j.min() < 0 or i.max() >= n or j.max() >= n):
+        raise ValueError("%s: vertex id out of range 1..%d" % (path, n))
+    keep = i != j
+    i, j, w = i[keep], j[keep], w[keep]
+    u, v = np.minimum(i, j), np.maximum(i, j)
+    key, inv = np.unique(u * n + v, return_inverse=True)
+    wsum = np.zeros(key.shape[0], dtype=np.int64)
+    np.add.at(wsum, inv, w)
+    nz = wsum != 0
+    key, wsum = key[nz], wsum[nz]
+    u, v = key // n, key % n
+    wdtype = np.int8 if (wsum.size == 0 or np.abs(wsum).max() <= 127) else np.int32
+    row_ptr, col, wt = csr_from_edges(n, u, v, wsum, wdtype)
+    colour, nc = greedy_colouring(n, row_ptr, col, colouring)
+    return Workload(name=name or os.path.basename(path), n=n, row_ptr=row_ptr, col=col, w=wt, colour=colour,
+                    n_colours=nc, n_replicas=replicas, first_replica=0, seed=seed,
+                    thr=linear_schedule(p0, p_end, sweeps), mode="gs", note="edge-list file %s" % path)
+
+
 def build_config(k: int, **kw) -> Workload:
     return {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}[k](**kw)
 

@@ -380,3 +380,82 @@ def test_generated_graphs_are_valid_inputs(k, kw):
         assert wl.nnz == n * (n - 1) and set(np.unique(wl.w)) <= set(range(-8, 9)) - {0}
     if k == 5:
         assert set(np.unique(wl.w)) <= set(range(-4, 5)) - {0}
+
+
+# ---------------------------------------------------------------------------------------------
+# edge-list file loader: the layout of the paper's benchmark files (L190), synthetic content
+# ---------------------------------------------------------------------------------------------
+def test_edge_list_loader_builds_a_valid_workload(oracle, tmp_path):
+    n = 60
+    u, v = W.erdos_renyi_edges(n, 0.15, 91)
+    wt = W.weights_from_hash(W.hash_pairs(91, u, v), "pm4")
+    lines = ["%d %d" % (n, u.size + 3)]
+    for a, b, c in zip(u, v, wt):
+        lines.append("%d %d %d" % (b + 1, a + 1, c))          # 1-based, either orientation
+    lines.append("%d %d %d" % (u[0] + 1, v[0] + 1, 2))        # duplicate pair: weights add up
+    lines.append("7 7 5")                                      # self loop: dropped
+    lines.append("%d %d %d" % (u[1] + 1, v[1] + 1, -int(wt[1])))   # cancels to zero: edge dropped
+    path = tmp_path / "graph.txt"
+    path.write_text("\n".join(lines) + "\n")
+    wl = W.load_edge_list(str(path), replicas=3, sweeps=20, colouring="index")
+    expect = wt.copy()
+    expect[0] += 2
+    keep = np.ones(u.size, dtype=bool)
+    keep[1] = False
+    ref = W.csr_from_edges(n, u[keep], v[keep], expect[keep], np.int8)
+    np.testing.assert_array_equal(wl.row_ptr, ref[0])
+    np.testing.assert_array_equal(wl.col, ref[1])
+    np.testing.assert_array_equal(wl.w, ref[2])
+    # proper colouring, usable by the oracle
+    for i in range(n):
+        nb = wl.col[wl.row_ptr[i]:wl.row_ptr[i + 1]]
+        assert np.all(wl.colour[nb] != wl.colour[i])
+    o = oracle.anneal_workload(wl, n_threads=1)
+    assert o["trace"].shape == (20, 3) and np.all(o["best_cut"] == o["trace"].max(axis=0))
+
+
+# ---------------------------------------------------------------------------------------------
+# general Ising / QUBO front door (eq. (1)-(3) L39-53): external field by the gauge reduction
+# ---------------------------------------------------------------------------------------------
+def test_field_reduction_preserves_every_energy(oracle):
+    from paper_1807_10750_b200 import frontdoor as F
+    n = 9
+    u, v = W.erdos_renyi_edges(n, 0.5, 7)
+    w = W.weights_from_hash(W.hash_pairs(7, u, v), "pm4")
+    f = (W.rand_u64(7, 3, n) % np.uint64(9)).astype(np.int64) - 4
+    n2, u2, v2, w2 = F.ising_with_field(n, u, v, w, f)
+    csr2 = W.csr_from_edges(n2, u2, v2, w2, np.int8)
+    S2 = all_states(n2)
+    E2, _ = oracle.energy_cut(n2, *csr2, S2)                 # pair energy of the augmented graph, every state
+    dec = F.decode_field_solution(S2)
+    Ef = np.array([F.field_energy(n, u, v, w, f, s) for s in dec])
+    np.testing.assert_array_equal(E2, Ef)                    # E'(s, s_n) = E_field(s * s_n), state by state
+    # and the minimum over the augmented graph is the minimum of the field problem
+    Eall = np.array([F.field_energy(n, u, v, w, f, s) for s in all_states(n)])
+    assert E2.min() == Eall.min()
+
+
+def test_qubo_to_ising_matches_enumeration():
+    from paper_1807_10750_b200 import frontdoor as F
+    n = 8
+    Q = (W.rand_u64(11, 5, n * n) % np.uint64(13)).astype(np.int64).reshape(n, n) - 6
+    u, v, w, f, const = F.qubo_to_ising(Q)
+    for code in range(1 << n):
+        x = np.array([(code >> k) & 1 for k in range(n)], dtype=np.int64)
+        s = 2 * x - 1
+        assert 4 * int(x @ Q @ x) == const + F.field_energy(n, u, v, w, f, s)
+
+
+def test_annealer_solves_a_small_field_problem(oracle):
+    from paper_1807_10750_b200 import frontdoor as F
+    n = 12
+    u, v = W.erdos_renyi_edges(n, 0.4, 13)
+    w = W.weights_from_hash(W.hash_pairs(13, u, v), "pm4")
+    f = (W.rand_u64(13, 3, n) % np.uint64(7)).astype(np.int64) - 3
+    wl = F.field_workload(n, u, v, w, f, replicas=8, sweeps=200, p0=0.2)
+    o = oracle.anneal_workload(wl, n_threads=1)
+    r = int(np.argmax(o["best_cut"]))
+    s = F.decode_field_solution(o["best_spins"][r])
+    Emin = min(F.field_energy(n, u, v, w, f, t) for t in all_states(n))
+    assert F.field_energy(n, u, v, w, f, s) == Emin
+    assert int(o["best_cut"][r]) == (wl.w_total - Emin) // 2

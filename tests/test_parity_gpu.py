@@ -407,6 +407,34 @@ def test_phase_timing_diagnostics_do_not_change_results():
     assert (t[:, :, 1] >= t[:, :, 0]).all() and (t[:, :, 0] > 0).all()
 
 
+def test_edge_list_file_workload(tmp_path):
+    """a graph read from an edge-list text file (synthetic content) through the same path."""
+    n = 700
+    u, v = hub_graph(n, 0.01, 97, [300])
+    wt = W.weights_from_hash(W.hash_pairs(97, u, v), "pm8")
+    path = tmp_path / "graph.txt"
+    path.write_text("%d %d\n" % (n, u.size) + "".join("%d %d %d\n" % (a + 1, b + 1, c) for a, b, c in zip(u, v, wt)))
+    wl = W.load_edge_list(str(path), replicas=36, sweeps=30, p0=0.15)
+    assert_same(gpu_anneal(wl), oracle_anneal(wl))
+
+
+def test_external_field_through_the_auxiliary_spin():
+    """an external field (eq. (1)-(3)) enters as one auxiliary vertex coupled to every spin with a
+    non-zero field (a hub of degree ~n); the augmented graph runs through the unchanged path."""
+    from paper_1807_10750_b200 import frontdoor as F
+    n = 3000
+    u, v = W.erdos_renyi_edges(n, 0.004, 101)
+    w = W.weights_from_hash(W.hash_pairs(101, u, v), "pm4")
+    f = (W.rand_u64(101, 3, n) % np.uint64(9)).astype(np.int64) - 4
+    wl = F.field_workload(n, u, v, w, f, replicas=33, sweeps=25, p0=0.2)
+    g = gpu_anneal(wl)
+    o = oracle_anneal(wl)
+    assert_same(g, o)
+    r = int(np.argmax(g["best_cut"]))
+    s = F.decode_field_solution(g["best_spins"][r])
+    assert F.field_energy(n, u, v, w, f, s) == wl.w_total - 2 * int(g["best_cut"][r])
+
+
 # ---------------------------------------------------------------------------------------------
 # dense tcgen05 engine (a8): K_n instances in Jacobi mode, J.S on the int8 tensor cores
 # ---------------------------------------------------------------------------------------------
