@@ -76,7 +76,7 @@ enum {
 };
 
 /* update order (Q8) */
-enum { ISING_MODE_GS = 0, ISING_MODE_JACOBI = 1, ISING_MODE_RACY = 2 };
+enum { ISING_MODE_GS = 0, ISING_MODE_JACOBI = 1, ISING_MODE_RACY = 2, ISING_MODE_EXACT_N = 3 };
 /* tie rule when h_i == 0 (L49: "If S=0, it can take any value"; Q3) */
 enum { ISING_TIE_MINUS = 0, ISING_TIE_KEEP = 1 };
 /* initial state (L82 / L169 "initialize all sigma_i"; Q4) */
@@ -127,13 +127,18 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
  * Run n_sweeps annealing sweeps on n_replicas independent replicas (Algorithm 2,
  * PAPER.md L164-184; replicas = the "number of GPU simulations" of L239 run side by side).
  *
- *   mode           ISING_MODE_GS (needs a colouring), ISING_MODE_JACOBI, or ISING_MODE_RACY
- *                  (paper-like unordered in-place update, L158; not deterministic)
+ *   mode           ISING_MODE_GS (needs a colouring), ISING_MODE_JACOBI, ISING_MODE_RACY
+ *                  (paper-like unordered in-place update, L158; not deterministic), or
+ *                  ISING_MODE_EXACT_N (Algorithm 1, L77-99; needs a colouring): every sweep is pure local
+ *                  minimisation in colour-class order, then exactly N = thresholds[t] (<= 4096, clamped
+ *                  to n) DISTINCT spins per replica are flipped, drawn as a uniform N-subset by Floyd's
+ *                  algorithm on Philox words (counter = (draw index, sweep, replica>>2, 2))
  *   tie_rule       ISING_TIE_*
  *   n_replicas     1 .. max_replicas; replica r of this call has global id first_replica + r,
  *                  which is what enters the Philox counter
  *   seed           Philox key
- *   thresholds     uint32 [n_sweeps], HOST; flip iff philox_word < thresholds[t]
+ *   thresholds     uint32 [n_sweeps], HOST; flip iff philox_word < thresholds[t] (ISING_MODE_EXACT_N: the
+ *                  number of spins to flip after sweep t)
  *   sweep_offset   absolute index of this call's first sweep (enters the Philox counter)
  *   init_mode      ISING_INIT_PHILOX: s_i = (philox(ctr=(i,0,r>>2,1))[r&3] & 1) ? +1 : -1
  *                  ISING_INIT_GIVEN: copy init_spins; ISING_INIT_CONTINUE: keep the handle's state

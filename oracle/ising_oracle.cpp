@@ -26,6 +26,8 @@
 //   * RNG (Q11): Philox4x32-10, key = 64-bit seed, counter =
 //     (spin id, absolute sweep, replica>>2, domain), word = replica & 3;
 //     flip iff word < thr[t] (unsigned, strict).  DOMAIN_FLIP = 0, DOMAIN_INIT = 1.
+//   * Algorithm 1's own flip step (L92), mode 2: after a sweep of pure minimisation flip
+//     exactly N = thr[t] distinct spins (Floyd's subset sampling on Philox words, DOMAIN_FLIPN = 2).
 //
 // Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors,
 // brute force over all 2^n cuts (n <= 20), cut identity vs an independent
@@ -37,6 +39,7 @@
 //
 // Build: g++ -O2 -std=c++17 -shared -fPIC -pthread -o liboracle.so ising_oracle.cpp
 // ===========================================================================
+#include <algorithm>
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
@@ -47,6 +50,7 @@ namespace {
 
 constexpr uint32_t DOMAIN_FLIP = 0;
 constexpr uint32_t DOMAIN_INIT = 1;
+constexpr uint32_t DOMAIN_FLIPN = 2;   // Algorithm 1's exact-N flip step: counter word 0 = draw index
 
 // Philox4x32-10 (Salmon et al., "Parallel random numbers: as easy as 1, 2, 3").
 // One round: (c0,c1,c2,c3) <- (hi(M1*c2)^c1^k0, lo(M1*c2), hi(M0*c0)^c3^k1, lo(M0*c0));
@@ -114,7 +118,7 @@ int64_t local_field(const Graph& g, const int8_t* s, int32_t i) {
 struct AnnealArgs {
     Graph g;
     const int32_t* order;     // [n] visiting order for GS (vertices sorted by (colour, id)); unused in Jacobi
-    int32_t mode;             // 0 GS, 1 Jacobi
+    int32_t mode;             // 0 GS (Algorithm 2), 1 Jacobi (Algorithm 2), 2 GS + exact-N flips (Algorithm 1)
     int32_t tie_rule;         // 0 MINUS, 1 KEEP
     int32_t n_replicas;
     int32_t first_replica;
@@ -152,7 +156,28 @@ void anneal_replica(const AnnealArgs& a, int32_t r) {
     for (int32_t t = 0; t < a.n_sweeps; ++t) {
         const uint32_t T = (uint32_t)(a.sweep_offset + t);
         const uint32_t thr = a.thr[t];
-        if (a.mode == 0) {
+        if (a.mode == 2) {
+            // Algorithm 1 (L77-99): a sweep of pure local minimisation in the sequential order, then "randomly
+            // choose and flip N spin glasses" (L92): N = thr[t] DISTINCT spins (clamped to n), drawn as a uniform
+            // N-subset by Floyd's algorithm: for j = n-N .. n-1: x = uniform integer in [0, j]; take x unless it
+            // was taken already, then take j.  The integer comes from one Philox word u (counter =
+            // (draw index, sweep, replica>>2, DOMAIN_FLIPN), word replica&3) as floor(u (j+1) / 2^32).
+            for (int32_t k = 0; k < n; ++k) {
+                const int32_t i = a.order[k];
+                s[i] = update_value(local_field(g, s.data(), i), s[i], a.tie_rule);
+            }
+            const int64_t N = std::min<int64_t>((int64_t)thr, (int64_t)n);
+            std::vector<int32_t> chosen;
+            for (int64_t j = (int64_t)n - N; j < (int64_t)n; ++j) {
+                const uint32_t u = philox_word(a.seed, (uint32_t)(j - ((int64_t)n - N)), T, rep, DOMAIN_FLIPN);
+                int32_t x = (int32_t)(((uint64_t)u * (uint64_t)(j + 1)) >> 32);
+                bool taken = false;
+                for (int32_t c : chosen) taken = taken || c == x;
+                if (taken) x = (int32_t)j;
+                chosen.push_back(x);
+            }
+            for (int32_t c : chosen) s[c] = (int8_t)-s[c];
+        } else if (a.mode == 0) {
             for (int32_t k = 0; k < n; ++k) {
                 const int32_t i = a.order[k];
                 int8_t v = update_value(local_field(g, s.data(), i), s[i], a.tie_rule);
@@ -222,7 +247,7 @@ int32_t oracle_anneal(int32_t n, const int64_t* row_ptr, const int32_t* col, con
     AnnealArgs a;
     a.g = Graph{n, row_ptr, col, wtype == 1 ? (const int8_t*)w : nullptr, wtype == 4 ? (const int32_t*)w : nullptr};
     if (!a.g.w8 && !a.g.w32) return 1;
-    if (mode == 0 && !order) return 2;
+    if ((mode == 0 || mode == 2) && !order) return 2;
     a.order = order; a.mode = mode; a.tie_rule = tie_rule;
     a.n_replicas = n_replicas; a.first_replica = first_replica; a.seed = seed;
     a.thr = thr; a.n_sweeps = n_sweeps; a.sweep_offset = sweep_offset;

@@ -16,7 +16,7 @@ import numpy as np
 
 from . import build as _build
 
-ISING_MODE_GS, ISING_MODE_JACOBI, ISING_MODE_RACY = 0, 1, 2
+ISING_MODE_GS, ISING_MODE_JACOBI, ISING_MODE_RACY, ISING_MODE_EXACT_N = 0, 1, 2, 3
 ISING_TIE_MINUS, ISING_TIE_KEEP = 0, 1
 ISING_INIT_PHILOX, ISING_INIT_GIVEN, ISING_INIT_CONTINUE = 0, 1, 2
 ISING_W_INT8, ISING_W_INT32 = 1, 4

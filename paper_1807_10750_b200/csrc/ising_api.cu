@@ -620,13 +620,16 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
                           int32_t sweep_offset, int32_t init_mode, const int8_t* init_spins, int64_t* cut_trace,
                           void* stream) {
     if (!p) return ISING_ERR_NULL_ARG;
-    if (mode < 0 || mode > 2 || tie_rule < 0 || tie_rule > 1 || init_mode < 0 || init_mode > 2 || n_sweeps < 0 ||
+    if (mode < 0 || mode > 3 || tie_rule < 0 || tie_rule > 1 || init_mode < 0 || init_mode > 2 || n_sweeps < 0 ||
         sweep_offset < 0 || first_replica < 0)
         return ISING_ERR_BAD_SHAPE;
     if (n_replicas < 1 || n_replicas > p->max_replicas) return ISING_ERR_TOO_MANY_REPLICAS;
     if (n_sweeps > 0 && !thresholds) return ISING_ERR_NULL_ARG;
     if (init_mode == ISING_INIT_GIVEN && !init_spins) return ISING_ERR_NULL_ARG;
-    if (mode == ISING_MODE_GS && p->n_colours == 0) return ISING_ERR_NO_COLOURING_FOR_GS;
+    if ((mode == ISING_MODE_GS || mode == ISING_MODE_EXACT_N) && p->n_colours == 0) return ISING_ERR_NO_COLOURING_FOR_GS;
+    if (mode == ISING_MODE_EXACT_N)
+        for (int32_t t = 0; t < n_sweeps; ++t)
+            if (thresholds[t] > (uint32_t)kMaxExactN) return ISING_ERR_BAD_SHAPE;
     if (init_mode == ISING_INIT_CONTINUE && (!p->have_state || p->last_R != n_replicas)) return ISING_ERR_NO_STATE;
     if (cut_trace && !is_device_ptr(cut_trace)) return ISING_ERR_BAD_SHAPE;
     cudaStream_t st = (cudaStream_t)stream;
@@ -792,6 +795,29 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
                                   cut_trace ? (long long*)cut_trace + (size_t)(t - 1) * n_replicas : nullptr,
                                   n_replicas, tiles, st);
             if (t < n_sweeps) p->cur ^= 1;
+        }
+    } else if (mode == ISING_MODE_EXACT_N) {
+        // Algorithm 1 (L77-99): a sweep of pure local minimisation (one launch per colour phase, no flips), then
+        // exactly N_t distinct spins per replica are flipped, then an evaluation pass for the cut
+        for (int32_t t = 0; t < n_sweeps; ++t) {
+            SweepParams q = sp;
+            q.src = p->state[p->cur]; q.dst = p->state[p->cur];
+            q.accum = p->sm.accum_eval;   // increments of the minimisation sweep: not used, the cut is evaluated below
+            q.thr = 0u; q.T = (uint32_t)(sweep_offset + t);
+            for (int32_t c = 0; c < p->n_colours; ++c) {
+                q.phase_begin = (uint32_t)c; q.phase_end = (uint32_t)c + 1;
+                launch_sweep(p, kKindGS, q, tiles, st);
+            }
+            if (thresholds[t] > 0u) {
+                k_flip_exact<<<(unsigned)n_replicas, 32, 0, st>>>(p->state[p->cur], p->inv, n, thresholds[t], q.T,
+                                                                 (uint32_t)first_replica, tile_stride, keys);
+                p->launches++;
+            }
+            SweepParams ev = sp;
+            ev.src = p->state[p->cur]; ev.dst = p->state[p->cur]; ev.accum = p->sm.accum[p->parity];
+            launch_sweep(p, kKindEval, ev, tiles, st);
+            launch_sweep_end(p, p->state[p->cur], 1, t == 0, sweep_offset + t,
+                             cut_trace ? (long long*)cut_trace + (size_t)t * n_replicas : nullptr, n_replicas, tiles, st);
         }
     } else {
         // paper-like racy in-place update of all spins (L158), then an evaluation pass for the cut

@@ -17,6 +17,7 @@ constexpr uint32_t kPhiloxW0 = 0x9E3779B9u;
 constexpr uint32_t kPhiloxW1 = 0xBB67AE85u;
 constexpr uint32_t kDomainFlip = 0u;
 constexpr uint32_t kDomainInit = 1u;
+constexpr uint32_t kDomainFlipN = 2u;   // Algorithm 1's exact-N flip step: counter word 0 = draw index
 
 // The ten round keys depend on the seed only, so the host computes them once per call
 // and the kernels receive them by value (they end up in uniform registers / constants).

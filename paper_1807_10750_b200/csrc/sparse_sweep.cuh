@@ -1166,6 +1166,36 @@ __global__ void k_export(const uint8_t* state, int8_t* out, const int32_t* perm,
         out[(size_t)rep * n + (uint32_t)perm[row]] = (int8_t)state[(size_t)tile * tile_stride + (size_t)row * kTile + rr];
 }
 
+// Algorithm 1's flip step ("randomly choose and flip N spin glasses"): after a
+// sweep of pure local minimisation exactly N DISTINCT spins of every replica are flipped.  The N-subset is drawn by
+// Floyd's algorithm: for j = n-N .. n-1: x = floor(u (j+1) / 2^32) with u = philox(seed; ctr = (j - (n-N), T,
+// r>>2, FLIPN))[r&3]; x is taken unless it was taken before, then j is.  One warp per replica: the draws are
+// sequential by definition, the membership scan over the spins chosen so far is spread over the lanes.
+constexpr int kMaxExactN = 4096;
+__global__ void __launch_bounds__(32) k_flip_exact(uint8_t* state, const int32_t* inv, uint32_t n, uint32_t N, uint32_t T,
+                                                    uint32_t rep0, unsigned long long tile_stride, const PhiloxKeys keys) {
+    __shared__ uint32_t chosen[kMaxExactN];
+    const uint32_t r = blockIdx.x, rep = rep0 + r, lane = threadIdx.x;
+    if (N > n) N = n;
+    for (uint32_t k = 0; k < N; ++k) {
+        const uint32_t j = n - N + k;
+        const uint4 v = philox4x32_10(k, T, rep >> 2, kDomainFlipN, keys);
+        const uint32_t u = (rep & 3u) == 0 ? v.x : (rep & 3u) == 1 ? v.y : (rep & 3u) == 2 ? v.z : v.w;
+        uint32_t x = (uint32_t)(((unsigned long long)u * (unsigned long long)(j + 1u)) >> 32);
+        bool taken = false;
+        for (uint32_t c = lane; c < k; c += 32) taken = taken || chosen[c] == x;
+        if (__any_sync(0xffffffffu, taken)) x = j;
+        __syncwarp();
+        if (lane == 0) chosen[k] = x;
+        __syncwarp();
+    }
+    uint8_t* base = state + (size_t)(r / kTile) * tile_stride + (r % kTile);
+    for (uint32_t c = lane; c < N; c += 32) {
+        uint8_t* q = base + (size_t)(uint32_t)inv[chosen[c]] * kTile;
+        *q = (uint8_t)(*q ^ 0xfeu);   // +1 <-> -1; distinct spins, so no two lanes touch the same byte
+    }
+}
+
 // energy_out / cut_out from an evaluation accumulator (accum = sum_i s_i h_i = 2 E).
 __global__ void k_finish_energy(const long long* accum, long long W, int32_t n_replicas, long long* energy_out,
                                 long long* cut_out) {

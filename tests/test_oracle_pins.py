@@ -459,3 +459,64 @@ def test_annealer_solves_a_small_field_problem(oracle):
     Emin = min(F.field_energy(n, u, v, w, f, t) for t in all_states(n))
     assert F.field_energy(n, u, v, w, f, s) == Emin
     assert int(o["best_cut"][r]) == (wl.w_total - Emin) // 2
+
+
+# ---------------------------------------------------------------------------------------------
+# Algorithm 1's exact-N flip step: oracle mode 2
+# ---------------------------------------------------------------------------------------------
+def _one_sweep(oracle, n, csr, order, N, init, seed=3, sweep_offset=0):
+    o = oracle.anneal(n, *csr, order=order, mode=2, n_replicas=init.shape[0], seed=seed,
+                      thr=np.array([N], dtype=np.uint32), sweep_offset=sweep_offset, init_spins=init)
+    return o["final"]
+
+
+def test_exact_n_flips_exactly_n_distinct_spins(oracle):
+    n = 90
+    csr = small_graph(n, 0.1, 17)
+    colour, nc = W.greedy_colouring(n, csr[0], csr[1], "index")
+    order = oracle.order_from_colour(colour)
+    init = W.random_spins(5, 6, n)
+    base = _one_sweep(oracle, n, csr, order, 0, init)                 # N = 0: the pure minimisation sweep
+    for N in (1, 7, 45, 89, 90, 500):
+        s = _one_sweep(oracle, n, csr, order, N, init)
+        assert np.all((s != base).sum(axis=1) == min(N, n))           # exactly N distinct spins flipped (N >= n: all)
+    # N = 0 is a descent sweep: identical to Algorithm 2 with a zero threshold
+    o0 = oracle.anneal(n, *csr, order=order, mode=0, n_replicas=6, seed=3, thr=np.zeros(1, dtype=np.uint32), init_spins=init)
+    np.testing.assert_array_equal(base, o0["final"])
+
+
+def test_exact_n_subset_is_uniform_over_the_spins(oracle):
+    """Empty graph: the minimisation sweep writes -1 everywhere (tie rule MINUS), so the +1 spins after the sweep
+    are exactly the chosen subset; over many (replica, sweep) draws every spin is chosen N/n of the time."""
+    n, N, R, M = 40, 6, 64, 60
+    row_ptr = np.zeros(n + 1, dtype=np.int64)
+    col = np.zeros(0, dtype=np.int32)
+    w = np.zeros(0, dtype=np.int8)
+    order = np.arange(n, dtype=np.int32)
+    counts = np.zeros(n, dtype=np.int64)
+    pair_seen = set()
+    for t in range(M):
+        o = oracle.anneal(n, row_ptr, col, w, order=order, mode=2, n_replicas=R, seed=11,
+                          thr=np.array([N], dtype=np.uint32), sweep_offset=t, n_threads=4)
+        chosen = o["final"] == 1
+        assert np.all(chosen.sum(axis=1) == N)
+        counts += chosen.sum(axis=0)
+        pair_seen.update(tuple(np.nonzero(c)[0]) for c in chosen)
+    draws = R * M
+    expect = draws * N / n
+    sigma = np.sqrt(draws * (N / n) * (1 - N / n))
+    assert np.all(np.abs(counts - expect) < 5 * sigma)
+    assert len(pair_seen) > 0.99 * draws          # different replicas / sweeps draw different subsets
+
+
+def test_exact_n_best_tracking_and_trace(oracle):
+    n = 60
+    csr = small_graph(n, 0.15, 23)
+    colour, nc = W.greedy_colouring(n, csr[0], csr[1], "index")
+    order = oracle.order_from_colour(colour)
+    thr = np.array([8, 6, 4, 2, 1, 0, 0], dtype=np.uint32)
+    o = oracle.anneal(n, *csr, order=order, mode=2, n_replicas=5, seed=2, thr=thr)
+    E, cut = oracle.energy_cut(n, *csr, o["final"])
+    np.testing.assert_array_equal(cut, o["trace"][-1])
+    np.testing.assert_array_equal(o["best_cut"], o["trace"].max(axis=0))
+    assert np.all(o["trace"][-1] >= o["trace"][-2])       # the last two sweeps are pure descent

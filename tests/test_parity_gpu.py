@@ -436,6 +436,33 @@ def test_external_field_through_the_auxiliary_spin():
 
 
 # ---------------------------------------------------------------------------------------------
+# Algorithm 1: minimisation sweep + exactly N distinct flips per replica
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("R", [5, 70])
+def test_exact_n_mode_matches_oracle(R):
+    wl = er_workload(1200, 0.01, 53, "pm4", np.int8, R, 1, seed=4)
+    counts = np.array([200, 150, 100, 64, 33, 7, 1, 0, 0, 4096], dtype=np.uint32)    # the last one is clamped to n
+    g = gpu_anneal(wl, thr=counts, mode=P.ISING_MODE_EXACT_N)
+    o = oracle_anneal(wl, thr=counts, mode=2)
+    assert_same(g, o)
+    # sweep split and first_replica: the draws are keyed on (draw index, absolute sweep, replica)
+    g1 = gpu_anneal(wl, thr=counts[:4], mode=P.ISING_MODE_EXACT_N, n_replicas=3, first_replica=2)
+    g2 = gpu_anneal(wl, thr=counts[4:], mode=P.ISING_MODE_EXACT_N, n_replicas=3, first_replica=2, sweep_offset=4,
+                    init_mode=P.ISING_INIT_CONTINUE, problem=g1["problem"])
+    np.testing.assert_array_equal(g2["final"], o["final"][2:5])
+
+
+def test_exact_n_mode_on_a_hub_graph():
+    wl = W.config5(n=20000, sweeps=1, replicas=32)
+    counts = np.array([300, 100, 10, 0], dtype=np.uint32)
+    g = gpu_anneal(wl, thr=counts, mode=P.ISING_MODE_EXACT_N)
+    o = oracle_anneal(wl, thr=counts, mode=2)
+    assert_same(g, o)
+    with pytest.raises(P.IsingError):
+        gpu_anneal(wl, thr=np.array([5000], dtype=np.uint32), mode=P.ISING_MODE_EXACT_N, problem=g["problem"])
+
+
+# ---------------------------------------------------------------------------------------------
 # dense tcgen05 engine (a8): K_n instances in Jacobi mode, J.S on the int8 tensor cores
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n,R,M", [(192, 40, 10), (300, 300, 6), (128, 256, 4), (520, 70, 5)])
