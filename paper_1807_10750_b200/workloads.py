@@ -252,6 +252,21 @@ def exponential_schedule(p0: float, p_end: float, m: int) -> np.ndarray:
 # --------------------------------------------------------------------------
 # the five BASELINE.json configurations (and scaled-down variants)
 # --------------------------------------------------------------------------
+def exact_n_schedule(n0: int, m: int, kind: str = "linear", factor: float = 0.01) -> np.ndarray:
+    """Numbers of spins to flip per sweep for Algorithm 1 (ISING_MODE_EXACT_N).  The paper's setting "set to 200
+    which decays linearly each sweep by a factor of 0.01" is ambiguous (reading Q6): "linear"
+    subtracts factor * n0 per sweep (N_t = max(0, round(n0 (1 - factor t))), zero after 1 / factor sweeps),
+    "geometric" multiplies by (1 - factor) per sweep."""
+    t = np.arange(m, dtype=np.float64)
+    if kind == "linear":
+        v = n0 * (1.0 - factor * t)
+    elif kind == "geometric":
+        v = n0 * (1.0 - factor) ** t
+    else:
+        raise ValueError(kind)
+    return np.maximum(0, np.rint(v)).astype(np.uint32)
+
+
 def _finish(name, n, u, v, wkind, wdtype, wseed, colouring, R, first, seed, thr, mode, note,
             torus_L=None):
     wt = weights_from_hash(hash_pairs(wseed, u, v), wkind)
