@@ -351,50 +351,90 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         d_colour = (const int32_t*)b;
     }
 
-    // ---- validate on the device
+    // ---- validate on the device.  With host inputs the O(n) planning below does not wait for it: the copies and
+    // k_validate run while the host plans (row_ptr and colour are range-checked on the host first, because the
+    // planning indexes with them); the report is read before anything is packed.
+    const bool plan_early = !rp_dev && (!colour || !co_dev);
+    if (plan_early) {
+        const int64_t* rp = row_ptr;
+        bool bad = rp[0] != 0 || rp[n] != nnz;
+        for (int32_t i = 0; i < n && !bad; ++i) bad = rp[i + 1] < rp[i] || rp[i] < 0 || rp[i + 1] > nnz;
+        if (bad) return ISING_ERR_BAD_SHAPE;
+        if (colour)
+            for (int32_t i = 0; i < n; ++i)
+                if (colour[i] < 0 || colour[i] >= n_colours) return ISING_ERR_BAD_COLOURING;
+    }
     CK(cudaMemsetAsync(d_rep, 0, sizeof(BuildReport), st));
     k_check_rowptr<<<(unsigned)((n + 1 + 255) / 256), 256, 0, st>>>(d_row_ptr, n, nnz, d_rep);
     BuildReport rep{};
-    CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    if (rep.err_mask) return ISING_ERR_BAD_SHAPE;
+    if (!plan_early) {
+        CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        if (rep.err_mask) return ISING_ERR_BAD_SHAPE;
+    }
     {
         const long long warps = n;
         const unsigned blocks = (unsigned)((warps * 32 + 255) / 256);
         k_validate<<<blocks, 256, 0, st>>>(n, d_row_ptr, d_col, d_w, wtype, d_colour, n_colours, d_rep);
     }
-    CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    CK(cudaGetLastError());
-    for (int code : {ISING_ERR_BAD_SHAPE, ISING_ERR_UNSORTED_OR_DUP, ISING_ERR_SELF_LOOP, ISING_ERR_ASYMMETRIC,
-                     ISING_ERR_BAD_COLOURING, ISING_ERR_FIELD_OVERFLOW})
-        if (rep.err_mask & (1u << code)) return code;
+    auto read_report = [&]() -> ising_status {
+        CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        CK(cudaGetLastError());
+        for (int code : {ISING_ERR_BAD_SHAPE, ISING_ERR_UNSORTED_OR_DUP, ISING_ERR_SELF_LOOP, ISING_ERR_ASYMMETRIC,
+                         ISING_ERR_BAD_COLOURING, ISING_ERR_FIELD_OVERFLOW})
+            if (rep.err_mask & (1u << code)) return code;
+        return ISING_OK;
+    };
+    if (!plan_early)
+        if (ising_status s = read_report()) return s;
 
     // ---- O(n) planning on the host: relabelling and slices
-    std::vector<int64_t> h_row_ptr(n + 1);
-    std::vector<int32_t> h_colour(n, 0);
-    if (rp_dev) CK(cudaMemcpy(h_row_ptr.data(), row_ptr, 8 * (size_t)(n + 1), cudaMemcpyDeviceToHost));
-    else std::memcpy(h_row_ptr.data(), row_ptr, 8 * (size_t)(n + 1));
-    if (colour) {
-        if (co_dev) CK(cudaMemcpy(h_colour.data(), colour, 4 * (size_t)n, cudaMemcpyDeviceToHost));
-        else std::memcpy(h_colour.data(), colour, 4 * (size_t)n);
+    std::vector<int64_t> rp_copy;
+    std::vector<int32_t> co_copy;
+    const int64_t* h_row_ptr = row_ptr;
+    const int32_t* h_colour = colour;
+    if (rp_dev) {
+        rp_copy.resize((size_t)n + 1);
+        CK(cudaMemcpy(rp_copy.data(), row_ptr, 8 * (size_t)(n + 1), cudaMemcpyDeviceToHost));
+        h_row_ptr = rp_copy.data();
+    }
+    if (colour && co_dev) {
+        co_copy.resize((size_t)n);
+        CK(cudaMemcpy(co_copy.data(), colour, 4 * (size_t)n, cudaMemcpyDeviceToHost));
+        h_colour = co_copy.data();
     }
     const int32_t C = n_colours > 0 ? n_colours : 1;
     std::vector<int32_t> perm(n), inv(n);
+    std::vector<int32_t> dsort(n);                       // degree of internal row k
+    std::vector<int64_t> cstart((size_t)C + 1, 0);       // internal rows of colour c: [cstart[c], cstart[c+1])
     {
         // stable counting sorts: by degree descending, then by colour ascending
+        std::vector<int32_t> deg(n);
         int64_t dmax = 0;
-        for (int32_t i = 0; i < n; ++i) dmax = std::max(dmax, h_row_ptr[i + 1] - h_row_ptr[i]);
-        std::vector<int64_t> cnt((size_t)dmax + 2, 0);
-        for (int32_t i = 0; i < n; ++i) cnt[(size_t)(dmax - (h_row_ptr[i + 1] - h_row_ptr[i])) + 1]++;
+        for (int32_t i = 0; i < n; ++i) {
+            const int64_t d = h_row_ptr[i + 1] - h_row_ptr[i];
+            deg[i] = (int32_t)d;
+            dmax = std::max(dmax, d);
+        }
+        std::vector<int32_t> cnt((size_t)dmax + 2, 0);
+        for (int32_t i = 0; i < n; ++i) cnt[(size_t)(dmax - deg[i]) + 1]++;
         for (size_t k = 1; k < cnt.size(); ++k) cnt[k] += cnt[k - 1];
         std::vector<int32_t> by_deg(n);
-        for (int32_t i = 0; i < n; ++i) by_deg[(size_t)cnt[(size_t)(dmax - (h_row_ptr[i + 1] - h_row_ptr[i]))]++] = i;
-        std::vector<int64_t> cc((size_t)C + 1, 0);
-        for (int32_t i = 0; i < n; ++i) cc[(size_t)h_colour[i] + 1]++;
-        for (size_t k = 1; k < cc.size(); ++k) cc[k] += cc[k - 1];
-        for (int32_t k = 0; k < n; ++k) perm[(size_t)cc[(size_t)h_colour[by_deg[k]]]++] = by_deg[k];
-        for (int32_t k = 0; k < n; ++k) inv[perm[k]] = k;
+        for (int32_t i = 0; i < n; ++i) by_deg[(size_t)cnt[(size_t)(dmax - deg[i])]++] = i;
+        if (h_colour)
+            for (int32_t i = 0; i < n; ++i) cstart[(size_t)h_colour[i] + 1]++;
+        else
+            cstart[1] = n;
+        for (size_t k = 1; k < cstart.size(); ++k) cstart[k] += cstart[k - 1];
+        std::vector<int64_t> cc(cstart.begin(), cstart.end() - 1);
+        for (int32_t k = 0; k < n; ++k) {
+            const int32_t i = by_deg[k];
+            const int64_t at = cc[h_colour ? (size_t)h_colour[i] : 0]++;
+            perm[(size_t)at] = i;
+            dsort[(size_t)at] = deg[i];
+            inv[i] = (int32_t)at;
+        }
     }
     // ---- work units: hubs (rows above kHubDegree, one CTA each) and slices (one warp each)
     int sm_count = 148, coop = 0;
@@ -410,7 +450,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     uint64_t tail_cells = 0;
     uint32_t n_hub_rows = 0;
     bool too_many_parts = false;
-    auto degree_of = [&](int32_t k) { return h_row_ptr[perm[k] + 1] - h_row_ptr[perm[k]]; };
+    auto degree_of = [&](int32_t k) { return (int64_t)dsort[k]; };
     // Edges per sub-row before a row is split over more sub-rows: 16 keeps the instruction count per edge low
     // (throughput-bound colour phases); 8 keeps every row inside the prefetched head cells, i.e. one gather round
     // trip per phase (latency-bound phases: fewer units than warps on the GPU).  Chosen per colour phase.
@@ -419,7 +459,8 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     const uint64_t tiles_all = (uint64_t)((max_replicas + kTile - 1) / kTile);
     auto emit_colour = [&](int32_t c, int32_t k, int sub_row_edges) {   // rows k.. of colour c -> slices; returns the next row
         const int64_t part_cells_max = (int64_t)kSubRows * (sub_row_edges / 4);
-        while (k < n && h_colour[perm[k]] == c) {
+        const int32_t k_end = (int32_t)cstart[(size_t)c + 1];
+        while (k < k_end) {
             const int64_t deg = degree_of(k);
             const int64_t groups = (deg + 3) / 4;
             if (groups > part_cells_max) {
@@ -443,8 +484,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
             const int l = spr_log2_for_degree(deg, sub_row_edges);
             const int rps = kSubRows >> l;
             int nr = 1;
-            while (nr < rps && k + nr < n && h_colour[perm[k + nr]] == c &&
-                   spr_log2_for_degree(degree_of(k + nr), sub_row_edges) == l)
+            while (nr < rps && k + nr < k_end && spr_log2_for_degree(degree_of(k + nr), sub_row_edges) == l)
                 ++nr;
             const int64_t G = std::max<int64_t>(1, (groups + (1ll << l) - 1) >> l);
             SliceDesc d;
@@ -477,10 +517,10 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         slice_begin[C] = (uint32_t)slices.size();
         for (const SliceDesc& d : slices) tail_cells += (uint64_t)(d.G > (uint32_t)kHeadGroups ? d.G - kHeadGroups : 0u) * kSubRows;
     }
-    if (too_many_parts) return ISING_ERR_BAD_SHAPE;
+    if (too_many_parts) { (void)cudaStreamSynchronize(st); return ISING_ERR_BAD_SHAPE; }   // the copies read the caller's arrays
     const uint64_t head_cells = (uint64_t)slices.size() * kSubRows * kHeadGroups;
     const uint64_t cells = head_cells + tail_cells;
-    if (cells > 0xffffffffull) return ISING_ERR_BAD_SHAPE;
+    if (cells > 0xffffffffull) { (void)cudaStreamSynchronize(st); return ISING_ERR_BAD_SHAPE; }
     {
         uint64_t at = head_cells;
         for (SliceDesc& d : slices) {
@@ -535,6 +575,8 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         }
     }
 
+    if (plan_early)
+        if (ising_status s = read_report()) return s;
     const bool wide = rep.max_abs_w > 127 || (uint64_t)rep.absw_max * 2ull >= (1ull << 31);
     const bool complete = n >= 2 && nnz == (int64_t)n * (n - 1);
     const bool want_dense = kDenseEnabled && complete && !(flags & ISING_LOAD_NO_DENSE) && rep.max_abs_w <= 127;
