@@ -150,7 +150,8 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
  * Asynchronous on `stream`.  n_sweeps == 0 only (re)initialises the state.
  * Tuning knob (results never depend on it): environment variable ISING_TICKET_MODE = 1 / 2 makes the
  * persistent Gauss-Seidel kernel hand out its work units by a CTA-local / grid-wide ticket counter
- * instead of the default strided assignment (0).
+ * instead of the default strided assignment (0); ISING_CLUSTER = 0 runs small graphs on the cooperative grid
+ * instead of one thread-block cluster per replica tile.
  */
 ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int32_t n_replicas,
                           int32_t first_replica, uint64_t seed, const uint32_t* thresholds,

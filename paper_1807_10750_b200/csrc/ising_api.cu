@@ -60,6 +60,7 @@ inline int spr_log2_for_degree(int64_t deg, int sub_row_edges) {
 }
 
 constexpr uint32_t kTicketMode = 0;   // unit hand-out of the persistent kernel: 0 static stride, 1 CTA-local tickets, 2 grid-wide tickets
+constexpr int kClusterCtas = 8;       // portable cluster size; 8 x 16 warps per replica tile
 constexpr uint32_t kThrCap = 1u << 16;   // thresholds per persistent launch (longer schedules are chunked)
 
 // Upper bounds used by ising_workspace_bytes (any degree distribution).
@@ -147,6 +148,7 @@ struct ising_problem {
     SliceDesc* slices = nullptr;
     uint32_t* sorig = nullptr;
     uint32_t* slice_aux = nullptr;       // [n_slices][2] (hub id, part index) of hub-part slices
+    int cluster_ctas = 0;                // small graph: the persistent kernel runs as one cluster of this many CTAs per replica tile (0: grid)
     unsigned long long* hub_acc = nullptr;   // [n_hubs][tiles_max][32] partial local fields of hub rows
     unsigned int* hub_cnt = nullptr;     // [n_hubs][tiles_max] parts arrived (monotone)
     PhaseRange* ranges = nullptr;
@@ -547,6 +549,8 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
             units = std::max<uint64_t>(units, (uint64_t)(slice_begin[c + 1] - slice_begin[c]) * tiles_max);
         n_cta = (uint32_t)std::min<uint64_t>(units, (uint64_t)std::min<int>(sm_count, (int)kMaxCtas));
     }
+    uint32_t max_phase_slices = 0;
+    for (int32_t c = 0; c < C; ++c) max_phase_slices = std::max(max_phase_slices, slice_begin[c + 1] - slice_begin[c]);
     std::vector<PhaseRange> ranges((size_t)C * n_cta);
     for (int32_t c = 0; c < C; ++c) {
         double total = 0;
@@ -587,6 +591,9 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     p->tiles_max = (max_replicas + kTile - 1) / kTile;
     p->W = rep.w_sum / 2; p->absw_max = rep.absw_max; p->wide = wide;
     p->n_slices = (uint32_t)slices.size(); p->n_hubs = n_hub_rows; p->cells = cells;
+    // latency-bound graphs whose biggest phase fits two rounds of one cluster's warps: cluster barrier instead of grid barrier
+    p->cluster_ctas = max_phase_slices <= 2u * kClusterCtas * kWarpsPerCta ? kClusterCtas : 0;   // (16-CTA clusters measured
+    // slower on config 3: 108 vs 73 ms, the eight clusters do not all fit at once)
     p->n_phases = (uint32_t)C; p->n_cta = n_cta; p->sm_count = sm_count; p->cooperative = coop != 0;
     p->flush_rows = wide ? 0x7fffffffu
                          : (uint32_t)std::max<int64_t>(1, ((1ll << 31) - 1) / std::max<int64_t>(1, 2 * rep.absw_max));
@@ -649,7 +656,8 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         p->dense = dense_create(n, max_replicas, dense_mem, dense_bytes, d_row_ptr, d_col, d_w, wtype, st);
         if (!p->dense) return fail(ISING_ERR_CUDA);
     }
-    CKP(cudaFuncSetAttribute(k_anneal_gs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
+    CKP(cudaFuncSetAttribute(k_anneal_gs<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
+    CKP(cudaFuncSetAttribute(k_anneal_gs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
     CKP(cudaStreamSynchronize(st));   // the host vectors die at return
     CKP(cudaGetLastError());
 #undef CKP
@@ -795,9 +803,27 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
                 a.timing = (t0 == 0 && s0 == 0) ? p->timing : nullptr;
                 a.timing_sweep = p->timing_sweep;
                 a.keys = keys;
-                void* args[] = {&a};
-                CK(cudaLaunchCooperativeKernel((const void*)k_anneal_gs, dim3(p->n_cta), dim3(kSweepThreads), args,
-                                               kAnnealDynSmem, st));
+                bool cluster = p->cluster_ctas > 0 && !p->timing;   // (the phase-timing diagnostics belong to the grid kernel)
+                if (const char* e = getenv("ISING_CLUSTER")) cluster = cluster && atoi(e) != 0;   // tuning knob
+                if (cluster) {
+                    // small graph: one cluster of kClusterCtas CTAs per replica tile, hardware cluster barrier
+                    a.ticket_mode = 0;
+                    cudaLaunchConfig_t cfg{};
+                    cfg.gridDim = dim3((unsigned)(bt * p->cluster_ctas));
+                    cfg.blockDim = dim3(kSweepThreads);
+                    cfg.dynamicSmemBytes = kAnnealDynSmem;
+                    cfg.stream = st;
+                    cudaLaunchAttribute at[1];
+                    at[0].id = cudaLaunchAttributeClusterDimension;
+                    at[0].val.clusterDim.x = (unsigned)p->cluster_ctas; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+                    cfg.attrs = at;
+                    cfg.numAttrs = 1;
+                    CK(cudaLaunchKernelEx(&cfg, k_anneal_gs<true>, a));
+                } else {
+                    void* args[] = {&a};
+                    CK(cudaLaunchCooperativeKernel((const void*)k_anneal_gs<false>, dim3(p->n_cta), dim3(kSweepThreads), args,
+                                                   kAnnealDynSmem, st));
+                }
                 p->launches++;
             }
         }

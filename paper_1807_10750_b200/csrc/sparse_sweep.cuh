@@ -741,8 +741,13 @@ struct AnnealParams {
 // Grid barrier of the persistent kernel (all CTAs co-resident: cooperative launch).  One
 // release-add per CTA on a monotone counter, acquire-polled by thread 0; bar.sync on both sides
 // extends the ordering to the whole CTA (PTX memory model: causality order is cumulative).
+template <bool CLUSTER>
 __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& epoch, unsigned int n_cta,
                                              unsigned long long* stamp, unsigned int* s_next) {
+    if (CLUSTER) {   // hardware barrier of the thread-block cluster; release / acquire at cluster scope covers global memory
+        asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+        return;
+    }
     __syncthreads();
     epoch += n_cta;
     if (stamp && threadIdx.x == 0) stamp[0] = (unsigned long long)clock64();
@@ -760,6 +765,7 @@ __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int
     if (stamp && threadIdx.x == 0) stamp[1] = (unsigned long long)clock64();
 }
 
+template <bool CLUSTER>
 __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealParams p) {
     __shared__ long long s_acc[kMaxPersistReplicas];
     __shared__ long long s_wacc[kWarpsPerCta][kTile];
@@ -783,12 +789,32 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     __shared__ uint32_t s_mask[kMaxPersistReplicas / kTile];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int sr = lane >> 1, half = lane & 1;
-    const uint32_t tiles = p.tiles, nR = p.tiles * kTile, n_cta = p.g.n_cta, C = p.g.n_phases;
+    // CLUSTER: one thread-block cluster per replica tile (small graphs: the units of a phase fit the warps of a few
+    // SMs): the CTAs of a cluster share nothing with the other clusters, and the barrier between colour phases is
+    // the hardware cluster barrier (~0.2 us) instead of the grid barrier (~1 us).  Otherwise: one cooperative grid
+    // for all tiles.
+    uint32_t cta = blockIdx.x, n_cta = p.g.n_cta, tile0 = 0;
+    if (CLUSTER) {
+        asm("mov.u32 %0, %%cluster_ctarank;" : "=r"(cta));
+        asm("mov.u32 %0, %%cluster_nctarank;" : "=r"(n_cta));
+        asm("mov.u32 %0, %%clusterid.x;" : "=r"(tile0));
+    }
+    const uint32_t tiles = CLUSTER ? 1u : p.tiles, nR = tiles * kTile, C = p.g.n_phases;
+    uint8_t* const state = p.state + (size_t)tile0 * p.tile_stride;
+    uint8_t* const bestp = p.best + (size_t)tile0 * p.tile_stride;
+    const long long* const E0 = p.E0 + tile0 * kTile;
+    long long* const accum = p.accum + (size_t)tile0 * 3u * kTile;
+    long long* const trace = p.trace ? p.trace + tile0 * kTile : nullptr;
+    long long* const E_out = p.E_out + tile0 * kTile;
+    long long* const best_out = p.best_out + tile0 * kTile;
+    int32_t* const best_sweep_out = p.best_sweep_out + tile0 * kTile;
+    const uint32_t rep0 = p.rep0 + tile0 * kTile;
+    const uint32_t n_rep = p.n_replicas > tile0 * kTile ? min(p.n_replicas - tile0 * kTile, nR) : 0u;
     for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {
         s_acc[i] = 0;
-        s_E[i] = p.E0[i];
-        s_best[i] = p.resume ? p.best_out[i] : (long long)0x8000000000000000ull;
-        s_bsweep[i] = p.resume ? p.best_sweep_out[i] : 0;
+        s_E[i] = E0[i];
+        s_best[i] = p.resume ? best_out[i] : (long long)0x8000000000000000ull;
+        s_bsweep[i] = p.resume ? best_sweep_out[i] : 0;
     }
     if (threadIdx.x < kMaxPersistReplicas / kTile) s_mask[threadIdx.x] = 0u;
     if (threadIdx.x == 0) s_next = (unsigned int)kWarpsPerCta;
@@ -803,9 +829,10 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
 
     // work of all phases, staged once in shared memory (first kRangeCache phases): the slices of the whole phase
     // (shared by all CTAs, see below)
-    const PhaseRange* my_ranges = p.g.ranges + blockIdx.x;
+    const PhaseRange* my_ranges = p.g.ranges + cta;
     auto load_range = [&](uint32_t ph_) {
-        PhaseRange r = ld_range(my_ranges + (size_t)ph_ * n_cta);
+        PhaseRange r{};
+        if (!CLUSTER) r = ld_range(my_ranges + (size_t)ph_ * n_cta);   // (only the CTA-major flag h0; built for the grid)
         r.s0 = __ldg(p.g.phase_slices + ph_);
         r.s1 = __ldg(p.g.phase_slices + ph_ + 1);
         return r;
@@ -817,7 +844,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     // this warp, so its static data can be prefetched across the grid barrier; the rest are handed out by a ticket
     // counter (one atomic per unit, requested one unit ahead), which evens out cache luck.
     const uint32_t n_static = n_cta * (uint32_t)kWarpsPerCta;
-    const uint32_t u_static = (uint32_t)warp * n_cta + blockIdx.x;
+    const uint32_t u_static = (uint32_t)warp * n_cta + cta;
     PhaseRange pr = range_of(0u);
     uint32_t nu = (pr.s1 - pr.s0) * tiles;
     // one-unit lookahead of the static data, kept across the grid barrier
@@ -836,7 +863,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             const PhaseRange prn = range_of(last_phase ? 0u : ph + 1u);
             const bool dyn = nu > n_static;   // then every warp of the grid owns a static unit
             unsigned int* ticket_ctr = p.tickets + (size_t)(t & 1u) * C + ph;
-            if (blockIdx.x == 0 && threadIdx.x == 0) p.tickets[(size_t)((t + 1u) & 1u) * C + ph] = 0u;   // last used a sweep ago
+            if (!CLUSTER && cta == 0 && threadIdx.x == 0) p.tickets[(size_t)((t + 1u) & 1u) * C + ph] = 0u;   // last used a sweep ago
             unsigned int tk = 0;
             uint32_t u_pos = u_static;
             if (dyn && lane == 0) {   // ticket of this warp's second unit (drawn one unit ahead from here on)
@@ -853,7 +880,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 auto stage_next = [&](uint32_t gb_) {   // needs: head of `nxt` landed (cp.async.wait_group 0 + __syncwarp)
                     pend_d = lds_desc(pa.desc(mslot));
                     pend_tile = lds32(pa.desc(mslot) + 16);
-                    issue_slice_gathers(p.state + (size_t)pend_tile * p.tile_stride + (size_t)half * 16, nxt, pend_d, sr, gb_);
+                    issue_slice_gathers(state + (size_t)pend_tile * p.tile_stride + (size_t)half * 16, nxt, pend_d, sr, gb_);
                     if (pend_d.G > (uint32_t)kHeadGroups) {   // tail cells: towards L2 now, read when the unit is computed
                         const size_t tail_at = (size_t)pend_d.off + sr;
                         if (half == 0) prefetch_l2(p.g.col4 + tail_at);
@@ -864,7 +891,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                     if (dyn) {
                         uint32_t u;
                         if (p.ticket_mode == 0u) u = (u_pos += n_static);
-                        else if (p.ticket_mode == 1u) u = __shfl_sync(0xffffffffu, tk, 0) * n_cta + blockIdx.x;
+                        else if (p.ticket_mode == 1u) u = __shfl_sync(0xffffffffu, tk, 0) * n_cta + cta;
                         else u = n_static + __shfl_sync(0xffffffffu, tk, 0);
                         have = u < nu;
                         if (have) {
@@ -883,7 +910,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 __syncwarp();
                 uint32_t cur_m = mslot;
                 bool first_unit = true;
-                unsigned long long* ts = (p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + blockIdx.x) * 8 : nullptr;
+                unsigned long long* ts = (!CLUSTER && p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + cta) * 8 : nullptr;
                 if (ts && threadIdx.x == 0) ts[2] = (unsigned long long)clock64();
                 stage_next(gb);
                 while (true) {
@@ -902,9 +929,10 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                         rows_acc = 0;
                         acc_tile = tile;
                     }
-                    PassCtx x = tiles == 1u ? make_ctx(p.state, p.state, p.best, s_mask[0], 0ull, 0u, half, p.rep0, thr, T, p.tie_rule)
-                                            : make_ctx(p.state, p.state, p.best, s_mask[tile], p.tile_stride, tile, half, p.rep0,
+                    PassCtx x = tiles == 1u ? make_ctx(state, state, bestp, s_mask[0], 0ull, 0u, half, rep0, thr, T, p.tie_rule)
+                                            : make_ctx(state, state, bestp, s_mask[tile], p.tile_stride, tile, half, rep0,
                                                        thr, T, p.tie_rule);
+                    x.tile += tile0;   // hub accumulators are indexed by the global tile
                     if (first_unit && ts && threadIdx.x == 0) { x.stamp = ts; ts[3] = (unsigned long long)clock64(); }
                     first_unit = false;
                     slice_compute(p.g, x, cur_d, pa.meta(cur_m, 0), sr, acc, p.keys, gb);
@@ -940,7 +968,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 rows_acc = 0;
                 if (lane == 0) s_wtile[warp] = acc_tile;
                 __syncthreads();
-                long long* slot = p.accum + (size_t)(t % 3u) * nR;
+                long long* slot = accum + (size_t)(t % 3u) * nR;
                 if (threadIdx.x < kTile) {   // one add per replica and run of warps on the same tile
                     long long run = 0;
                     uint32_t run_tile = s_wtile[0];
@@ -968,26 +996,26 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                     }
                 }
             }
-            grid_barrier(p.barrier, epoch, n_cta,
-                         (p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + blockIdx.x) * 8 : nullptr, &s_next);
+            grid_barrier<CLUSTER>(p.barrier, epoch, n_cta,
+                         (!CLUSTER && p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + cta) * 8 : nullptr, &s_next);
         }
 
         // sweep end (every CTA redundantly): E, cut = (W - E)/2 (eq. 4), improved mask
         {
-            const long long* slot = p.accum + (size_t)(t % 3u) * nR;
-            long long* zero_slot = p.accum + (size_t)((t + 2u) % 3u) * nR;
+            const long long* slot = accum + (size_t)(t % 3u) * nR;
+            long long* zero_slot = accum + (size_t)((t + 2u) % 3u) * nR;
             for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {   // nR is a multiple of 32: warp-uniform
                 const long long E = s_E[i] + __ldcg(slot + i);
                 const long long cut = (p.W - E) / 2;
-                const bool live = i < p.n_replicas;
+                const bool live = i < n_rep;
                 const bool improved = live && cut > s_best[i];
                 s_E[i] = E;
                 if (improved) { s_best[i] = cut; s_bsweep[i] = (int)T; }
                 const uint32_t m = __ballot_sync(0xffffffffu, improved);
                 if (lane == 0) s_mask[i >> 5] = m;
-                if (blockIdx.x == 0) {
+                if (cta == 0) {
                     zero_slot[i] = 0;
-                    if (live && p.trace) p.trace[(size_t)t * p.trace_stride + i] = cut;
+                    if (live && trace) trace[(size_t)t * p.trace_stride + i] = cut;
                 }
             }
             __syncthreads();
@@ -998,12 +1026,12 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     for (uint32_t tile = 0; tile < tiles; ++tile) {
         const uint32_t mask = s_mask[tile];
         if (mask == 0u) continue;
-        const uint4* src = reinterpret_cast<const uint4*>(p.state + (size_t)tile * p.tile_stride);
-        uint4* best = reinterpret_cast<uint4*>(p.best + (size_t)tile * p.tile_stride);
+        const uint4* src = reinterpret_cast<const uint4*>(state + (size_t)tile * p.tile_stride);
+        uint4* best = reinterpret_cast<uint4*>(bestp + (size_t)tile * p.tile_stride);
         const uint32_t m_lo = mask & 0xffffu, m_hi = mask >> 16;
         const unsigned long long units = p.n * 2ull;
-        for (unsigned long long uu = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; uu < units;
-             uu += (unsigned long long)gridDim.x * blockDim.x) {
+        for (unsigned long long uu = (unsigned long long)cta * blockDim.x + threadIdx.x; uu < units;
+             uu += (unsigned long long)n_cta * blockDim.x) {
             const uint32_t m = (uu & 1ull) ? m_hi : m_lo;
             if (m == 0u) continue;
             const uint4 s = __ldcg(src + uu);
@@ -1018,11 +1046,11 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             best[uu] = b;
         }
     }
-    if (blockIdx.x == 0) {
+    if (cta == 0) {
         for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {
-            p.E_out[i] = s_E[i];
-            p.best_out[i] = s_best[i];
-            p.best_sweep_out[i] = s_bsweep[i];
+            E_out[i] = s_E[i];
+            best_out[i] = s_best[i];
+            best_sweep_out[i] = s_bsweep[i];
         }
     }
 }

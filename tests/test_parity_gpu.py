@@ -379,6 +379,22 @@ def test_ticket_scheduling_knob_gives_identical_results(ticket_mode, monkeypatch
     assert_same(g, o, best_spins=False)
 
 
+@pytest.mark.parametrize("cluster", ["0", "1"])
+def test_small_graph_through_grid_and_cluster_kernels(cluster, monkeypatch):
+    """Small graphs run the persistent kernel as one thread-block cluster per replica tile (hardware cluster barrier
+    between colour phases); ISING_CLUSTER=0 forces the cooperative-grid variant.  Both must match the oracle, also
+    with several tiles, a ragged replica count, KEEP ties and a continued run."""
+    monkeypatch.setenv("ISING_CLUSTER", cluster)
+    wl = er_workload(900, 0.015, 67, "pm4", np.int8, 75, 40, seed=6, p0=0.2)
+    g = gpu_anneal(wl, tie_rule=1)
+    o = oracle_anneal(wl, tie_rule=1)
+    assert_same(g, o)
+    g1 = gpu_anneal(wl, thr=wl.thr[:15], problem=g["problem"])
+    g2 = gpu_anneal(wl, thr=wl.thr[15:], sweep_offset=15, init_mode=P.ISING_INIT_CONTINUE, problem=g["problem"])
+    np.testing.assert_array_equal(g2["final"], oracle_anneal(wl)["final"])
+    monkeypatch.delenv("ISING_CLUSTER")
+
+
 def test_more_replicas_than_one_persistent_launch():
     wl = er_workload(300, 0.05, 23, "pm4", np.int8, 1100, 6, p0=0.3)
     g = gpu_anneal(wl, want_best_spins=False)
