@@ -800,21 +800,22 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
         asm("mov.u32 %0, %%clusterid.x;" : "=r"(tile0));
     }
     const uint32_t tiles = CLUSTER ? 1u : p.tiles, nR = tiles * kTile, C = p.g.n_phases;
-    uint8_t* const state = p.state + (size_t)tile0 * p.tile_stride;
-    uint8_t* const bestp = p.best + (size_t)tile0 * p.tile_stride;
-    const long long* const E0 = p.E0 + tile0 * kTile;
-    long long* const accum = p.accum + (size_t)tile0 * 3u * kTile;
-    long long* const trace = p.trace ? p.trace + tile0 * kTile : nullptr;
-    long long* const E_out = p.E_out + tile0 * kTile;
-    long long* const best_out = p.best_out + tile0 * kTile;
-    int32_t* const best_sweep_out = p.best_sweep_out + tile0 * kTile;
-    const uint32_t rep0 = p.rep0 + tile0 * kTile;
-    const uint32_t n_rep = p.n_replicas > tile0 * kTile ? min(p.n_replicas - tile0 * kTile, nR) : 0u;
+    // per-tile views of the launch parameters (grid variant: the parameters themselves, read where they are used)
+    auto state = [&]() { return CLUSTER ? p.state + (size_t)tile0 * p.tile_stride : p.state; };
+    auto bestp = [&]() { return CLUSTER ? p.best + (size_t)tile0 * p.tile_stride : p.best; };
+    auto E0 = [&]() { return CLUSTER ? p.E0 + tile0 * kTile : p.E0; };
+    auto accum = [&]() { return CLUSTER ? p.accum + (size_t)tile0 * 3u * kTile : p.accum; };
+    auto trace = [&]() { return (CLUSTER && p.trace) ? p.trace + tile0 * kTile : p.trace; };
+    auto E_out = [&]() { return CLUSTER ? p.E_out + tile0 * kTile : p.E_out; };
+    auto best_out = [&]() { return CLUSTER ? p.best_out + tile0 * kTile : p.best_out; };
+    auto best_sweep_out = [&]() { return CLUSTER ? p.best_sweep_out + tile0 * kTile : p.best_sweep_out; };
+    auto rep0 = [&]() { return CLUSTER ? p.rep0 + tile0 * kTile : p.rep0; };
+    auto n_rep = [&]() { return CLUSTER ? (p.n_replicas > tile0 * kTile ? min(p.n_replicas - tile0 * kTile, nR) : 0u) : p.n_replicas; };
     for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {
         s_acc[i] = 0;
-        s_E[i] = E0[i];
-        s_best[i] = p.resume ? best_out[i] : (long long)0x8000000000000000ull;
-        s_bsweep[i] = p.resume ? best_sweep_out[i] : 0;
+        s_E[i] = E0()[i];
+        s_best[i] = p.resume ? best_out()[i] : (long long)0x8000000000000000ull;
+        s_bsweep[i] = p.resume ? best_sweep_out()[i] : 0;
     }
     if (threadIdx.x < kMaxPersistReplicas / kTile) s_mask[threadIdx.x] = 0u;
     if (threadIdx.x == 0) s_next = (unsigned int)kWarpsPerCta;
@@ -831,8 +832,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     // (shared by all CTAs, see below)
     const PhaseRange* my_ranges = p.g.ranges + cta;
     auto load_range = [&](uint32_t ph_) {
-        PhaseRange r{};
-        if (!CLUSTER) r = ld_range(my_ranges + (size_t)ph_ * n_cta);   // (only the CTA-major flag h0; built for the grid)
+        PhaseRange r = ld_range(CLUSTER ? p.g.ranges : my_ranges + (size_t)ph_ * n_cta);   // (s0 / s1 are replaced below)
         r.s0 = __ldg(p.g.phase_slices + ph_);
         r.s1 = __ldg(p.g.phase_slices + ph_ + 1);
         return r;
@@ -880,7 +880,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 auto stage_next = [&](uint32_t gb_) {   // needs: head of `nxt` landed (cp.async.wait_group 0 + __syncwarp)
                     pend_d = lds_desc(pa.desc(mslot));
                     pend_tile = lds32(pa.desc(mslot) + 16);
-                    issue_slice_gathers(state + (size_t)pend_tile * p.tile_stride + (size_t)half * 16, nxt, pend_d, sr, gb_);
+                    issue_slice_gathers(state() + (size_t)pend_tile * p.tile_stride + (size_t)half * 16, nxt, pend_d, sr, gb_);
                     if (pend_d.G > (uint32_t)kHeadGroups) {   // tail cells: towards L2 now, read when the unit is computed
                         const size_t tail_at = (size_t)pend_d.off + sr;
                         if (half == 0) prefetch_l2(p.g.col4 + tail_at);
@@ -929,10 +929,10 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                         rows_acc = 0;
                         acc_tile = tile;
                     }
-                    PassCtx x = tiles == 1u ? make_ctx(state, state, bestp, s_mask[0], 0ull, 0u, half, rep0, thr, T, p.tie_rule)
-                                            : make_ctx(state, state, bestp, s_mask[tile], p.tile_stride, tile, half, rep0,
+                    PassCtx x = tiles == 1u ? make_ctx(state(), state(), bestp(), s_mask[0], 0ull, 0u, half, rep0(), thr, T, p.tie_rule)
+                                            : make_ctx(state(), state(), bestp(), s_mask[tile], p.tile_stride, tile, half, rep0(),
                                                        thr, T, p.tie_rule);
-                    x.tile += tile0;   // hub accumulators are indexed by the global tile
+                    if (CLUSTER) x.tile += tile0;   // hub accumulators are indexed by the global tile
                     if (first_unit && ts && threadIdx.x == 0) { x.stamp = ts; ts[3] = (unsigned long long)clock64(); }
                     first_unit = false;
                     slice_compute(p.g, x, cur_d, pa.meta(cur_m, 0), sr, acc, p.keys, gb);
@@ -968,7 +968,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 rows_acc = 0;
                 if (lane == 0) s_wtile[warp] = acc_tile;
                 __syncthreads();
-                long long* slot = accum + (size_t)(t % 3u) * nR;
+                long long* slot = accum() + (size_t)(t % 3u) * nR;
                 if (threadIdx.x < kTile) {   // one add per replica and run of warps on the same tile
                     long long run = 0;
                     uint32_t run_tile = s_wtile[0];
@@ -1002,12 +1002,12 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
 
         // sweep end (every CTA redundantly): E, cut = (W - E)/2 (eq. 4), improved mask
         {
-            const long long* slot = accum + (size_t)(t % 3u) * nR;
-            long long* zero_slot = accum + (size_t)((t + 2u) % 3u) * nR;
+            const long long* slot = accum() + (size_t)(t % 3u) * nR;
+            long long* zero_slot = accum() + (size_t)((t + 2u) % 3u) * nR;
             for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {   // nR is a multiple of 32: warp-uniform
                 const long long E = s_E[i] + __ldcg(slot + i);
                 const long long cut = (p.W - E) / 2;
-                const bool live = i < n_rep;
+                const bool live = i < n_rep();
                 const bool improved = live && cut > s_best[i];
                 s_E[i] = E;
                 if (improved) { s_best[i] = cut; s_bsweep[i] = (int)T; }
@@ -1015,7 +1015,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 if (lane == 0) s_mask[i >> 5] = m;
                 if (cta == 0) {
                     zero_slot[i] = 0;
-                    if (live && trace) trace[(size_t)t * p.trace_stride + i] = cut;
+                    if (live && trace()) trace()[(size_t)t * p.trace_stride + i] = cut;
                 }
             }
             __syncthreads();
@@ -1026,8 +1026,8 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     for (uint32_t tile = 0; tile < tiles; ++tile) {
         const uint32_t mask = s_mask[tile];
         if (mask == 0u) continue;
-        const uint4* src = reinterpret_cast<const uint4*>(state + (size_t)tile * p.tile_stride);
-        uint4* best = reinterpret_cast<uint4*>(bestp + (size_t)tile * p.tile_stride);
+        const uint4* src = reinterpret_cast<const uint4*>(state() + (size_t)tile * p.tile_stride);
+        uint4* best = reinterpret_cast<uint4*>(bestp() + (size_t)tile * p.tile_stride);
         const uint32_t m_lo = mask & 0xffffu, m_hi = mask >> 16;
         const unsigned long long units = p.n * 2ull;
         for (unsigned long long uu = (unsigned long long)cta * blockDim.x + threadIdx.x; uu < units;
@@ -1048,9 +1048,9 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     }
     if (cta == 0) {
         for (uint32_t i = threadIdx.x; i < nR; i += blockDim.x) {
-            E_out[i] = s_E[i];
-            best_out[i] = s_best[i];
-            best_sweep_out[i] = s_bsweep[i];
+            E_out()[i] = s_E[i];
+            best_out()[i] = s_best[i];
+            best_sweep_out()[i] = s_bsweep[i];
         }
     }
 }
