@@ -20,18 +20,23 @@ def cfg5():
 
 def test_config5_full_size_all_replicas_first_sweeps(cfg5):
     wl = cfg5
-    M = 6
+    M = 40
     g = gpu_anneal(wl, thr=wl.thr[:M], want_best_spins=False)
-    o = oracle_anneal(wl, thr=wl.thr[:M])
+    o = oracle_anneal(wl, thr=wl.thr[:M], n_threads=16)
     assert_same(g, o, best_spins=False)
     # best state of one replica, full vector
     s, cut, sweep, rep = P.ising_best_state(g["problem"], 17)
     np.testing.assert_array_equal(s.cpu().numpy(), o["best_spins"][17])
+    # the cold end of the schedule (sweeps 460..499, flip probability ~2e-4) from the oracle's state, all replicas
+    g3 = gpu_anneal(wl, thr=wl.thr[460:], sweep_offset=460, init_spins=o["final"], want_best_spins=False,
+                    problem=g["problem"])
+    o3 = oracle_anneal(wl, thr=wl.thr[460:], sweep_offset=460, init_spins=o["final"], n_threads=16)
+    assert_same(g3, o3, best_spins=False)
     # a replica subset straddling the Philox groups, run longer, same problem handle
     for first in (3,):
-        g2 = gpu_anneal(wl, thr=wl.thr[:40], n_replicas=2, first_replica=first, problem=g["problem"],
+        g2 = gpu_anneal(wl, thr=wl.thr[:120], n_replicas=2, first_replica=first, problem=g["problem"],
                         want_best_spins=False)
-        o2 = oracle_anneal(wl, thr=wl.thr[:40], n_replicas=2, first_replica=first)
+        o2 = oracle_anneal(wl, thr=wl.thr[:120], n_replicas=2, first_replica=first)
         assert_same(g2, o2, best_spins=False)
 
 
