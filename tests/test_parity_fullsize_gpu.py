@@ -46,3 +46,17 @@ def test_config5_energy_cut_of_final_state(cfg5):
     trace = P.anneal_workload(p, wl, thr=wl.thr[:3], cut_trace=True)
     E, cut = P.ising_energy_cut(p, None, wl.n_replicas)     # from the definition, current state
     np.testing.assert_array_equal(cut.cpu().numpy(), trace.cpu().numpy()[2])
+
+
+def test_config4_full_size_dense_engine_all_replicas_first_sweeps():
+    """K_4096 x 1024 replicas on the tcgen05 engine in the launch configuration bench.py times (32 x 4 tiles): every
+    replica for the first sweeps, and replicas straddling the 256-replica tile edges for longer (SURVEY 8(c) plan)."""
+    wl = W.config4()
+    g = gpu_anneal(wl, thr=wl.thr[:2], want_best_spins=False)
+    assert g["problem"].has_dense_engine
+    o = oracle_anneal(wl, thr=wl.thr[:2], n_threads=16)
+    assert_same(g, o, best_spins=False)
+    for first in (254, 1020):
+        g2 = gpu_anneal(wl, thr=wl.thr[:12], n_replicas=4, first_replica=first, problem=g["problem"], want_best_spins=False)
+        o2 = oracle_anneal(wl, thr=wl.thr[:12], n_replicas=4, first_replica=first, n_threads=4)
+        assert_same(g2, o2, best_spins=False)
