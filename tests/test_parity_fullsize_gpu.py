@@ -60,3 +60,11 @@ def test_config4_full_size_dense_engine_all_replicas_first_sweeps():
         g2 = gpu_anneal(wl, thr=wl.thr[:12], n_replicas=4, first_replica=first, problem=g["problem"], want_best_spins=False)
         o2 = oracle_anneal(wl, thr=wl.thr[:12], n_replicas=4, first_replica=first, n_threads=4)
         assert_same(g2, o2, best_spins=False)
+
+
+def test_config3_full_schedule_on_a_replica_subset():
+    """100 x 100 torus, the complete 5000-sweep schedule for 16 replicas straddling a tile edge (ids 120..135)."""
+    wl = W.config3()
+    g = gpu_anneal(wl, n_replicas=16, first_replica=120)
+    o = oracle_anneal(wl, n_replicas=16, first_replica=120, n_threads=16)
+    assert_same(g, o)
