@@ -455,7 +455,8 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     auto degree_of = [&](int32_t k) { return (int64_t)dsort[k]; };
     // Edges per sub-row before a row is split over more sub-rows: 16 keeps the instruction count per edge low
     // (throughput-bound colour phases); 8 keeps every row inside the prefetched head cells, i.e. one gather round
-    // trip per phase (latency-bound phases: fewer units than warps on the GPU).  Chosen per colour phase.
+    // trip per phase (latency-bound phases: fewer units than HALF the warps on the GPU; measured on config 5 in ms
+    // per 500 sweeps: threshold 2x the warps 112.9, 1x 110.8, 1/2 109.6, 1/3 109.6, 1/4 109.9).  Chosen per colour phase.
     // A row of more than 16 sub-rows x sub_row_edges edges (a hub) is cut into P balanced PARTS, one slice each,
     // whose partial fields meet in hub_acc (integer atomics); the part that arrives last finishes the row.
     const uint64_t tiles_all = (uint64_t)((max_replicas + kTile - 1) / kTile);
@@ -508,7 +509,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
             const size_t mark = slices.size();
             const uint32_t hub_mark = n_hub_rows;
             const int32_t k_end = emit_colour(c, k, kSubRowEdges);
-            if ((uint64_t)(slices.size() - mark) * tiles_all < (uint64_t)sm_count * kWarpsPerCta) {   // latency-bound phase
+            if ((uint64_t)(slices.size() - mark) * tiles_all * 2ull < (uint64_t)sm_count * kWarpsPerCta) {   // latency-bound phase: less than half a round of the grid's warps
                 slices.resize(mark);
                 slice_aux.resize(2 * mark);
                 n_hub_rows = hub_mark;
