@@ -457,7 +457,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     // (throughput-bound colour phases); 8 keeps every row inside the prefetched head cells, i.e. one gather round
     // trip per phase (latency-bound phases: fewer units than HALF the warps on the GPU; measured on config 5 in ms
     // per 500 sweeps: threshold 2x the warps 112.9, 1x 110.8, 1/2 109.6, 1/3 109.6, 1/4 109.9).  Chosen per colour phase.
-    // A row of more than 16 sub-rows x sub_row_edges edges (a hub) is cut into P balanced PARTS, one slice each,
+    // A row of more than 16 sub-rows x sub_row_edges edges (a hub) is cut into P balanced PARTS of <= 128 edges, one slice each,
     // whose partial fields meet in hub_acc (integer atomics); the part that arrives last finishes the row.
     const uint64_t tiles_all = (uint64_t)((max_replicas + kTile - 1) / kTile);
     auto emit_colour = [&](int32_t c, int32_t k, int sub_row_edges) {   // rows k.. of colour c -> slices; returns the next row
@@ -467,7 +467,11 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
             const int64_t deg = degree_of(k);
             const int64_t groups = (deg + 3) / 4;
             if (groups > part_cells_max) {
-                const int64_t P = (groups + part_cells_max - 1) / part_cells_max;
+                // parts of at most 128 edges in every phase: a part lives in the prefetched head cells alone (measured
+                // on config 5: 256-edge parts in the 16-edge phases 109.6 ms, 128-edge parts 108.9 ms; cutting the rows
+                // of 129-256 edges into two parts as well: 113.4 ms)
+                const int64_t part_size = kSubRows * kHeadGroups;
+                const int64_t P = (groups + part_size - 1) / part_size;
                 const int64_t cpp = (groups + P - 1) / P;
                 if (P > 0x7fff) too_many_parts = true;   // packed arrival count / biased sum of part_finish
                 for (int64_t q = 0; q < P; ++q) {
