@@ -267,9 +267,8 @@ int32_t oracle_anneal(int32_t n, const int64_t* row_ptr, const int32_t* col, con
     return 0;
 }
 
-// Brute force over all 2^n states (n <= 24): maximum cut, and the cut of every state
-// is available through oracle_energy_cut.  Gray-code walk with incremental update from
-// the DEFINITION of the cut change of a single vertex (sum over its row).
+// Brute force over all 2^n states (n <= 24): plain enumeration, the cut of every state from the
+// definition (energy() above); the first state reaching the maximum is returned.
 int32_t oracle_bruteforce_maxcut(int32_t n, const int64_t* row_ptr, const int32_t* col, const void* w,
                                  int32_t wtype, int64_t* max_cut_out, int8_t* argmax_spins_out) {
     if (n > 24 || n < 1) return 1;

@@ -255,6 +255,31 @@ def test_flip_threshold_extremes(oracle):
     assert E1[0] <= E0[0]
 
 
+def test_flip_counter_words_and_domain(oracle):
+    """Q11 / include/ising.h:18: the flip word of spin i, absolute sweep T, replica r is
+    philox4x32_10(ctr=(i, T, r>>2, DOMAIN_FLIP=0), key=seed)[r&3].  Edgeless graph, Jacobi, tie rule MINUS: h = 0,
+    the argmin is -1, so the spin after sweep T is +1 IFF that word < thr.  The expectation comes from the raw,
+    KAT-pinned Philox function (not from the annealer), with sweep, replica group and spin all different and
+    non-zero so that a permuted counter word or another domain constant fails."""
+    n, R, first, off, M = 37, 9, 5, 3, 2
+    seed = 0x1234_5678_9ABC_DEF1
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    row_ptr = np.zeros(n + 1, dtype=np.int64)
+    col = np.zeros(0, dtype=np.int32)
+    w = np.zeros(0, dtype=np.int8)
+    thr = np.array([0x6000_0000, 0x9000_0000], dtype=np.uint32)
+    for mode, order in ((1, None), (0, np.arange(n, dtype=np.int32))):
+        for m in (1, 2):            # the state after sweep off and after sweep off + 1
+            res = oracle.anneal(n, row_ptr, col, w, order=order, mode=mode, thr=thr[:m], n_replicas=R,
+                                first_replica=first, seed=seed, sweep_offset=off)
+            T = off + m - 1
+            for r in range(R):
+                rep = first + r
+                for i in range(n):
+                    word = int(oracle.philox4x32_10([i, T, rep >> 2, 0], key)[rep & 3])
+                    assert (res["final"][r, i] == 1) == (word < int(thr[m - 1])), (mode, m, r, i)
+
+
 @pytest.mark.parametrize("p", [0.5, 0.1, 0.003])
 def test_flip_rate_statistics(oracle, p):
     # edgeless graph: h=0 -> argmin = -1 (MINUS); a spin ends +1 iff its Philox word < thr
@@ -507,6 +532,31 @@ def test_exact_n_subset_is_uniform_over_the_spins(oracle):
     sigma = np.sqrt(draws * (N / n) * (1 - N / n))
     assert np.all(np.abs(counts - expect) < 5 * sigma)
     assert len(pair_seen) > 0.99 * draws          # different replicas / sweeps draw different subsets
+
+
+def test_exact_n_draw_counter_words_and_domain(oracle):
+    """Reading Q5 (Algorithm 1, L92): draw k of sweep T, replica r uses philox4x32_10(ctr=(k, T, r>>2,
+    DOMAIN_FLIPN=2), key=seed)[r&3] and x = floor(u (j+1) / 2^32), j = n - N + k (Floyd).  Empty graph, MINUS: the
+    minimisation sweep writes -1 everywhere, so the +1 spins are exactly the subset -- recomputed here from the raw,
+    KAT-pinned Philox function with non-zero sweep / replica group."""
+    n, N, R, first, off = 23, 5, 6, 6, 4
+    seed = 0xFEDC_BA98_7654_3211
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    row_ptr = np.zeros(n + 1, dtype=np.int64)
+    o = oracle.anneal(n, row_ptr, np.zeros(0, np.int32), np.zeros(0, np.int8), order=np.arange(n, dtype=np.int32),
+                      mode=2, n_replicas=R, first_replica=first, seed=seed, thr=np.array([N], dtype=np.uint32),
+                      sweep_offset=off)
+    for r in range(R):
+        rep = first + r
+        chosen = []
+        for k in range(N):
+            j = n - N + k
+            u = int(oracle.philox4x32_10([k, off, rep >> 2, 2], key)[rep & 3])
+            x = (u * (j + 1)) >> 32
+            chosen.append(j if x in chosen else x)
+        expect = -np.ones(n, dtype=np.int8)
+        expect[chosen] = 1
+        np.testing.assert_array_equal(o["final"][r], expect)
 
 
 def test_exact_n_best_tracking_and_trace(oracle):
