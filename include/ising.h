@@ -86,7 +86,11 @@ enum { ISING_W_INT8 = 1, ISING_W_INT32 = 4 };
 /* load flags */
 enum {
     ISING_LOAD_DEFAULT = 0,
-    ISING_LOAD_NO_DENSE = 1   /* never build the dense tcgen05 engine, even for a complete graph */
+    ISING_LOAD_NO_DENSE = 1,      /* never build the dense tcgen05 engine, even for a complete graph */
+    /* Gauss-Seidel engine selection (results never depend on it; the default picks the fastest that applies):       */
+    ISING_LOAD_NO_SMALL = 2,      /* do not run a small graph wholly inside one CTA per four replicas (shared memory)   */
+    ISING_LOAD_NO_CLUSTER = 4,    /* do not run a small graph on one thread-block cluster per replica tile              */
+    ISING_LOAD_NO_TAIL_CHAIN = 8  /* big graph: every colour class is a grid-wide phase (no shared-memory tail chain)    */
 };
 
 /*
@@ -116,7 +120,8 @@ ising_status ising_workspace_bytes(int32_t n, int64_t nnz, int32_t wtype, int32_
  *
  * A complete graph (nnz == n(n-1)) with int8-range weights additionally gets the dense
  * engine (J as an int8 matrix, local fields J.S on tcgen05 tensor cores), used by
- * ISING_MODE_JACOBI.  Synchronous.  Errors: every ISING_ERR_* above.
+ * ISING_MODE_JACOBI.  Limits: a row may hold at most 32767 x 128 edges (ISING_ERR_BAD_SHAPE beyond).
+ * Synchronous.  Errors: every ISING_ERR_* above.
  */
 ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
                             const void* weights, int32_t wtype, const int32_t* colour,
@@ -147,11 +152,8 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
  *
  * After every sweep the cut of every replica is evaluated (eq. 4) and the best state seen
  * in THIS call is captured (strictly greater cut wins, so the earliest sweep wins ties).
- * Asynchronous on `stream`.  n_sweeps == 0 only (re)initialises the state.
- * Tuning knob (results never depend on it): environment variable ISING_TICKET_MODE = 1 / 2 makes the
- * persistent Gauss-Seidel kernel hand out its work units by a CTA-local / grid-wide ticket counter
- * instead of the default strided assignment (0); ISING_CLUSTER = 0 runs small graphs on the cooperative grid
- * instead of one thread-block cluster per replica tile.
+ * Asynchronous on `stream` (except ISING_INIT_GIVEN, which reads back a validity flag of the given spins).
+ * `thresholds` is copied before the call returns.  n_sweeps == 0 only (re)initialises the state.
  */
 ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int32_t n_replicas,
                           int32_t first_replica, uint64_t seed, const uint32_t* thresholds,
@@ -196,21 +198,12 @@ ising_status ising_current_state(ising_problem* p, int8_t* spins_out, int32_t n_
  *   what: 0 n, 1 nnz, 2 n_colours, 3 max_replicas, 4 W = sum_{i<j} w_ij, 5 dense engine built (0/1),
  *         6 kernels launched by this handle so far, 7 max_i sum_j |w_ij|, 8 workspace bytes in use,
  *         9 slices of the sparse layout, 10 padded edge slots of the sparse layout, 11 hub rows,
- *         12 CTAs of the persistent grid
+ *         12 CTAs of the persistent grid, 13 Gauss-Seidel engine (0 launch per phase, 1 persistent grid, 2 persistent
+ *         clusters, 3 persistent grid + shared-memory tail chain, 4 shared-memory chain for the whole graph),
+ *         14 rows of the shared-memory chain, 15 virtual phases of the persistent kernel,
+ *         16 chunks of the chain, 17 1 if the chain is resident in shared memory
  */
 ising_status ising_problem_info(const ising_problem* p, int32_t what, int64_t* value_out);
-
-/*
- * Diagnostics of the persistent Gauss-Seidel kernel: the next ising_anneal calls record, for sweep
- * `sweep` of the call, the SM clock of every CTA when it arrives at and when it leaves the grid
- * barrier that ends each colour phase.
- *   stamps   uint64 [n_colours][n_cta][8] (0 arrive, 1 leave, 2-6 stages of the first unit of warp 0: pipeline
- *            start, gathers landed, fields done, hub part arrived, row finished; 7 unused), DEVICE;
- *            n_cta = ising_problem_info(12);
- *            NULL switches the recording off
- * Stamps of different CTAs come from different SM clocks: compare differences within one CTA.
- */
-ising_status ising_debug_phase_timing(ising_problem* p, uint64_t* stamps, int32_t sweep);
 
 /* Release the handle (the workspace returns to the caller).  NULL is allowed. */
 ising_status ising_free(ising_problem* p);

@@ -1,0 +1,27 @@
+/*
+ * ising_debug.h -- diagnostics of the B200-native Ising annealer.  NOT part of the product boundary (include/ising.h):
+ * nothing here changes a result; it only records where the persistent Gauss-Seidel kernel spends its time.
+ */
+#ifndef ISING_B200_DEBUG_H
+#define ISING_B200_DEBUG_H
+
+#include "ising.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/*
+ * The next ising_anneal calls (persistent cooperative-grid Gauss-Seidel kernel only) record, for sweep `sweep` of the
+ * call, the SM clock of every CTA when it arrives at and when it leaves the grid barrier that ends each virtual phase
+ * (the colour phases; with a tail chain: the phases before the tail, the bulk pseudo-phase, then the chain).
+ *   stamps   uint64 [ising_problem_info(15) + 1][ising_problem_info(12)][8], DEVICE: word 0 arrival, word 1 departure,
+ *            words 2-7 unused; NULL switches the recording off
+ * Stamps of different CTAs come from different SM clocks: compare differences within one CTA.
+ */
+ising_status ising_debug_phase_timing(ising_problem* p, uint64_t* stamps, int32_t sweep);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ISING_B200_DEBUG_H */

@@ -21,6 +21,9 @@ ISING_TIE_MINUS, ISING_TIE_KEEP = 0, 1
 ISING_INIT_PHILOX, ISING_INIT_GIVEN, ISING_INIT_CONTINUE = 0, 1, 2
 ISING_W_INT8, ISING_W_INT32 = 1, 4
 ISING_LOAD_DEFAULT, ISING_LOAD_NO_DENSE = 0, 1
+ISING_LOAD_NO_SMALL, ISING_LOAD_NO_CLUSTER, ISING_LOAD_NO_TAIL_CHAIN = 2, 4, 8
+# ising_problem_info(13): the Gauss-Seidel engine of a loaded problem
+ENGINE_PER_PHASE, ENGINE_GRID, ENGINE_CLUSTER, ENGINE_GRID_TAIL_CHAIN, ENGINE_SMALL = 0, 1, 2, 3, 4
 
 STATUS_NAMES = {
     0: "ISING_OK", 1: "ISING_ERR_NULL_ARG", 2: "ISING_ERR_BAD_SHAPE", 3: "ISING_ERR_UNSORTED_OR_DUP",
@@ -150,12 +153,16 @@ class Problem:
     def launches(self) -> int:
         return self.info(6)
 
+    @property
+    def engine(self) -> int:
+        """ENGINE_* : which Gauss-Seidel kernel ising_anneal will use for this problem."""
+        return self.info(13)
+
     def phase_timing(self, sweep: int = 0):
-        """Diagnostics: record SM clocks of sweep `sweep` of the next GS anneal (per colour phase and CTA:
-        0/1 barrier arrive / leave, 2-6 stages of the first unit of warp 0).
-        Returns the int64 device tensor [n_colours][n_cta][8] the kernel will fill."""
+        """Diagnostics (include/ising_debug.h): record SM clocks of sweep `sweep` of the next GS anneal (per virtual
+        phase and CTA: 0/1 barrier arrive / leave).  Returns the int64 device tensor [virtual phases + 1][n_cta][8]."""
         t = _torch()
-        buf = t.zeros((max(1, self.n_colours), self.info(12), 8), dtype=t.int64, device="cuda")
+        buf = t.zeros((self.info(15) + 1, self.info(12), 8), dtype=t.int64, device="cuda")
         _check(lib().ising_debug_phase_timing(self.handle, buf.data_ptr(), sweep), "ising_debug_phase_timing")
         self._keep.append(buf)
         return buf

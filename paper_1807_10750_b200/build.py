@@ -19,7 +19,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
 
 def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh"))
-                  + [os.path.join(os.path.dirname(_HERE), "include", "ising.h")])
+                  + glob.glob(os.path.join(os.path.dirname(_HERE), "include", "*.h")))
 
 
 def is_stale() -> bool:
@@ -40,7 +40,8 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     nvcc = nvcc_path()
     if nvcc is None:
         raise RuntimeError("nvcc not found: cannot build libising_b200.so (there is no CPU fallback)")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    tuning = ["-DISING_TUNING_ENV"] if os.environ.get("ISING_BUILD_TUNING") == "1" else []   # env knobs: tuning builds only
+    cmd = [nvcc] + NVCC_FLAGS + tuning + (["-Xptxas", "-v"] if verbose else []) + \
           ["-o", LIB + ".tmp", os.path.join(CSRC, "ising_api.cu")]
     subprocess.check_call(cmd)
     os.replace(LIB + ".tmp", LIB)

@@ -1,0 +1,483 @@
+// Shared-memory chain engine: colour-class Gauss-Seidel levels executed by ONE CTA per group of four replicas, with a
+// __syncthreads between colour classes instead of a grid / cluster barrier.
+//
+// Replicas never interact ("a number of GPU simulations"), so a CTA that owns ALL rows of a
+// set of colour classes for four replicas (one 32-bit word of spin bytes per row) needs no other CTA to walk through
+// these classes in order.  Two uses:
+//   FULL  (k_anneal_small): the whole graph is the chain.  val[row] = the four spin bytes, cells hold every edge; all
+//         sweeps x colour classes of an ising_anneal call run without any global synchronisation and, when the packed
+//         graph fits shared memory ("resident"), without global traffic inside a sweep except trace / best capture.
+//         This is the small-graph regime of the paper's own benchmarks (800 .. 20 000 vertices, Table III).
+//   DELTA (tail of k_anneal_gs): the chain rows are the last colour classes of a big graph (few rows, hub-like, a
+//         dependent level per class).  Their local fields are first computed by the whole grid from the values all
+//         spins hold BEFORE the chain ("bulk" pseudo-phase, h0); the chain then only adds, per row, the corrections
+//         w * (new - old) of its LOWER-coloured chain neighbours, which it keeps in shared memory: val[row] = new - old
+//         per replica byte (0 / +2 / -2), written when the row is updated and read only by later levels.
+// Layout: a chain row's cells hold 4 edges each: four 16-bit LOCAL neighbour ids (uint2) + four int8 weights (one
+// word), padded with weight 0.  Rows are cut into CHUNKS (row ranges, 8-row aligned, first cell 4-aligned) that fit
+// one shared-memory buffer; a chunk is fetched with 16-byte cp.async by all threads and holds, block after block:
+// 16-bit cell pointers relative to the chunk, [DELTA: h0 (int4 per row) and the rows' current spin words], neighbour
+// ids, weights.  SEGMENTS = runs of rows of one level inside one chunk; L lanes share a row (its cells strided over
+// the lanes, fields summed by a butterfly).  The flip decisions (state-independent) are drawn ahead of the levels, one
+// Philox call per row and thread, into a byte per row of shared memory.
+#pragma once
+#include "common.cuh"
+#include "primitives.cuh"
+
+namespace ising {
+
+constexpr int kChainGroups = 8;                 // chain CTAs per replica tile: four replicas (one spin word) each
+constexpr uint32_t kChainMaxLocal = 65535;      // local row ids are 16 bit
+constexpr int kChainMaxChunks = 96;
+constexpr int kChainMaxSegs = 192;
+constexpr int kSmallThreadsMax = 1024;
+
+struct ChainSeg {
+    uint32_t r0, r1;   // local rows [r0, r1) of one level, inside one chunk
+    uint32_t info;     // bits 0-7: log2(lanes per row); bit 8: the level ends with this segment (CTA barrier follows)
+    uint32_t pad;
+};
+struct ChainChunk {
+    uint32_t r0, r1;   // local rows [r0, r1); r0 is a multiple of 8
+    uint32_t c0, c1;   // cells [c0, c1); both multiples of 4
+    uint32_t ptr_at;   // first entry of this chunk in rel16 (multiple of 8): r1 - r0 + 1 pointers relative to c0
+    uint32_t seg0, seg1;
+    uint32_t pad;
+};
+
+struct ChainView {
+    const ChainChunk* chunks;
+    const ChainSeg* segs;
+    const uint16_t* rel16;
+    const uint32_t* orig;    // [n_t_pad] caller id of local row r (Philox counter word 0)
+    const uint2* cidx;       // [cells] four 16-bit local neighbour ids
+    const uint32_t* cw;      // [cells] four int8 weights
+    int* h0;                 // DELTA: [tiles][8][n_t_pad][4] local fields from the pre-chain values (zero between sweeps)
+    uint32_t* old;           // DELTA: [tiles][8][n_t_pad] compact copy of the chain rows' spin words
+    uint32_t n_chunks, n_segs;
+    uint32_t n_t, n_t_pad;   // chain rows, padded to a multiple of 8
+    uint32_t row_lo;         // internal row of local row 0
+    uint32_t resident;       // FULL: one chunk that stays in shared memory for the whole call
+    uint32_t buf_bytes;      // capacity of one chunk buffer
+    uint32_t threads;        // CTA size the segments' lanes-per-row were planned for
+    uint32_t narrow;         // a sweep's energy increments of all chain rows fit int32
+};
+
+struct ChunkLayout { uint32_t ptr, h0, old, idx, w, bytes; };
+__host__ __device__ inline uint32_t chain_align16(uint32_t x) { return (x + 15u) & ~15u; }
+__host__ __device__ inline ChunkLayout chunk_layout(uint32_t R, uint32_t Nc, bool delta) {
+    ChunkLayout l;
+    uint32_t at = 0;
+    l.ptr = at;  at += chain_align16(2u * (R + 1u));
+    l.h0 = at;   if (delta) at += 16u * R;
+    l.old = at;  if (delta) at += chain_align16(4u * R);
+    l.idx = at;  at += 8u * Nc;
+    l.w = at;    at += 4u * Nc;
+    l.bytes = at;
+    return l;
+}
+
+__device__ __forceinline__ uint2 lds64(uint32_t smem_addr) {
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(smem_addr));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds16(uint32_t smem_addr) {
+    uint32_t v;
+    asm volatile("{ .reg .u16 t; ld.shared.u16 t, [%1]; cvt.u32.u16 %0, t; }" : "=r"(v) : "r"(smem_addr));
+    return v;
+}
+
+// All threads of the CTA: request chunk `ck` into the buffer at shared address `buf` (one commit group).
+template <bool DELTA>
+__device__ __forceinline__ void chain_issue_chunk(const ChainView& v, const ChainChunk& ck, uint32_t buf, uint32_t slot,
+                                                  uint32_t tid, uint32_t nthr) {
+    const uint32_t R = ck.r1 - ck.r0, Nc = ck.c1 - ck.c0;
+    const ChunkLayout l = chunk_layout(R, Nc, DELTA);
+    const size_t srow = (size_t)slot * v.n_t_pad + ck.r0;
+    for (uint32_t off = tid << 4; off < l.bytes; off += nthr << 4) {
+        const char* src;
+        if (off >= l.w) src = reinterpret_cast<const char*>(v.cw + ck.c0) + (off - l.w);
+        else if (off >= l.idx) src = reinterpret_cast<const char*>(v.cidx + ck.c0) + (off - l.idx);
+        else if (DELTA && off >= l.old) src = reinterpret_cast<const char*>(v.old + srow) + (off - l.old);
+        else if (DELTA && off >= l.h0) src = reinterpret_cast<const char*>(v.h0 + srow * 4) + (off - l.h0);
+        else src = reinterpret_cast<const char*>(v.rel16 + ck.ptr_at) + off;
+        cp_async16(buf + off, src);
+    }
+    cp_async_commit();
+}
+
+struct ChainRt {             // per sweep
+    uint32_t thr, T;
+    uint32_t rl0;            // global id of replica 0 of this CTA's word
+    int32_t tie_rule;
+};
+
+// Flip bits (Alg. 2, reading Q11) of the four replicas rl0 .. rl0+3 of spin `orig` in sweep T.
+__device__ __forceinline__ uint32_t chain_flip4(uint32_t orig, const ChainRt& rt, const PhiloxKeys& keys) {
+    const uint32_t cw = rt.rl0 >> 2, sh = rt.rl0 & 3u;
+    uint32_t m = lt4(philox4x32_10(orig, rt.T, cw, kDomainFlip, keys), rt.thr);
+    if (sh) m = ((m | (lt4(philox4x32_10(orig, rt.T, cw + 1u, kDomainFlip, keys), rt.thr) << 4)) >> sh) & 15u;
+    return m;
+}
+
+// Flip nibbles of local rows [r0, r1) into flip[] (one byte per row), one row per thread.
+__device__ __forceinline__ void chain_draw_flips(const ChainView& v, uint32_t flip, uint32_t r0, uint32_t r1,
+                                                 const ChainRt& rt, const PhiloxKeys& keys, uint32_t tid, uint32_t nthr) {
+    if (rt.thr == 0u) return;
+    for (uint32_t r = r0 + tid; r < r1; r += 4u * nthr) {   // four rows at a time: the loads and the Philox chains interleave
+        uint32_t o[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) o[j] = r + j * nthr < r1 ? __ldg(v.orig + r + j * nthr) : 0u;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (r + j * nthr < r1) {
+                const uint32_t f = chain_flip4(o[j], rt, keys);
+                asm volatile("st.shared.u8 [%0], %1;" ::"r"(flip + r + j * nthr), "r"(f) : "memory");
+            }
+        }
+    }
+}
+__device__ __forceinline__ uint32_t lds8(uint32_t smem_addr) {
+    uint32_t v;
+    asm volatile("{ .reg .u16 t; ld.shared.u8 t, [%1]; cvt.u32.u16 %0, t; }" : "=r"(v) : "r"(smem_addr));
+    return v;
+}
+
+// DELTA-only global targets of a chain CTA (its word of every chain row).
+struct ChainGlobal {
+    uint8_t* state;      // &state[tile][row_lo][4 g]   (row stride kTile)
+    uint8_t* best;       // same position in the captured best state
+    uint32_t* old;       // compact copy [n_t_pad] of this CTA
+    uint32_t cap4;       // capture mask of this CTA's four replicas (improved in the previous sweep)
+};
+
+// One segment: every row takes its energy-minimising value (L47-49, Q1/Q3), the scheduled flip (L177), and its
+// energy increment dE = (a - s) h is added to dE[] (a7; exact because a colour class is an independent set).
+template <bool DELTA>
+__device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChunk& ck, uint32_t buf, uint32_t val,
+                                              uint32_t flip, const ChainRt& rt, const PhiloxKeys& keys, long long (&dE)[4],
+                                              const ChainGlobal& cg, uint32_t tid, uint32_t nthr) {
+    const uint32_t logL = sg.info & 0xffu, L = 1u << logL, q = tid & (L - 1u);
+    const uint32_t rpi = nthr >> logL;
+    const ChunkLayout l = chunk_layout(ck.r1 - ck.r0, ck.c1 - ck.c0, DELTA);
+    uint32_t r = sg.r0 + (tid >> logL);
+    for (uint32_t rw = sg.r0 + ((tid & ~31u) >> logL); rw < sg.r1; rw += rpi, r += rpi) {   // warp-uniform trip count
+        const bool act = r < sg.r1;
+        const uint32_t lr = act ? r - ck.r0 : 0u;
+        uint32_t p0 = 0, p1 = 0, f4 = 0;
+        if (act) {
+            p0 = lds16(buf + l.ptr + 2u * lr);
+            p1 = lds16(buf + l.ptr + 2u * lr + 2u);
+            if (q == 0 && rt.thr != 0u) f4 = lds8(flip + r);
+        }
+        int h0 = 0, h1 = 0, h2 = 0, h3 = 0;
+        for (uint32_t k = p0 + q; k < p1; k += L) {
+            const uint2 ix = lds64(buf + l.idx + 8u * k);
+            const uint32_t w = lds32(buf + l.w + 4u * k);
+            const uint32_t e0 = lds32(val + 4u * (ix.x & 0xffffu)), e1 = lds32(val + 4u * (ix.x >> 16));
+            const uint32_t e2 = lds32(val + 4u * (ix.y & 0xffffu)), e3 = lds32(val + 4u * (ix.y >> 16));
+            uint32_t t0, t1, t2, t3;
+            transpose4x4(e0, e1, e2, e3, t0, t1, t2, t3);
+            h0 = __dp4a((int)t0, (int)w, h0);
+            h1 = __dp4a((int)t1, (int)w, h1);
+            h2 = __dp4a((int)t2, (int)w, h2);
+            h3 = __dp4a((int)t3, (int)w, h3);
+        }
+        for (uint32_t o = 1; o < L; o <<= 1) {
+            h0 += __shfl_xor_sync(0xffffffffu, h0, o);
+            h1 += __shfl_xor_sync(0xffffffffu, h1, o);
+            h2 += __shfl_xor_sync(0xffffffffu, h2, o);
+            h3 += __shfl_xor_sync(0xffffffffu, h3, o);
+        }
+        if (act && q == 0) {
+            uint32_t oldw;
+            if (DELTA) {
+                oldw = lds32(buf + l.old + 4u * lr);
+                const uint4 hh = lds128(buf + l.h0 + 16u * lr);
+                h0 += (int)hh.x; h1 += (int)hh.y; h2 += (int)hh.z; h3 += (int)hh.w;
+            } else {
+                oldw = lds32(val + 4u * r);
+            }
+            uint32_t a = ~sign_bytes(h0, h1, h2, h3) | 0x01010101u;   // +1 where h < 0, else -1
+            if (rt.tie_rule == 1) {                                   // KEEP: h == 0 leaves the spin
+                const uint32_t z = (h0 == 0 ? 0xffu : 0u) | (h1 == 0 ? 0xff00u : 0u) | (h2 == 0 ? 0xff0000u : 0u) |
+                                   (h3 == 0 ? 0xff000000u : 0u);
+                a = (a & ~z) | (oldw & z);
+            }
+            a ^= ((f4 * 0x00204081u) & 0x01010101u) * 0xfeu;
+            const uint32_t d2 = (a << 1) & (a ^ oldw);                // a - s per byte: 0, +2, -2
+            if (d2 != 0u) {
+                dE[0] += (long long)(sbyte(d2, 0) * h0);
+                dE[1] += (long long)(sbyte(d2, 1) * h1);
+                dE[2] += (long long)(sbyte(d2, 2) * h2);
+                dE[3] += (long long)(sbyte(d2, 3) * h3);
+            }
+            if (DELTA) {
+                sts32(val + 4u * r, d2);
+                const size_t at = (size_t)r * kTile;
+                if (d2 != 0u) {
+                    *reinterpret_cast<uint32_t*>(cg.state + at) = a;
+                    cg.old[r] = a;
+                }
+                if (cg.cap4 != 0u) {   // fused best-state capture: the value the row held after the previous sweep
+                    uint32_t* bp = reinterpret_cast<uint32_t*>(cg.best + at);
+                    if (cg.cap4 == 15u) {
+                        *bp = oldw;
+                    } else {
+                        const uint32_t km = nibble_to_bytemask(cg.cap4);
+                        *bp = (oldw & km) | (__ldcg(bp) & ~km);
+                    }
+                }
+            } else {
+                sts32(val + 4u * r, a);
+            }
+        }
+    }
+}
+
+// One pass over all chain levels (one sweep of the chain rows), chunks streamed through two buffers.
+// s_chunks / s_segs: the tables in shared memory.  DELTA: h0 of a chunk is cleared once it has landed.
+template <bool DELTA>
+__device__ __forceinline__ void chain_pass_streamed(const ChainView& v, const ChainChunk* s_chunks, const ChainSeg* s_segs,
+                                                    uint32_t val, uint32_t flip, uint32_t buf0, uint32_t slot, const ChainRt& rt,
+                                                    const PhiloxKeys& keys, long long (&dE)[4], const ChainGlobal& cg,
+                                                    uint32_t tid, uint32_t nthr, bool first_issued,
+                                                    unsigned long long* dbg = nullptr, uint32_t dbg_stride = 0) {
+    const uint32_t bb = v.buf_bytes;
+    uint32_t dj = 0;
+    auto stamp = [&]() {   // diagnostics: slots 2..7 of consecutive rows of the phase-timing buffer
+        if (dbg) { dbg[(size_t)(dj / 6u) * dbg_stride + 2u + dj % 6u] = (unsigned long long)clock64(); ++dj; }
+    };
+    stamp();
+    if (!first_issued) chain_issue_chunk<DELTA>(v, s_chunks[0], buf0, slot, tid, nthr);
+    chain_draw_flips(v, flip, s_chunks[0].r0, s_chunks[0].r1, rt, keys, tid, nthr);
+    for (uint32_t k = 0; k < v.n_chunks; ++k) {
+        const ChainChunk ck = s_chunks[k];
+        const uint32_t buf = buf0 + (k & 1u) * bb;
+        if (k + 1u < v.n_chunks) {   // next chunk: request it, draw its rows' flips while it is on its way
+            chain_issue_chunk<DELTA>(v, s_chunks[k + 1u], buf0 + ((k + 1u) & 1u) * bb, slot, tid, nthr);
+            chain_draw_flips(v, flip, s_chunks[k + 1u].r0, s_chunks[k + 1u].r1, rt, keys, tid, nthr);
+            cp_async_wait<1>();
+        } else {
+            cp_async_wait<0>();
+        }
+        __syncthreads();
+        stamp();
+        if (DELTA) {
+            int4* hz = reinterpret_cast<int4*>(v.h0) + (size_t)slot * v.n_t_pad + ck.r0;
+            for (uint32_t i = tid; i < ck.r1 - ck.r0; i += nthr) __stcg(hz + i, make_int4(0, 0, 0, 0));
+        }
+        bool synced = false;
+        for (uint32_t s = ck.seg0; s < ck.seg1; ++s) {
+            const ChainSeg sg = s_segs[s];
+            chain_segment<DELTA>(sg, ck, buf, val, flip, rt, keys, dE, cg, tid, nthr);
+            synced = (sg.info & 0x100u) != 0u;
+            if (synced) __syncthreads();
+            stamp();
+        }
+        if (!synced) __syncthreads();   // the buffer is free for the chunk after next
+    }
+}
+
+// Sum of the threads' dE[] into s_dE[4] (shared; zero before).  narrow: every partial sum of a sweep fits int32
+// (chain rows x 2 max_i sum_j |w_ij| < 2^31, checked at load): one REDUX per value and one atomic per warp.
+__device__ __forceinline__ void chain_reduce_dE(long long (&dE)[4], long long* s_dE, uint32_t tid, bool narrow) {
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        long long x = dE[b];
+        if (narrow) {
+            x = (long long)__reduce_add_sync(0xffffffffu, (int)x);
+        } else {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        }
+        if ((tid & 31u) == 0u && x != 0)
+            atomicAdd(reinterpret_cast<unsigned long long*>(s_dE + b), (unsigned long long)x);
+        dE[b] = 0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_anneal_small: a whole ising_anneal call (Gauss-Seidel, int8 weights) for a graph whose chain fits one CTA.
+// Grid = tiles x 8 CTAs, one per word of four replicas; CTAs never synchronise with one another.
+// ---------------------------------------------------------------------------------------------
+struct SmallParams {
+    ChainView v;
+    uint8_t* state;                 // [tiles][n][32], standard layout: read at start, written at the end
+    uint8_t* best;                  // captured best state, standard layout (written at the end)
+    uint32_t* best_compact;         // scratch [tiles * 8][bc_stride]: this CTA's words of its best state
+    uint32_t bc_stride;
+    unsigned long long tile_stride;
+    uint32_t n_replicas, rep0;
+    int32_t tie_rule;
+    uint32_t n_sweeps, sweep_offset;
+    const uint32_t* thr;            // DEVICE [n_sweeps]
+    long long W;
+    const long long* E0;            // [tiles * 32]
+    long long* trace;               // [n_sweeps][trace_stride] or nullptr
+    unsigned long long trace_stride;
+    long long* E_out;
+    long long* best_out;
+    int32_t* best_sweep_out;
+    int32_t resume;
+    unsigned long long* timing;     // diagnostics (resident chain only): SM-clock stamps of CTA 0 in sweep timing_sweep: sweep start,
+                                    // flips drawn, after every segment, dE reduced, cut / best done, capture done; or nullptr
+    uint32_t timing_sweep;
+    PhiloxKeys keys;
+};
+
+__global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const SmallParams p) {
+    extern __shared__ __align__(128) uint8_t chain_smem[];
+    __shared__ ChainChunk s_chunks[kChainMaxChunks];
+    __shared__ ChainSeg s_segs[kChainMaxSegs];
+    __shared__ long long s_dE[4], s_E[4], s_bc[4];
+    __shared__ int s_bs[4];
+    __shared__ uint32_t s_imp;
+    const uint32_t tid = threadIdx.x, nthr = blockDim.x;
+    const uint32_t tile = blockIdx.x / kChainGroups, g = blockIdx.x % kChainGroups, slot = blockIdx.x;
+    const uint32_t r_first = tile * kTile + 4u * g;      // first replica of this CTA within the call
+    if (r_first >= p.n_replicas) return;                 // no live replica in this word
+    const ChainView& v = p.v;
+    const uint32_t n = v.n_t;
+    const uint32_t val = (uint32_t)__cvta_generic_to_shared(chain_smem);
+    const uint32_t flip = val + chain_align16(4u * v.n_t_pad);
+    const uint32_t buf0 = flip + chain_align16(v.n_t_pad);
+    uint8_t* const gstate = p.state + (size_t)tile * p.tile_stride + 4u * g;
+    uint8_t* const gbest = p.best + (size_t)tile * p.tile_stride + 4u * g;
+    uint32_t* const bcomp = p.best_compact + (size_t)slot * p.bc_stride;
+
+    for (uint32_t i = tid; i < v.n_chunks * (uint32_t)(sizeof(ChainChunk) / 4); i += nthr)
+        reinterpret_cast<uint32_t*>(s_chunks)[i] = __ldg(reinterpret_cast<const uint32_t*>(v.chunks) + i);
+    for (uint32_t i = tid; i < v.n_segs * (uint32_t)(sizeof(ChainSeg) / 4); i += nthr)
+        reinterpret_cast<uint32_t*>(s_segs)[i] = __ldg(reinterpret_cast<const uint32_t*>(v.segs) + i);
+    for (uint32_t r = tid; r < n; r += nthr) {
+        sts32(val + 4u * r, __ldcg(reinterpret_cast<const uint32_t*>(gstate + (size_t)r * kTile)));
+        if (p.resume) bcomp[r] = __ldcg(reinterpret_cast<const uint32_t*>(gbest + (size_t)r * kTile));
+    }
+    if (tid < 4u) {
+        s_dE[tid] = 0;
+        s_E[tid] = p.E0[r_first + tid];
+        s_bc[tid] = p.resume ? p.best_out[r_first + tid] : (long long)0x8000000000000000ull;
+        s_bs[tid] = p.resume ? p.best_sweep_out[r_first + tid] : 0;
+    }
+    __syncthreads();
+    if (v.resident) {
+        chain_issue_chunk<false>(v, s_chunks[0], buf0, slot, tid, nthr);
+        cp_async_wait<0>();
+        __syncthreads();
+    }
+    ChainGlobal cg{};
+    ChainRt rt;
+    rt.rl0 = p.rep0 + r_first;
+    rt.tie_rule = p.tie_rule;
+    long long dE[4] = {0, 0, 0, 0};
+    for (uint32_t t = 0; t < p.n_sweeps; ++t) {
+        rt.thr = __ldg(p.thr + t);
+        rt.T = p.sweep_offset + t;
+        unsigned long long* ts = (p.timing && t == p.timing_sweep && blockIdx.x == 0 && tid == 0) ? p.timing : nullptr;
+        if (ts) *ts++ = (unsigned long long)clock64();
+        if (v.resident) {
+            chain_draw_flips(v, flip, 0u, n, rt, p.keys, tid, nthr);
+            __syncthreads();
+            if (ts) *ts++ = (unsigned long long)clock64();
+            const ChainChunk ck = s_chunks[0];
+            for (uint32_t s = 0; s < v.n_segs; ++s) {
+                const ChainSeg sg = s_segs[s];
+                chain_segment<false>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
+                if (sg.info & 0x100u) __syncthreads();
+                if (ts) *ts++ = (unsigned long long)clock64();
+            }
+        } else {
+            chain_pass_streamed<false>(v, s_chunks, s_segs, val, flip, buf0, slot, rt, p.keys, dE, cg, tid, nthr, false);
+        }
+        chain_reduce_dE(dE, s_dE, tid, v.narrow != 0u);
+        __syncthreads();
+        if (ts) *ts++ = (unsigned long long)clock64();
+        if (tid < 4u) {   // a7: E, cut = (W - E)/2 (eq. 4), best tracking (strictly greater: the earliest sweep wins)
+            const long long E = s_E[tid] + s_dE[tid];
+            const long long cut = (p.W - E) / 2;
+            const bool live = r_first + tid < p.n_replicas;
+            const bool improved = live && cut > s_bc[tid];
+            s_E[tid] = E;
+            s_dE[tid] = 0;
+            if (improved) { s_bc[tid] = cut; s_bs[tid] = (int)rt.T; }
+            if (live && p.trace) p.trace[(size_t)t * p.trace_stride + r_first + tid] = cut;
+            const uint32_t m = __ballot_sync(0xfu, improved);
+            if (tid == 0) s_imp = m;
+        }
+        __syncthreads();
+        if (ts) *ts++ = (unsigned long long)clock64();
+        const uint32_t imp = s_imp;
+        if (imp != 0u) {   // capture the improved replicas' bytes of every row
+            const uint32_t km = nibble_to_bytemask(imp);
+            for (uint32_t r = tid; r < n; r += nthr) {
+                const uint32_t s = lds32(val + 4u * r);
+                bcomp[r] = imp == 15u ? s : ((s & km) | (bcomp[r] & ~km));
+            }
+            __syncthreads();   // the next sweep rewrites val
+        }
+        if (ts) *ts++ = (unsigned long long)clock64();
+    }
+    // final state and best state back to the standard layout
+    for (uint32_t r = tid; r < n; r += nthr) {
+        *reinterpret_cast<uint32_t*>(gstate + (size_t)r * kTile) = lds32(val + 4u * r);
+        *reinterpret_cast<uint32_t*>(gbest + (size_t)r * kTile) = bcomp[r];
+    }
+    if (tid < 4u) {
+        p.E_out[r_first + tid] = s_E[tid];
+        p.best_out[r_first + tid] = s_bc[tid];
+        p.best_sweep_out[r_first + tid] = s_bs[tid];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Chain builder (a1): one warp per chain row scans the row of the caller's CSR and keeps the qualifying neighbours
+// (FULL: all; DELTA: chain rows of a lower colour).  Pass 1 counts cells, pass 2 (after the host has cut the rows into
+// chunks and fixed the cell pointers) fills them.
+// ---------------------------------------------------------------------------------------------
+template <bool FILL>
+__global__ void k_chain_build(uint32_t n_t, uint32_t row_lo, int delta, const int32_t* perm, const int32_t* inv,
+                              const long long* row_ptr, const int32_t* col, const void* w, int wtype,
+                              const int32_t* colour, const uint32_t* cptr, uint32_t* counts, uint16_t* idx16,
+                              int8_t* w8, uint32_t* orig_out) {
+    const uint32_t r = (uint32_t)(((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+    const uint32_t lane = threadIdx.x & 31u;
+    if (r >= n_t) return;
+    const int32_t orig = perm[row_lo + r];
+    const long long b = row_ptr[orig], e = row_ptr[orig + 1];
+    const int32_t c_own = delta ? colour[orig] : 0;
+    const unsigned long long base_at = FILL ? 4ull * cptr[r] : 0ull;
+    uint32_t cnt = 0;
+    for (long long at0 = b; at0 < e; at0 += 32) {
+        const long long i = at0 + lane;
+        bool ok = false;
+        uint32_t u = 0;
+        int wv = 0;
+        if (i < e) {
+            const int32_t j = col[i];
+            u = (uint32_t)inv[j];
+            ok = !delta || (u >= row_lo && colour[j] < c_own);
+            wv = wtype == 1 ? (int)reinterpret_cast<const int8_t*>(w)[i] : (int)reinterpret_cast<const int32_t*>(w)[i];
+        }
+        const uint32_t m = __ballot_sync(0xffffffffu, ok);
+        if (FILL && ok) {
+            const unsigned long long at = base_at + cnt + __popc(m & ((1u << lane) - 1u));
+            idx16[at] = (uint16_t)(u - row_lo);
+            w8[at] = (int8_t)wv;
+        }
+        cnt += __popc(m);
+    }
+    if (!FILL) {
+        if (lane == 0) counts[r] = (cnt + 3u) / 4u;
+    } else {
+        const unsigned long long end_at = 4ull * cptr[r + 1];   // padding (and the alignment gap before the next chunk)
+        for (unsigned long long at = base_at + cnt + lane; at < end_at; at += 32) {
+            idx16[at] = (uint16_t)r;
+            w8[at] = 0;
+        }
+        if (lane == 0) orig_out[r] = (uint32_t)orig;
+    }
+}
+
+}  // namespace ising

@@ -23,8 +23,8 @@
 //     sector per spin per tile of 32 replicas, so a neighbour gather is one sector and a
 //     thread pair reads it with two 16-byte loads;
 //   * ranges[phase][cta] is the static, cost-balanced split of every colour phase over the
-//     CTAs of the grid (launch-per-phase kernels; hubs also in the persistent kernel, which hands out
-//     the slices of a phase by ticket, phase_slices[phase] .. phase_slices[phase + 1]).
+//     CTAs of the grid (launch-per-phase kernels); the persistent kernel deals the slices
+//     phase_slices[phase] .. phase_slices[phase + 1] out itself (strided over all warps of the grid).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -50,9 +50,8 @@ struct SliceDesc {
     uint32_t meta;   // log2(SPR) | (valid rows << 8) | (parts P of the hub this slice is a part of, else 0) << 16
 };
 
-struct PhaseRange {  // work of one CTA in one colour phase (absolute indices)
-    uint32_t s0, s1; // slices
-    uint32_t h0, h1; // unused
+struct PhaseRange {  // work of one CTA in one colour phase of the launch-per-phase kernels (absolute slice indices)
+    uint32_t s0, s1;
 };
 
 enum SweepKind : int { kKindGS = 0, kKindJacobi = 1, kKindEval = 2 };

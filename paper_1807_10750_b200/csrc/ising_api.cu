@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "../../include/ising.h"
+#include "../../include/ising_debug.h"
 #include "builder.cuh"
 #include "common.cuh"
 #include "dense_tcgen05.cuh"
@@ -59,7 +60,6 @@ inline int spr_log2_for_degree(int64_t deg, int sub_row_edges) {
     return l;
 }
 
-constexpr uint32_t kTicketMode = 0;   // unit hand-out of the persistent kernel: 0 static stride, 1 CTA-local tickets, 2 grid-wide tickets
 constexpr int kClusterCtas = 8;       // portable cluster size; 8 x 16 warps per replica tile
 constexpr uint32_t kThrCap = 1u << 16;   // thresholds per persistent launch (longer schedules are chunked)
 
@@ -88,9 +88,10 @@ struct SmallArrays {
     int32_t* best_sweep;
     uint32_t* thr;         // kThrCap
     unsigned int* barrier;
-    unsigned int* tickets;  // 2 * phases
     int* flag;
 };
+
+size_t chain_ws_bound(int64_t n, int64_t nnz, int64_t tiles);
 
 size_t workspace_need(int64_t n, int64_t nnz, int wtype, int64_t max_replicas, int64_t C, bool wide,
                       uint64_t n_slices, uint64_t n_hubs, uint64_t cells, bool with_raw, bool dense) {
@@ -124,10 +125,11 @@ size_t workspace_need(int64_t n, int64_t nnz, int wtype, int64_t max_replicas, i
     add(4 * (size_t)tiles * kTile);           // best_sweep
     add(4 * (size_t)kThrCap);                 // thr
     add(256);                                 // barrier
-    add(8 * (size_t)phases);                  // tickets
     add(4 * (size_t)(phases + 1));            // phase_slices
     add(256);                                 // flag
     if (dense) add(dense_workspace_bytes(n, max_replicas));
+    add(4 * (size_t)(phases + 2));            // vphase_slices
+    if (C > 0) add(chain_ws_bound(n, nnz, (int64_t)tiles));
     return align_up(s) + kAlign;
 }
 
@@ -176,6 +178,15 @@ struct ising_problem {
     bool cooperative = false;
     uint32_t flush_rows = 1;
     unsigned long long* timing = nullptr;   // diagnostics buffer of the next Gauss-Seidel anneal
+    // chain engine (chain.cuh): either the whole graph (k_anneal_small) or the tail classes of the persistent kernel
+    ChainView chain{};
+    bool chain_small = false;
+    bool chain_delta = false;
+    uint32_t small_threads = 0;
+    size_t small_dyn = 0;
+    uint32_t* vphase_slices = nullptr;      // [n_vphases + 1] slice ranges of the persistent kernel's virtual phases
+    std::vector<uint32_t> thr_host;         // the call's thresholds (pageable copy: the caller's array is free on return)
+    uint32_t n_vphases = 0;
     uint32_t timing_sweep = 0;
 };
 
@@ -252,6 +263,135 @@ void launch_sweep_end(ising_problem* p, const uint8_t* src, int energy_mode, int
     k_sweep_end<<<dim3((unsigned)bx, (unsigned)tiles, 1), 256, 0, st>>>(ep);
     p->launches++;
     p->parity ^= 1;
+}
+
+
+// ---- chain engine, host side (chain.cuh) --------------------------------------------------------------
+constexpr uint32_t kTailRowsMax = 12288;        // most chain rows the persistent kernel's tail can hold (val <= 48 KB of the 144 KB)
+constexpr uint32_t kTailRowsDefault = 1600;     // chain rows of the tail: the chain walks ~150 warp instructions per row and word on ONE
+                                                // SM per four replicas, so it pays only for the classes that are pure latency on the grid
+                                                // (config 5, us per sweep: 700 rows 199.4, 1600 195.9, 2500 200.4, 4000 206.5, 12288 245.6)
+constexpr uint32_t kChainLevelThreads = 384;      // lanes per row: a level keeps about this many threads busy (the row
+                                                   // update runs on one lane of L: more lanes, more warps issuing it)
+constexpr uint64_t kSmallStreamBytesMax = 1ull << 20;   // a streamed small graph may re-read at most this per sweep and CTA
+
+// Tuning knobs read from the environment exist only in builds with -DISING_TUNING_ENV (never in the shipped library).
+inline int64_t tail_rows_limit() {
+#ifdef ISING_TUNING_ENV
+    if (const char* e = getenv("ISING_TAIL_ROWS")) return std::min<int64_t>(atoll(e), (int64_t)kTailRowsMax);
+#endif
+    return (int64_t)kTailRowsDefault;
+}
+inline uint32_t level_threads() {
+#ifdef ISING_TUNING_ENV
+    if (const char* e = getenv("ISING_LEVEL_THREADS")) return (uint32_t)atoi(e);
+#endif
+    return kChainLevelThreads;
+}
+inline uint32_t small_threads_override(uint32_t t) {
+#ifdef ISING_TUNING_ENV
+    if (const char* e = getenv("ISING_SMALL_THREADS")) return (uint32_t)atoi(e);
+#endif
+    return t;
+}
+inline uint32_t align4u(uint32_t x) { return (x + 3u) & ~3u; }
+inline uint32_t pow2_floor(uint32_t x) { uint32_t r = 1; while (2u * r <= x) r *= 2u; return r; }
+inline uint32_t pow2_ceil(uint32_t x) { uint32_t r = 1; while (r < x) r *= 2u; return r; }
+
+struct ChainPlan {
+    bool ok = false;
+    std::vector<ChainChunk> chunks;
+    std::vector<ChainSeg> segs;
+    std::vector<uint32_t> cptr;      // [n_t + 1] first cell of every row (a chunk starts at a multiple of 4)
+    std::vector<uint16_t> rel16;
+    uint32_t cells = 0;
+    uint32_t max_chunk_bytes = 0;
+    uint64_t total_bytes = 0;
+};
+
+// counts[r] = cells of local row r; lvl = ascending local row boundaries of the levels (front 0, back n_t).
+ChainPlan plan_chain(const std::vector<uint32_t>& counts, const std::vector<uint32_t>& lvl, uint32_t buf_bytes, bool delta,
+                     uint32_t threads) {
+    ChainPlan pl;
+    const uint32_t n_t = (uint32_t)counts.size();
+    pl.cptr.assign((size_t)n_t + 1, 0u);
+    uint32_t r0 = 0, cell = 0;
+    while (r0 < n_t) {
+        ChainChunk ck{};
+        ck.r0 = r0;
+        ck.c0 = cell;
+        uint32_t r1 = r0, nc = 0;
+        while (r1 < n_t) {
+            const uint32_t step_end = std::min(n_t, r1 + 8u);
+            uint32_t add = 0;
+            for (uint32_t r = r1; r < step_end; ++r) add += counts[r];
+            const uint32_t nc2 = align4u(nc + add);
+            if (nc2 > 65532u || chunk_layout(step_end - r0, nc2, delta).bytes > buf_bytes) break;
+            r1 = step_end;
+            nc += add;
+        }
+        if (r1 == r0) return pl;   // eight rows do not fit one buffer
+        uint32_t at = cell;
+        for (uint32_t r = r0; r < r1; ++r) { pl.cptr[r] = at; at += counts[r]; }
+        cell += align4u(nc);
+        ck.r1 = r1;
+        ck.c1 = cell;
+        const uint32_t bytes = chunk_layout(r1 - r0, ck.c1 - ck.c0, delta).bytes;
+        pl.max_chunk_bytes = std::max(pl.max_chunk_bytes, bytes);
+        pl.total_bytes += bytes;
+        pl.chunks.push_back(ck);
+        r0 = r1;
+    }
+    pl.cptr[n_t] = cell;
+    pl.cells = cell;
+    if (pl.chunks.size() > (size_t)kChainMaxChunks) return pl;
+    for (ChainChunk& ck : pl.chunks) {
+        ck.ptr_at = (uint32_t)pl.rel16.size();
+        for (uint32_t r = ck.r0; r < ck.r1; ++r) pl.rel16.push_back((uint16_t)(pl.cptr[r] - ck.c0));
+        pl.rel16.push_back((uint16_t)(ck.c1 - ck.c0));
+        while (pl.rel16.size() % 8u) pl.rel16.push_back(0);
+        ck.seg0 = (uint32_t)pl.segs.size();
+        for (size_t j = 0; j + 1 < lvl.size(); ++j) {
+            const uint32_t a = lvl[j], b = lvl[j + 1];
+            if (b <= a) continue;
+            const uint32_t s0 = std::max(a, ck.r0), s1 = std::min(b, ck.r1);
+            if (s0 >= s1) continue;
+            const uint32_t cells_seg = (s1 == ck.r1 ? ck.c1 : pl.cptr[s1]) - pl.cptr[s0];
+            const uint32_t avg = (cells_seg + (s1 - s0) - 1u) / (s1 - s0);
+            uint32_t L = std::min<uint32_t>(32u, pow2_ceil(std::max(1u, avg)));
+            L = std::min(L, pow2_floor(std::max(1u, std::min(threads, level_threads()) / (b - a))));
+            uint32_t logL = 0;
+            while ((1u << logL) < L) ++logL;
+            ChainSeg sg{};
+            sg.r0 = s0; sg.r1 = s1;
+            sg.info = logL | (b <= ck.r1 ? 0x100u : 0u);
+            pl.segs.push_back(sg);
+        }
+        ck.seg1 = (uint32_t)pl.segs.size();
+    }
+    while (pl.rel16.size() % 8u) pl.rel16.push_back(0);
+    if (pl.segs.size() > (size_t)kChainMaxSegs) return pl;
+    pl.ok = true;
+    return pl;
+}
+
+// Upper bound of what the chain arrays take in the workspace (either use).
+size_t chain_ws_bound(int64_t n, int64_t nnz, int64_t tiles) {
+    const uint64_t nt = (uint64_t)std::min<int64_t>(n, (int64_t)kChainMaxLocal);
+    const uint64_t cells = (uint64_t)nnz / 4 + nt + 4ull * kChainMaxChunks + 8;
+    const uint64_t tl = (uint64_t)std::min<int64_t>(tiles, kMaxPersistReplicas / kTile);
+    size_t b = 0;
+    auto add = [&](size_t x) { b = align_up(b) + x; };
+    add(4 * (nt + 2));                                   // counts / cell pointers
+    add(2 * (nt + 1 + 8ull * (kChainMaxChunks + 1)));    // rel16
+    add(4 * (nt + 16));                                  // orig
+    add(8 * cells);
+    add(4 * cells);
+    add(sizeof(ChainChunk) * kChainMaxChunks);
+    add(sizeof(ChainSeg) * kChainMaxSegs);
+    add(tl * kChainGroups * ((uint64_t)kTailRowsMax + 8) * 16);   // h0
+    add(tl * kChainGroups * ((uint64_t)kTailRowsMax + 8) * 4);    // old
+    return align_up(b) + kAlign;
 }
 
 ising_status check_device() {
@@ -506,6 +646,18 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         }
         return k;
     };
+    // Tail chain (chain.cuh, DELTA): the last colour classes of a big graph hold few, hub-like rows and cost a grid
+    // barrier plus a dependent unit each (config 5: 14 of 22 phases, 8 % of the edges, 29 % of the sweep).  If the
+    // classes c_tail .. C-1 hold at most kTailRows rows in all, the persistent kernel computes their fields in ONE
+    // bulk pseudo-phase and walks the classes inside one CTA per four replicas.  Graphs small enough for
+    // k_anneal_small are wholly a chain and need no tail.
+    int32_t c_tail = C;
+    if (colour && C >= 3 && !(flags & ISING_LOAD_NO_TAIL_CHAIN)) {
+        const int64_t tail_rows = tail_rows_limit();
+        int32_t c = C;
+        while (c > 1 && (int64_t)n - cstart[(size_t)c - 1] <= tail_rows) --c;
+        if (C - c >= 2) c_tail = c;
+    }
     {
         int32_t k = 0;
         for (int32_t c = 0; c < C; ++c) {
@@ -513,7 +665,8 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
             const size_t mark = slices.size();
             const uint32_t hub_mark = n_hub_rows;
             const int32_t k_end = emit_colour(c, k, kSubRowEdges);
-            if ((uint64_t)(slices.size() - mark) * tiles_all * 2ull < (uint64_t)sm_count * kWarpsPerCta) {   // latency-bound phase: less than half a round of the grid's warps
+            if (c < c_tail &&   // (the tail classes are throughput work of the bulk pseudo-phase)
+                (uint64_t)(slices.size() - mark) * tiles_all * 2ull < (uint64_t)sm_count * kWarpsPerCta) {   // latency-bound phase: less than half a round of the grid's warps
                 slices.resize(mark);
                 slice_aux.resize(2 * mark);
                 n_hub_rows = hub_mark;
@@ -567,7 +720,6 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
             PhaseRange& r = ranges[(size_t)c * n_cta + b];
             const double target = remaining / (double)(n_cta - b);
             double mine = 0;
-            r.h0 = r.h1 = 0;
             r.s0 = pos;
             if (b + 1 == n_cta) {
                 while (pos < end) mine += slice_cost(slices[pos++]);
@@ -597,7 +749,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     p->W = rep.w_sum / 2; p->absw_max = rep.absw_max; p->wide = wide;
     p->n_slices = (uint32_t)slices.size(); p->n_hubs = n_hub_rows; p->cells = cells;
     // latency-bound graphs whose biggest phase fits two rounds of one cluster's warps: cluster barrier instead of grid barrier
-    p->cluster_ctas = max_phase_slices <= 2u * kClusterCtas * kWarpsPerCta ? kClusterCtas : 0;   // (16-CTA clusters measured
+    p->cluster_ctas = (max_phase_slices <= 2u * kClusterCtas * kWarpsPerCta && !(flags & ISING_LOAD_NO_CLUSTER)) ? kClusterCtas : 0;   // (16-CTA clusters measured
     // slower on config 3: 108 vs 73 ms, the eight clusters do not all fit at once)
     p->n_phases = (uint32_t)C; p->n_cta = n_cta; p->sm_count = sm_count; p->cooperative = coop != 0;
     p->flush_rows = wide ? 0x7fffffffu
@@ -630,7 +782,6 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     p->sm.best_sweep = (int32_t*)ws.take(4 * tiles * kTile);
     p->sm.thr = (uint32_t*)ws.take(4 * (size_t)kThrCap);
     p->sm.barrier = (unsigned int*)ws.take(256);
-    p->sm.tickets = (unsigned int*)ws.take(8 * (size_t)C);
     p->phase_slices = (uint32_t*)ws.take(4 * ((size_t)C + 1));
     p->sm.flag = (int*)ws.take(256);
     void* dense_mem = nullptr;
@@ -661,6 +812,124 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
         p->dense = dense_create(n, max_replicas, dense_mem, dense_bytes, d_row_ptr, d_col, d_w, wtype, st);
         if (!p->dense) return fail(ISING_ERR_CUDA);
     }
+
+    // ---- chain engine (chain.cuh): the whole graph (k_anneal_small) or the tail classes of the persistent kernel
+    p->vphase_slices = (uint32_t*)ws.take(4 * ((size_t)C + 2));
+    if (ws.overflow) return fail(ISING_ERR_WORKSPACE_TOO_SMALL);
+    const bool persistent_ok = colour && !wide && coop != 0;
+    const bool try_small = colour && !wide && (int64_t)n <= (int64_t)kChainMaxLocal && !(flags & ISING_LOAD_NO_SMALL);
+    const bool try_tail = persistent_ok && c_tail < C && p->cluster_ctas == 0 &&
+                          n_cta >= (uint32_t)kChainGroups * (uint32_t)std::min<int>(p->tiles_max, kMaxPersistReplicas / kTile);
+    for (int pass = 0; pass < 2; ++pass) {   // the whole graph as a chain if it fits one CTA, else the tail classes
+        const bool delta = pass == 1;
+        if (delta ? (p->chain_small || !try_tail) : !try_small) continue;
+        const uint32_t row_lo = delta ? (uint32_t)cstart[(size_t)c_tail] : 0u;
+        const uint32_t n_t = (uint32_t)n - row_lo, n_t_pad = (n_t + 7u) & ~7u;
+        std::vector<uint32_t> lvl;
+        for (int32_t c = delta ? c_tail : 0; c <= C; ++c) lvl.push_back((uint32_t)cstart[(size_t)c] - row_lo);
+        uint32_t* d_cnt = (uint32_t*)ws.take(4 * ((size_t)n_t + 2));
+        if (ws.overflow) return fail(ISING_ERR_WORKSPACE_TOO_SMALL);
+        const unsigned cb = (unsigned)(((unsigned long long)n_t * 32 + 255) / 256);
+        k_chain_build<false><<<cb, 256, 0, st>>>(n_t, row_lo, delta ? 1 : 0, p->perm, p->inv, d_row_ptr, d_col, d_w, wtype,
+                                                 d_colour, nullptr, d_cnt, nullptr, nullptr, nullptr);
+        std::vector<uint32_t> counts(n_t);
+        CKP(cudaMemcpyAsync(counts.data(), d_cnt, 4 * (size_t)n_t, cudaMemcpyDeviceToHost, st));
+        CKP(cudaStreamSynchronize(st));
+        int smem_optin = 0;
+        {
+            int dev = 0;
+            CKP(cudaGetDevice(&dev));
+            CKP(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        }
+        ChainPlan pl;
+        bool resident = false;
+        uint32_t threads = kSweepThreads, buf_bytes = 0;
+        const uint32_t val_bytes = chain_align16(4u * n_t_pad) + chain_align16(n_t_pad);   // val[] + flip[]
+        if (delta) {
+            buf_bytes = val_bytes < kChainSmemBytes ? ((kChainSmemBytes - val_bytes) / 2u) & ~15u : 0u;
+            if (buf_bytes >= 4096u) pl = plan_chain(counts, lvl, buf_bytes, true, threads);
+        } else {
+            // CTA size: enough threads to give every row of the widest level min(32, its cells) lanes
+            uint64_t want = 128;
+            for (size_t j = 0; j + 1 < lvl.size(); ++j) {
+                const uint32_t rows = lvl[j + 1] - lvl[j];
+                if (!rows) continue;
+                uint64_t cells = 0;
+                for (uint32_t r = lvl[j]; r < lvl[j + 1]; ++r) cells += counts[r];
+                const uint32_t avg = (uint32_t)((cells + rows - 1) / rows);
+                want = std::max<uint64_t>(want, (uint64_t)rows * std::min<uint32_t>(4u, pow2_ceil(std::max(1u, avg))));
+            }
+            threads = (uint32_t)std::min<uint64_t>((uint64_t)kSmallThreadsMax, pow2_ceil((uint32_t)std::min<uint64_t>(want, 4096)));
+            threads = small_threads_override(std::max(threads, 256u));
+            cudaFuncAttributes fa{};
+            CKP(cudaFuncGetAttributes(&fa, k_anneal_small));
+            const int64_t cap = (int64_t)smem_optin - (int64_t)fa.sharedSizeBytes - (int64_t)val_bytes - 256;
+            if (cap >= 8192) {
+                pl = plan_chain(counts, lvl, (uint32_t)cap & ~15u, false, threads);
+                resident = pl.ok && pl.chunks.size() == 1;
+                buf_bytes = resident ? (pl.max_chunk_bytes + 15u) & ~15u : 0u;
+                if (!resident) {
+                    buf_bytes = ((uint32_t)(cap / 2)) & ~15u;
+                    pl = plan_chain(counts, lvl, buf_bytes, false, threads);
+                    if (pl.ok && pl.total_bytes > kSmallStreamBytesMax) pl.ok = false;
+                    if (pl.ok) buf_bytes = (pl.max_chunk_bytes + 15u) & ~15u;
+                }
+            }
+        }
+        if (pl.ok) {
+            uint32_t* d_cptr = d_cnt;   // (same buffer: n_t + 1 entries)
+            uint16_t* d_rel = (uint16_t*)ws.take(2 * (pl.rel16.size() + 8));
+            uint32_t* d_orig = (uint32_t*)ws.take(4 * ((size_t)n_t_pad + 16));
+            uint2* d_cidx = (uint2*)ws.take(8 * ((size_t)pl.cells + 4));
+            uint32_t* d_cw = (uint32_t*)ws.take(4 * ((size_t)pl.cells + 4));
+            ChainChunk* d_chunks = (ChainChunk*)ws.take(sizeof(ChainChunk) * pl.chunks.size());
+            ChainSeg* d_segs = (ChainSeg*)ws.take(sizeof(ChainSeg) * pl.segs.size());
+            int* d_h0 = nullptr;
+            uint32_t* d_old = nullptr;
+            const size_t tl = (size_t)std::min<int>(p->tiles_max, kMaxPersistReplicas / kTile);
+            if (delta) {
+                d_h0 = (int*)ws.take(tl * kChainGroups * (size_t)n_t_pad * 16);
+                d_old = (uint32_t*)ws.take(tl * kChainGroups * (size_t)n_t_pad * 4);
+            }
+            if (ws.overflow) return fail(ISING_ERR_WORKSPACE_TOO_SMALL);
+            CKP(cudaMemcpyAsync(d_cptr, pl.cptr.data(), 4 * pl.cptr.size(), cudaMemcpyHostToDevice, st));
+            CKP(cudaMemcpyAsync(d_rel, pl.rel16.data(), 2 * pl.rel16.size(), cudaMemcpyHostToDevice, st));
+            CKP(cudaMemcpyAsync(d_chunks, pl.chunks.data(), sizeof(ChainChunk) * pl.chunks.size(), cudaMemcpyHostToDevice, st));
+            CKP(cudaMemcpyAsync(d_segs, pl.segs.data(), sizeof(ChainSeg) * pl.segs.size(), cudaMemcpyHostToDevice, st));
+            CKP(cudaMemsetAsync(d_orig, 0, 4 * ((size_t)n_t_pad + 16), st));
+            if (delta) CKP(cudaMemsetAsync(d_h0, 0, tl * kChainGroups * (size_t)n_t_pad * 16, st));
+            k_chain_build<true><<<cb, 256, 0, st>>>(n_t, row_lo, delta ? 1 : 0, p->perm, p->inv, d_row_ptr, d_col, d_w, wtype,
+                                                    d_colour, d_cptr, nullptr, reinterpret_cast<uint16_t*>(d_cidx),
+                                                    reinterpret_cast<int8_t*>(d_cw), d_orig);
+            ChainView& v = p->chain;
+            v.chunks = d_chunks; v.segs = d_segs; v.rel16 = d_rel; v.orig = d_orig; v.cidx = d_cidx; v.cw = d_cw;
+            v.h0 = d_h0; v.old = d_old;
+            v.n_chunks = (uint32_t)pl.chunks.size(); v.n_segs = (uint32_t)pl.segs.size();
+            v.n_t = n_t; v.n_t_pad = n_t_pad; v.row_lo = row_lo; v.resident = resident ? 1u : 0u;
+            v.buf_bytes = buf_bytes; v.threads = threads;
+            v.narrow = (uint64_t)n_t * 2ull * (uint64_t)rep.absw_max < (1ull << 31) ? 1u : 0u;
+            if (delta) {
+                p->chain_delta = true;
+            } else {
+                p->chain_small = true;
+                p->small_threads = threads;
+                p->small_dyn = (size_t)val_bytes + (size_t)buf_bytes * (resident ? 1u : 2u);
+            }
+            CKP(cudaStreamSynchronize(st));   // the plan's host vectors die here
+        }
+    }
+    {
+        // virtual phases of the persistent kernel: the colour phases, or (tail chain) the phases before the tail plus
+        // ONE bulk pseudo-phase holding every slice of the tail classes
+        std::vector<uint32_t> vps;
+        const int32_t c_cut = p->chain_delta ? c_tail : C;
+        for (int32_t c = 0; c <= c_cut; ++c) vps.push_back(slice_begin[(size_t)c]);
+        if (p->chain_delta) vps.push_back(slice_begin[(size_t)C]);
+        p->n_vphases = (uint32_t)vps.size() - 1u;
+        CKP(cudaMemcpyAsync(p->vphase_slices, vps.data(), 4 * vps.size(), cudaMemcpyHostToDevice, st));
+        CKP(cudaStreamSynchronize(st));
+    }
+    p->ws_used = ws.used;
     CKP(cudaFuncSetAttribute(k_anneal_gs<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
     CKP(cudaFuncSetAttribute(k_anneal_gs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
     CKP(cudaStreamSynchronize(st));   // the host vectors die at return
@@ -732,6 +1001,11 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
     p->have_best = false;
     if (n_sweeps == 0) { CK(cudaGetLastError()); return ISING_OK; }
 
+    try {
+        p->thr_host.assign(thresholds, thresholds + n_sweeps);
+    } catch (...) {
+        return ISING_ERR_CUDA;
+    }
     const size_t small_bytes = 8 * (size_t)tiles * kTile;
     CK(cudaMemsetAsync(p->sm.accum[0], 0, small_bytes, st));
     CK(cudaMemsetAsync(p->sm.accum[1], 0, small_bytes, st));
@@ -759,7 +1033,49 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
     sp.tie_rule = tie_rule;
     sp.keys = keys;
 
-    if (mode == ISING_MODE_GS && !p->wide && p->cooperative) {
+    if (mode == ISING_MODE_GS && p->chain_small) {
+        // small graph (chain.cuh, FULL): initial energy from the definition, then ONE launch of independent CTAs (one per
+        // word of four replicas) per chunk of <= kThrCap sweeps; no grid-wide synchronisation at all
+        CK(cudaMemsetAsync(p->sm.accum_eval, 0, small_bytes, st));
+        SweepParams ev = sp;
+        ev.src = p->state[p->cur]; ev.dst = p->state[p->cur]; ev.accum = p->sm.accum_eval;
+        launch_sweep(p, kKindEval, ev, tiles, st);
+        k_finish_energy<<<(unsigned)((tiles * kTile + 255) / 256), 256, 0, st>>>(p->sm.accum_eval, p->W, tiles * kTile,
+                                                                              p->sm.E[0], nullptr);
+        p->launches++;
+        CK(cudaFuncSetAttribute(k_anneal_small, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->small_dyn));
+        for (int32_t s0 = 0; s0 < n_sweeps; s0 += (int32_t)kThrCap) {
+            const int32_t ns = std::min<int32_t>((int32_t)kThrCap, n_sweeps - s0);
+            CK(cudaMemcpyAsync(p->sm.thr, p->thr_host.data() + s0, 4 * (size_t)ns, cudaMemcpyHostToDevice, st));
+            SmallParams a{};
+            a.v = p->chain;
+            a.state = p->state[p->cur];
+            a.best = p->best;
+            a.best_compact = reinterpret_cast<uint32_t*>(p->state[p->cur ^ 1]);
+            a.bc_stride = n;
+            a.tile_stride = tile_stride;
+            a.n_replicas = (uint32_t)n_replicas;
+            a.rep0 = (uint32_t)first_replica;
+            a.tie_rule = tie_rule;
+            a.n_sweeps = (uint32_t)ns;
+            a.sweep_offset = (uint32_t)(sweep_offset + s0);
+            a.thr = p->sm.thr;
+            a.W = p->W;
+            a.E0 = p->sm.E[0];
+            a.trace = cut_trace ? (long long*)cut_trace + (size_t)s0 * n_replicas : nullptr;
+            a.trace_stride = (unsigned long long)n_replicas;
+            a.E_out = p->sm.E[0];
+            a.best_out = p->sm.bestcut[0];
+            a.best_sweep_out = p->sm.best_sweep;
+            a.resume = s0 > 0 ? 1 : 0;
+            a.timing = s0 == 0 ? p->timing : nullptr;
+            a.timing_sweep = p->timing_sweep;
+            a.keys = keys;
+            k_anneal_small<<<(unsigned)(tiles * kChainGroups), p->small_threads, p->small_dyn, st>>>(a);
+            p->launches++;
+        }
+        p->parity = 0;
+    } else if (mode == ISING_MODE_GS && !p->wide && p->cooperative) {
         // the hot path: initial energy from the definition (evaluation pass), then ONE persistent
         // cooperative launch per batch of <= 1024 replicas and chunk of <= kThrCap sweeps
         CK(cudaMemsetAsync(p->sm.accum_eval, 0, small_bytes, st));
@@ -774,10 +1090,9 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
             const int bt = std::min(kBatchTiles, tiles - t0);
             for (int32_t s0 = 0; s0 < n_sweeps; s0 += (int32_t)kThrCap) {
                 const int32_t ns = std::min<int32_t>((int32_t)kThrCap, n_sweeps - s0);
-                CK(cudaMemcpyAsync(p->sm.thr, thresholds + s0, 4 * (size_t)ns, cudaMemcpyHostToDevice, st));
+                CK(cudaMemcpyAsync(p->sm.thr, p->thr_host.data() + s0, 4 * (size_t)ns, cudaMemcpyHostToDevice, st));
                 CK(cudaMemsetAsync(p->sm.accum3, 0, 8 * 3 * (size_t)kMaxPersistReplicas, st));
                 CK(cudaMemsetAsync(p->sm.barrier, 0, 256, st));
-                CK(cudaMemsetAsync(p->sm.tickets, 0, 8 * (size_t)p->n_phases, st));
                 AnnealParams a{};
                 a.g = graph_view(p);
                 a.state = p->state[p->cur] + (size_t)t0 * tile_stride;
@@ -801,18 +1116,17 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
                 a.best_out = p->sm.bestcut[0] + (size_t)t0 * kTile;
                 a.best_sweep_out = p->sm.best_sweep + (size_t)t0 * kTile;
                 a.barrier = p->sm.barrier;
-                a.tickets = p->sm.tickets;
-                a.ticket_mode = kTicketMode;
-                if (const char* e = getenv("ISING_TICKET_MODE")) a.ticket_mode = (uint32_t)atoi(e) % 3u;   // tuning knob
+                a.vphase_slices = p->vphase_slices;
+                a.n_vphases = p->n_vphases;
+                a.chain_on = p->chain_delta ? 1u : 0u;
+                a.chain = p->chain;
                 a.resume = s0 > 0 ? 1 : 0;
                 a.timing = (t0 == 0 && s0 == 0) ? p->timing : nullptr;
                 a.timing_sweep = p->timing_sweep;
                 a.keys = keys;
                 bool cluster = p->cluster_ctas > 0 && !p->timing;   // (the phase-timing diagnostics belong to the grid kernel)
-                if (const char* e = getenv("ISING_CLUSTER")) cluster = cluster && atoi(e) != 0;   // tuning knob
                 if (cluster) {
                     // small graph: one cluster of kClusterCtas CTAs per replica tile, hardware cluster barrier
-                    a.ticket_mode = 0;
                     cudaLaunchConfig_t cfg{};
                     cfg.gridDim = dim3((unsigned)(bt * p->cluster_ctas));
                     cfg.blockDim = dim3(kSweepThreads);
@@ -1041,6 +1355,12 @@ ising_status ising_problem_info(const ising_problem* p, int32_t what, int64_t* v
         case 10: *value_out = (int64_t)p->cells * 4; break;
         case 11: *value_out = p->n_hubs; break;
         case 12: *value_out = p->n_cta; break;
+        case 13: *value_out = p->chain_small ? 4 : !(p->n_colours > 0 && !p->wide && p->cooperative) ? 0
+                                  : p->chain_delta ? 3 : p->cluster_ctas > 0 ? 2 : 1; break;
+        case 14: *value_out = (p->chain_small || p->chain_delta) ? p->chain.n_t : 0; break;
+        case 15: *value_out = p->n_vphases; break;
+        case 16: *value_out = (p->chain_small || p->chain_delta) ? p->chain.n_chunks : 0; break;
+        case 17: *value_out = (p->chain_small || p->chain_delta) ? p->chain.resident : 0; break;
         default: return ISING_ERR_BAD_SHAPE;
     }
     return ISING_OK;

@@ -21,39 +21,10 @@
 //                the cut reduction, trace and best-state capture fused in (a7, a9).
 #pragma once
 #include "common.cuh"
+#include "primitives.cuh"
+#include "chain.cuh"
 
 namespace ising {
-
-// 4x4 byte transpose: in e[j] = bytes (replica 0..3) of edge j; out t[b] = bytes (edge 0..3)
-// of replica b.
-__device__ __forceinline__ void transpose4x4(uint32_t e0, uint32_t e1, uint32_t e2, uint32_t e3,
-                                             uint32_t& t0, uint32_t& t1, uint32_t& t2, uint32_t& t3) {
-    const uint32_t x0 = __byte_perm(e0, e1, 0x5140);
-    const uint32_t x1 = __byte_perm(e2, e3, 0x5140);
-    const uint32_t x2 = __byte_perm(e0, e1, 0x7362);
-    const uint32_t x3 = __byte_perm(e2, e3, 0x7362);
-    t0 = __byte_perm(x0, x1, 0x5410);
-    t1 = __byte_perm(x0, x1, 0x7632);
-    t2 = __byte_perm(x2, x3, 0x5410);
-    t3 = __byte_perm(x2, x3, 0x7632);
-}
-
-__device__ __forceinline__ void field_word(int (&h)[16], int k, uint32_t e0, uint32_t e1, uint32_t e2,
-                                           uint32_t e3, uint32_t w) {
-    uint32_t t0, t1, t2, t3;
-    transpose4x4(e0, e1, e2, e3, t0, t1, t2, t3);
-    h[4 * k + 0] = __dp4a((int)t0, (int)w, h[4 * k + 0]);
-    h[4 * k + 1] = __dp4a((int)t1, (int)w, h[4 * k + 1]);
-    h[4 * k + 2] = __dp4a((int)t2, (int)w, h[4 * k + 2]);
-    h[4 * k + 3] = __dp4a((int)t3, (int)w, h[4 * k + 3]);
-}
-
-__device__ __forceinline__ int sbyte(uint32_t word, int b) { return (int)(int8_t)(word >> (8 * b)); }
-
-__device__ __forceinline__ void field_word_wide(int (&h)[16], int k, uint32_t e, int w) {
-#pragma unroll
-    for (int b = 0; b < 4; ++b) h[4 * k + b] += sbyte(e, b) * w;
-}
 
 __device__ __forceinline__ void field_cell(int (&h)[16], const uint4& e0, const uint4& e1, const uint4& e2,
                                            const uint4& e3, uint32_t w) {
@@ -73,15 +44,6 @@ __device__ __forceinline__ void field_cell_wide(int (&h)[16], const uint4& e0, c
     field_word_wide(h, 2, e2.z, w.z); field_word_wide(h, 3, e2.w, w.z);
     field_word_wide(h, 0, e3.x, w.w); field_word_wide(h, 1, e3.y, w.w);
     field_word_wide(h, 2, e3.z, w.w); field_word_wide(h, 3, e3.w, w.w);
-}
-
-__device__ __forceinline__ uint32_t nibble_to_bytemask(uint32_t nib) {
-    // bit b of nib -> byte b = 0xff (the four copies of nib at shifts 0, 7, 14, 21 do not overlap)
-    return ((nib * 0x00204081u) & 0x01010101u) * 0xffu;
-}
-
-__device__ __forceinline__ uint32_t lt4(const uint4& u, uint32_t thr) {
-    return (u.x < thr ? 1u : 0u) | (u.y < thr ? 2u : 0u) | (u.z < thr ? 4u : 0u) | (u.w < thr ? 8u : 0u);
 }
 
 // Flip decisions of Algorithm 2 (L177) for the 16 replicas rep_lane0 .. rep_lane0+15 of spin
@@ -195,24 +157,8 @@ struct PassCtx {
     uint32_t rep_lane0;    // global id of this lane's replica 0
     uint32_t thr, T;
     int32_t tie_rule;
-    uint32_t tile;         // replica tile of this unit (index into hub_acc / hub_cnt)
-    unsigned long long* stamp;   // diagnostics: SM-clock stamps of this unit's stages (one lane of one warp), or nullptr
+    uint32_t tile;         // replica tile of this unit (index into hub_acc / hub_cnt / h0)
 };
-__device__ __forceinline__ void dbg_stamp(const PassCtx& x, int k) {
-    if (x.stamp) x.stamp[k] = (unsigned long long)clock64();
-}
-
-__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
-    uint32_t r;
-    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(sel));
-    return r;
-}
-// byte b of the result = 0xff if v_b < 0 else 0x00 (PRMT sign replication of the top bytes)
-__device__ __forceinline__ uint32_t sign_bytes(int v0, int v1, int v2, int v3) {
-    const uint32_t t0 = prmt((uint32_t)v0, (uint32_t)v1, 0xfbfbu);
-    const uint32_t t1 = prmt((uint32_t)v2, (uint32_t)v3, 0xfbfbu);
-    return prmt(t0, t1, 0x5410u);
-}
 
 // a4-a7 for one row and this lane's 16 replicas, four replicas (one word of spin bytes) at a time.
 template <int KIND, typename Acc>
@@ -325,7 +271,6 @@ __device__ __forceinline__ void part_finish(const GraphView& g, const PassCtx& x
         asm volatile("atom.relaxed.gpu.global.add.u64 %0, [%1], %2;" : "=l"(now) : "l"(sp), "l"(mine) : "memory");
         speculate();
         now += mine;
-        dbg_stamp(x, 5);
         if ((uint32_t)(__shfl_sync(0xffffffffu, now, 0) >> 32) != parts) return;
         while ((uint32_t)(now >> 32) != parts)
             asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(now) : "l"(sp) : "memory");
@@ -342,7 +287,6 @@ __device__ __forceinline__ void part_finish(const GraphView& g, const PassCtx& x
             asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(g.hub_cnt + slot) : "memory");
         speculate();
         old = __shfl_sync(0xffffffffu, old, 0);
-        dbg_stamp(x, 5);
         if ((old + 1u) % parts != 0u) return;
         __syncwarp();
         total = __ldcg(accp);
@@ -352,7 +296,6 @@ __device__ __forceinline__ void part_finish(const GraphView& g, const PassCtx& x
     for (int k = 0; k < 16; ++k) h[k] = __shfl_sync(0xffffffffu, total, 2 * k + half);   // replica half * 16 + k
     if (sr == 0) {
         row_update<KIND>(x, h, so4, bold, finish_flip_mask(flip, x.rep_lane0), row_off, acc);
-        dbg_stamp(x, 6);
     }
 }
 
@@ -459,33 +402,6 @@ constexpr int kGatherSlots = 2 * 4 + 1;
 constexpr uint32_t kSlotBytes = kSweepThreads * 16;                    // one slot of every thread of the CTA
 constexpr uint32_t kGatherBufBytes = kGatherSlots * kSlotBytes;
 
-__device__ __forceinline__ void cp_async16(uint32_t smem_addr, const void* gptr) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr), "l"(gptr) : "memory");
-}
-__device__ __forceinline__ void prefetch_l2(const void* gptr) {
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(gptr));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-__device__ __forceinline__ uint4 lds128(uint32_t smem_addr) {
-    uint4 v;
-    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(smem_addr));
-    return v;
-}
-
-__device__ __forceinline__ void cp_async4(uint32_t smem_addr, const void* gptr) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_addr), "l"(gptr) : "memory");
-}
-__device__ __forceinline__ uint32_t lds32(uint32_t smem_addr) {
-    uint32_t v;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(smem_addr));
-    return v;
-}
-__device__ __forceinline__ void sts32(uint32_t smem_addr, uint32_t v) {
-    asm volatile("st.shared.u32 [%0], %1;" ::"r"(smem_addr), "r"(v) : "memory");
-}
-
 // Static data of a unit on its way to the compute stage.  Only the eight neighbour indices of the head groups
 // travel through registers (they form the gather addresses); weights, caller ids and the descriptor go straight
 // from global to shared memory (cp.async): meta slot m of this thread = {w0, w1, orig}, descriptor slot of the
@@ -523,22 +439,25 @@ __device__ __forceinline__ HeadIdx request_head(const GraphView& g, const PipeAd
 
 // src: the unit's tile, lane half included.  gb: shared address of slot 0 of this thread in the target buffer.
 __device__ __forceinline__ void issue_slice_gathers(const uint8_t* src, const HeadIdx& hd, const SliceDesc& d, int sr,
-                                                    uint32_t gb) {
+                                                    uint32_t gb, bool own) {
     const int log_spr = (int)(d.meta & 0xffu);
     const int nrows = (int)((d.meta >> 8) & 0xffu);
     const int rloc = sr >> log_spr;
     const bool owner = ((sr & ((1 << log_spr) - 1)) == 0) && rloc < nrows;
-    cp_async16(gb + 0 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.x * kTile);
-    cp_async16(gb + 1 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.y * kTile);
-    cp_async16(gb + 2 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.z * kTile);
-    cp_async16(gb + 3 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.w * kTile);
+    // padding entries (weight 0) point at the sub-row's own row: they are not fetched at all (zero-filled slot), which
+    // saves their L1 wavefronts (15 % of the slots of config 5)
+    const uint32_t pad = d.row0 + (rloc < nrows ? (uint32_t)rloc : 0u);
+    cp_async16_if(gb + 0 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.x * kTile, (uint32_t)hd.c0.x != pad);
+    cp_async16_if(gb + 1 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.y * kTile, (uint32_t)hd.c0.y != pad);
+    cp_async16_if(gb + 2 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.z * kTile, (uint32_t)hd.c0.z != pad);
+    cp_async16_if(gb + 3 * kSlotBytes, src + (size_t)(uint32_t)hd.c0.w * kTile, (uint32_t)hd.c0.w != pad);
     if (d.G > 1) {
-        cp_async16(gb + 4 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.x * kTile);
-        cp_async16(gb + 5 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.y * kTile);
-        cp_async16(gb + 6 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.z * kTile);
-        cp_async16(gb + 7 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.w * kTile);
+        cp_async16_if(gb + 4 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.x * kTile, (uint32_t)hd.c1.x != pad);
+        cp_async16_if(gb + 5 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.y * kTile, (uint32_t)hd.c1.y != pad);
+        cp_async16_if(gb + 6 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.z * kTile, (uint32_t)hd.c1.z != pad);
+        cp_async16_if(gb + 7 * kSlotBytes, src + (size_t)(uint32_t)hd.c1.w * kTile, (uint32_t)hd.c1.w != pad);
     }
-    if (owner) cp_async16(gb + 8 * kSlotBytes, src + (size_t)(d.row0 + (uint32_t)rloc) * kTile);
+    if (owner && own) cp_async16(gb + 8 * kSlotBytes, src + (size_t)(d.row0 + (uint32_t)rloc) * kTile);
     cp_async_commit();
 }
 
@@ -549,10 +468,48 @@ __device__ __forceinline__ SliceDesc lds_desc(uint32_t addr) {
     return d;
 }
 
+// BULK pseudo-phase of the persistent kernel (chain.cuh, DELTA): the slices of the chain rows' colour classes do not
+// update their rows; they add the rows' local fields, computed from the values all spins hold before the chain, to
+// h0[tile][replica >> 2][row - row_lo][replica & 3] (fire-and-forget integer REDs; the chain clears them).
+struct BulkDst {
+    int* h0;
+    uint32_t row_lo, n_t_pad;
+};
+__device__ __forceinline__ void bulk_red(int* p, int v) {
+    asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void bulk_deposit(const BulkDst& bd, uint32_t tile, const SliceDesc& d, int (&h)[16],
+                                             int log_spr, bool owner, int rloc) {
+    const int lane = threadIdx.x & 31, sr = lane >> 1, half = lane & 1;
+    if ((d.meta >> 16) != 0u || log_spr == 4) {   // one row per slice: lane (sr, half) deposits replica half * 16 + sr
+        uint32_t none = 0;
+        half_reduce16(h, none, half);
+        int v = h[0];
+#pragma unroll
+        for (int k = 1; k < 16; ++k) v = sr == k ? h[k] : v;
+        const uint32_t rep = (uint32_t)(half * 16 + sr);
+        bulk_red(bd.h0 + ((((size_t)tile * kChainGroups + (rep >> 2)) * bd.n_t_pad + (d.row0 - bd.row_lo)) << 2) + (rep & 3u), v);
+    } else {
+        for (int lvl = 0; lvl < log_spr; ++lvl) {
+#pragma unroll
+            for (int k = 0; k < 16; ++k) h[k] += __shfl_xor_sync(0xffffffffu, h[k], 2 << lvl);
+        }
+        if (owner) {
+            const uint32_t lr = d.row0 + (uint32_t)rloc - bd.row_lo;
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                const uint32_t rep = (uint32_t)(half * 16 + k);
+                bulk_red(bd.h0 + ((((size_t)tile * kChainGroups + (rep >> 2)) * bd.n_t_pad + lr) << 2) + (rep & 3u), h[k]);
+            }
+        }
+    }
+}
+
 // Compute stage of one (slice, tile) unit whose head gathers have landed in buffer gb (Gauss-Seidel, int8 weights).
 template <typename Acc>
 __device__ __forceinline__ void slice_compute(const GraphView& g, const PassCtx& x, const SliceDesc& d, uint32_t ma,
-                                              int sr, const Acc& acc, const PhiloxKeys& keys, uint32_t gb) {
+                                              int sr, const Acc& acc, const PhiloxKeys& keys, uint32_t gb, bool bulk,
+                                              const BulkDst& bd) {
     // ma: this thread's meta slot of the unit (w0, w1, orig one word plane apart)
     const int log_spr = (int)(d.meta & 0xffu);
     const int nrows = (int)((d.meta >> 8) & 0xffu);
@@ -560,7 +517,7 @@ __device__ __forceinline__ void slice_compute(const GraphView& g, const PassCtx&
     const int rloc = sr >> log_spr;
     const bool owner = ((sr & (int)(spr - 1)) == 0) && rloc < nrows;
     const size_t row_off = (size_t)(d.row0 + (uint32_t)rloc) * kTile;
-    const uint4 bold = ld_best_early<kKindGS>(x, owner, row_off);
+    const uint4 bold = ld_best_early<kKindGS>(x, owner && !bulk, row_off);
     // tail cells (rows of 129..256 edges only): through registers, requested right away
     const size_t tail_at = (size_t)d.off + sr;
     int4 c2 = make_int4(0, 0, 0, 0), c3 = c2;
@@ -576,7 +533,7 @@ __device__ __forceinline__ void slice_compute(const GraphView& g, const PassCtx&
     uint32_t flip = 0;
     const uint32_t orig = lds32(ma + 2u * kSweepThreads * 4u);
     const uint32_t parts = d.meta >> 16;
-    if (orig != 0xffffffffu && parts == 0u)
+    if (orig != 0xffffffffu && parts == 0u && !bulk)
         flip = flip_mask_part(orig, x.T, x.rep_lane0, x.thr, (uint32_t)sr & (spr - 1), spr, keys);
 
     int h[16];
@@ -602,10 +559,13 @@ __device__ __forceinline__ void slice_compute(const GraphView& g, const PassCtx&
             field_cell(h, e0, e1, e2, e3, w2);
         }
     }
+    if (bulk) {
+        bulk_deposit(bd, x.tile, d, h, log_spr, owner, rloc);
+        return;
+    }
     uint4 so4 = make_uint4(0u, 0u, 0u, 0u);
     if (owner) so4 = lds128(gb + 8 * kSlotBytes);
 
-    dbg_stamp(x, 4);
     if (parts != 0u) {   // hub part: sorig = {caller id, hub id, part index, ...}
         const uint32_t orig0 = __shfl_sync(0xffffffffu, orig, 0), hub = __shfl_sync(0xffffffffu, orig, 2);
         part_finish<kKindGS, true>(g, x, d.row0, parts, orig0, hub, h, so4, acc, keys);
@@ -625,9 +585,9 @@ __device__ __forceinline__ void slice_compute(const GraphView& g, const PassCtx&
 }
 
 __device__ __forceinline__ PhaseRange ld_range(const PhaseRange* p) {
-    const int4 v = ld_stream(reinterpret_cast<const int4*>(p));
+    const uint2 v = __ldg(reinterpret_cast<const uint2*>(p));
     PhaseRange r;
-    r.s0 = (uint32_t)v.x; r.s1 = (uint32_t)v.y; r.h0 = (uint32_t)v.z; r.h1 = (uint32_t)v.w;
+    r.s0 = v.x; r.s1 = v.y;
     return r;
 }
 
@@ -645,7 +605,6 @@ __device__ __forceinline__ PassCtx make_ctx(const uint8_t* src, uint8_t* dst, ui
     x.T = T;
     x.tie_rule = tie_rule;
     x.tile = tile;
-    x.stamp = nullptr;
     return x;
 }
 
@@ -703,7 +662,8 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_sweep(const SweepParams p)
 // grid = g.n_cta CTAs (one per SM at most), all co-resident.
 // ---------------------------------------------------------------------------------------------
 constexpr size_t kAnnealDynSmem = 16 * kSweepThreads * sizeof(int) + 2 * (size_t)kGatherBufBytes + kMetaBytes + kDescBytes;   // s_dE, two gather buffers, meta / descriptor slots
-constexpr int kRangeCache = 128;   // phases whose per-CTA ranges are kept in shared memory
+constexpr int kPhaseCache = 128;   // virtual phases whose slice ranges are kept in shared memory
+constexpr uint32_t kChainSmemBytes = 2u * kGatherBufBytes;   // what the chain may use of the dynamic shared memory (the gather buffers)
 
 struct AnnealParams {
     GraphView g;
@@ -727,13 +687,16 @@ struct AnnealParams {
     long long* best_out;            // [tiles*32]
     int32_t* best_sweep_out;        // [tiles*32]
     unsigned int* barrier;          // zero at launch
-    unsigned int* tickets;          // [2][n_phases] slice-ticket counters (sweep parity x phase), zero at launch
-    uint32_t ticket_mode;           // how a warp gets its units after the static first one: 0 static stride (unit k of a warp =
-                                    // its static unit + k * n_static), 1 CTA-local tickets (shared-memory counter over the CTA's
-                                    // stride set), 2 grid-wide tickets (global counter)
     int32_t resume;                 // 1: best_out / best_sweep_out hold the bests of the sweeps before this chunk
-    unsigned long long* timing;     // diagnostics: [n_phases][n_cta][8] SM-clock stamps of sweep timing_sweep (0/1: barrier
-                                    // arrive / leave, 2-6: stages of the first unit of warp 0), or nullptr
+    // Virtual phases of a sweep: the colour phases 0 .. n_vphases-1 as slice ranges.  With a chain (chain_on), the
+    // last virtual phase is the BULK pseudo-phase: every slice of the chain rows' colour classes, fields deposited in
+    // chain.h0 instead of updating the rows; the chain (chain.cuh, DELTA) follows it on CTAs 0 .. 8 * tiles - 1.
+    const uint32_t* vphase_slices;  // [n_vphases + 1]
+    uint32_t n_vphases;
+    uint32_t chain_on;
+    ChainView chain;
+    unsigned long long* timing;     // diagnostics: [n_vphases + 1][n_cta][8] SM-clock stamps of sweep timing_sweep (0 / 1: arrival at
+                                    // / departure from the barrier that ends the virtual phase; row n_vphases: the chain), or nullptr
     uint32_t timing_sweep;
     PhiloxKeys keys;
 };
@@ -746,7 +709,7 @@ struct AnnealParams {
 constexpr unsigned kBarrierBackoffNs = 40;
 template <bool CLUSTER>
 __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& epoch, unsigned int n_cta,
-                                             unsigned long long* stamp, unsigned int* s_next) {
+                                             unsigned long long* stamp) {
     if (CLUSTER) {   // hardware barrier of the thread-block cluster; release / acquire at cluster scope covers global memory
         asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
         return;
@@ -754,16 +717,13 @@ __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int
     __syncthreads();
     epoch += n_cta;
     if (stamp && threadIdx.x == 0) stamp[0] = (unsigned long long)clock64();
-    if (threadIdx.x == 0) {
-        *s_next = (unsigned int)kWarpsPerCta;   // CTA-local unit tickets of the next phase (no warp draws one right now)
-        if (n_cta > 1) {
-            asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
-            unsigned int v;
-            for (;;) {
-                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
-                if ((int)(v - epoch) >= 0) break;
-                __nanosleep(kBarrierBackoffNs);
-            }
+    if (threadIdx.x == 0 && n_cta > 1) {
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
+        unsigned int v;
+        for (;;) {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
+            if ((int)(v - epoch) >= 0) break;
+            __nanosleep(kBarrierBackoffNs);
         }
     }
     __syncthreads();
@@ -775,8 +735,10 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     __shared__ long long s_acc[kMaxPersistReplicas];
     __shared__ long long s_wacc[kWarpsPerCta][kTile];
     __shared__ uint32_t s_wtile[kWarpsPerCta];
-    __shared__ unsigned int s_next;           // CTA-local unit tickets (ticket_mode 1)
-    __shared__ PhaseRange s_ranges[kRangeCache];
+    __shared__ uint32_t s_ps[kPhaseCache + 1];                // first slice of every virtual phase
+    __shared__ ChainChunk s_chunks[CLUSTER ? 1 : kChainMaxChunks];
+    __shared__ ChainSeg s_segs[CLUSTER ? 1 : kChainMaxSegs];
+    __shared__ long long s_cdE[4];
     // 128-byte alignment matters: a warp's 512-byte row of 16-byte slots must not straddle a fifth 128-byte line
     // (measured: +18 % time when the static arrays happened to end 16 bytes past a line)
     extern __shared__ __align__(128) int s_dE_raw[];         // dynamic: [16][kSweepThreads] per-thread energy increments (SmemAcc)
@@ -794,17 +756,19 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     __shared__ uint32_t s_mask[kMaxPersistReplicas / kTile];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int sr = lane >> 1, half = lane & 1;
-    // CLUSTER: one thread-block cluster per replica tile (small graphs: the units of a phase fit the warps of a few
-    // SMs): the CTAs of a cluster share nothing with the other clusters, and the barrier between colour phases is
-    // the hardware cluster barrier (~0.2 us) instead of the grid barrier (~1 us).  Otherwise: one cooperative grid
-    // for all tiles.
+    // CLUSTER: one thread-block cluster per replica tile (graphs whose phases fit the warps of a few SMs but not one
+    // CTA's shared memory): the CTAs of a cluster share nothing with the other clusters, and the barrier between
+    // colour phases is the hardware cluster barrier (~0.2 us) instead of the grid barrier (~1 us).  Otherwise: one
+    // cooperative grid for all tiles.
     uint32_t cta = blockIdx.x, n_cta = p.g.n_cta, tile0 = 0;
     if (CLUSTER) {
         asm("mov.u32 %0, %%cluster_ctarank;" : "=r"(cta));
         asm("mov.u32 %0, %%cluster_nctarank;" : "=r"(n_cta));
         asm("mov.u32 %0, %%clusterid.x;" : "=r"(tile0));
     }
-    const uint32_t tiles = CLUSTER ? 1u : p.tiles, nR = tiles * kTile, C = p.g.n_phases;
+    const uint32_t tiles = CLUSTER ? 1u : p.tiles, nR = tiles * kTile, VP = p.n_vphases;
+    const bool chain_on = !CLUSTER && p.chain_on != 0u;
+    const bool chain_cta = chain_on && cta < (uint32_t)kChainGroups * tiles;
     // per-tile views of the launch parameters (grid variant: the parameters themselves, read where they are used)
     auto state = [&]() { return CLUSTER ? p.state + (size_t)tile0 * p.tile_stride : p.state; };
     auto bestp = [&]() { return CLUSTER ? p.best + (size_t)tile0 * p.tile_stride : p.best; };
@@ -823,8 +787,22 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
         s_bsweep[i] = p.resume ? best_sweep_out()[i] : 0;
     }
     if (threadIdx.x < kMaxPersistReplicas / kTile) s_mask[threadIdx.x] = 0u;
-    if (threadIdx.x == 0) s_next = (unsigned int)kWarpsPerCta;
+    if (threadIdx.x < 4) s_cdE[threadIdx.x] = 0;
     s_wacc[threadIdx.x >> 5][threadIdx.x & 31] = 0;
+    for (uint32_t i = threadIdx.x; i <= min(VP, (uint32_t)kPhaseCache); i += blockDim.x) s_ps[i] = __ldg(p.vphase_slices + i);
+    // chain CTA (cta = 8 * tile + g owns the word of replicas 4 g .. 4 g + 3 of every chain row of its tile): tables
+    // into shared memory, compact copy of the chain rows' current spin words
+    const uint32_t ctile = cta / (uint32_t)kChainGroups, cgrp = cta % (uint32_t)kChainGroups;
+    if constexpr (!CLUSTER) if (chain_cta) {
+        const ChainView& v = p.chain;
+        for (uint32_t i = threadIdx.x; i < v.n_chunks * (uint32_t)(sizeof(ChainChunk) / 4); i += blockDim.x)
+            reinterpret_cast<uint32_t*>(s_chunks)[i] = __ldg(reinterpret_cast<const uint32_t*>(v.chunks) + i);
+        for (uint32_t i = threadIdx.x; i < v.n_segs * (uint32_t)(sizeof(ChainSeg) / 4); i += blockDim.x)
+            reinterpret_cast<uint32_t*>(s_segs)[i] = __ldg(reinterpret_cast<const uint32_t*>(v.segs) + i);
+        const uint8_t* sp = p.state + (size_t)ctile * p.tile_stride + (size_t)v.row_lo * kTile + 4u * cgrp;
+        for (uint32_t r = threadIdx.x; r < v.n_t; r += blockDim.x)
+            v.old[(size_t)cta * v.n_t_pad + r] = __ldcg(reinterpret_cast<const uint32_t*>(sp + (size_t)r * kTile));
+    }
     __syncthreads();
 
     const SmemAcc acc{&s_dE[0][threadIdx.x]};
@@ -832,91 +810,64 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     for (int k = 0; k < 16; ++k) s_dE[k][threadIdx.x] = 0;
     uint32_t rows_acc = 0, acc_tile = 0;
     unsigned int epoch = 0;
+    BulkDst bd{};
+    if (!CLUSTER) { bd.h0 = p.chain.h0; bd.row_lo = p.chain.row_lo; bd.n_t_pad = p.chain.n_t_pad; }
 
-    // work of all phases, staged once in shared memory (first kRangeCache phases): the slices of the whole phase
-    // (shared by all CTAs, see below)
-    const PhaseRange* my_ranges = p.g.ranges + cta;
-    auto load_range = [&](uint32_t ph_) {
-        PhaseRange r = ld_range(CLUSTER ? p.g.ranges : my_ranges + (size_t)ph_ * n_cta);   // (s0 / s1 are replaced below)
-        r.s0 = __ldg(p.g.phase_slices + ph_);
-        r.s1 = __ldg(p.g.phase_slices + ph_ + 1);
-        return r;
-    };
-    for (uint32_t i = threadIdx.x; i < min(C, (uint32_t)kRangeCache); i += blockDim.x) s_ranges[i] = load_range(i);
-    __syncthreads();
-    auto range_of = [&](uint32_t ph_) { return ph_ < (uint32_t)kRangeCache ? s_ranges[ph_] : load_range(ph_); };
-    // Slice units of a phase (heaviest first): the first n_cta * 16 are static, unit warp * n_cta + cta belongs to
-    // this warp, so its static data can be prefetched across the grid barrier; the rest are handed out by a ticket
-    // counter (one atomic per unit, requested one unit ahead), which evens out cache luck.
+    auto ps_of = [&](uint32_t vp_) { return vp_ <= (uint32_t)kPhaseCache ? s_ps[vp_] : __ldg(p.vphase_slices + vp_); };
+    // Slice units of a phase (heaviest first) are dealt out statically: unit k of warp w of CTA b is
+    // w * n_cta + b + k * (16 n_cta), so every warp gets the same mix of heavy and light units and the static data of
+    // its first unit can be requested across the barrier that precedes the phase.
     const uint32_t n_static = n_cta * (uint32_t)kWarpsPerCta;
     const uint32_t u_static = (uint32_t)warp * n_cta + cta;
-    PhaseRange pr = range_of(0u);
-    uint32_t nu = (pr.s1 - pr.s0) * tiles;
-    // one-unit lookahead of the static data, kept across the grid barrier
+    uint32_t ps0 = ps_of(0u);
+    uint32_t nu = (ps_of(1u) - ps0) * tiles;
+    // one-unit lookahead of the static data, kept across the barrier
     bool have = u_static < nu;
     HeadIdx nxt{};
     uint32_t mslot = 0;   // meta slot of the unit whose head is in flight (`nxt`)
-    if (have) nxt = tiles == 1u ? request_head(p.g, pa, mslot, pr.s0 + u_static, 0u, sr, lane)
-                              : request_head(p.g, pa, mslot, pr.s0 + u_static / tiles, u_static % tiles, sr, lane);
+    if (have) nxt = tiles == 1u ? request_head(p.g, pa, mslot, ps0 + u_static, 0u, sr, lane)
+                              : request_head(p.g, pa, mslot, ps0 + u_static / tiles, u_static % tiles, sr, lane);
 
     for (uint32_t t = 0; t < p.n_sweeps; ++t) {
         const uint32_t thr = __ldg(p.thr + t);
         const uint32_t T = p.sweep_offset + t;
-        for (uint32_t ph = 0; ph < C; ++ph) {
-            const bool last_phase = ph + 1 == C;
+        unsigned long long* const tsw = (!CLUSTER && p.timing && t == p.timing_sweep) ? p.timing + (size_t)cta * 8 : nullptr;
+        for (uint32_t vp = 0; vp < VP; ++vp) {
+            const bool last_phase = vp + 1 == VP;
             const bool very_last = last_phase && t + 1 == p.n_sweeps;
-            const PhaseRange prn = range_of(last_phase ? 0u : ph + 1u);
-            const bool dyn = nu > n_static;   // then every warp of the grid owns a static unit
-            unsigned int* ticket_ctr = p.tickets + (size_t)(t & 1u) * C + ph;
-            if (!CLUSTER && cta == 0 && threadIdx.x == 0) p.tickets[(size_t)((t + 1u) & 1u) * C + ph] = 0u;   // last used a sweep ago
-            unsigned int tk = 0;
-            uint32_t u_pos = u_static;
-            if (dyn && lane == 0) {   // ticket of this warp's second unit (drawn one unit ahead from here on)
-                if (p.ticket_mode == 1u) tk = atomicAdd(&s_next, 1u);
-                else if (p.ticket_mode == 2u) tk = atomicAdd(ticket_ctr, 1u);
-            }
+            const bool bulk = chain_on && last_phase;
+            const uint32_t vpn = last_phase ? 0u : vp + 1u;
+            const uint32_t psn0 = ps_of(vpn), psn1 = ps_of(vpn + 1u);
 
             if (have) {
                 // software pipeline: unit k is computed from gather buffer gb while the gathers of unit k+1 fly
                 // into the other buffer and the head of unit k+2 is on its way (indices -> `nxt`, the rest -> its
-                // meta slot); with tickets, the ticket of the unit after that is being drawn
+                // meta slot)
                 SliceDesc pend_d{};
                 uint32_t pend_tile = 0;
+                uint32_t u_pos = u_static;
                 auto stage_next = [&](uint32_t gb_) {   // needs: head of `nxt` landed (cp.async.wait_group 0 + __syncwarp)
                     pend_d = lds_desc(pa.desc(mslot));
                     pend_tile = lds32(pa.desc(mslot) + 16);
-                    issue_slice_gathers(state() + (size_t)pend_tile * p.tile_stride + (size_t)half * 16, nxt, pend_d, sr, gb_);
+                    issue_slice_gathers(state() + (size_t)pend_tile * p.tile_stride + (size_t)half * 16, nxt, pend_d, sr, gb_, !bulk);
                     if (pend_d.G > (uint32_t)kHeadGroups) {   // tail cells: towards L2 now, read when the unit is computed
                         const size_t tail_at = (size_t)pend_d.off + sr;
                         if (half == 0) prefetch_l2(p.g.col4 + tail_at);
                         else if (pend_d.G > (uint32_t)kHeadGroups + 1u) prefetch_l2(p.g.col4 + tail_at + kSubRows);
                         if (lane == 0) prefetch_l2(p.g.w4 + tail_at);
                     }
-                    have = false;
-                    if (dyn) {
-                        uint32_t u;
-                        if (p.ticket_mode == 0u) u = (u_pos += n_static);
-                        else if (p.ticket_mode == 1u) u = __shfl_sync(0xffffffffu, tk, 0) * n_cta + cta;
-                        else u = n_static + __shfl_sync(0xffffffffu, tk, 0);
-                        have = u < nu;
-                        if (have) {
-                            mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
-                            nxt = tiles == 1u ? request_head(p.g, pa, mslot, pr.s0 + u, 0u, sr, lane)
-                                              : request_head(p.g, pa, mslot, pr.s0 + u / tiles, u % tiles, sr, lane);
-                            if (lane == 0) {
-                                if (p.ticket_mode == 1u) tk = atomicAdd(&s_next, 1u);
-                                else if (p.ticket_mode == 2u) tk = atomicAdd(ticket_ctr, 1u);
-                            }
-                        }
+                    u_pos += n_static;
+                    have = u_pos < nu;
+                    if (have) {
+                        mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
+                        nxt = tiles == 1u ? request_head(p.g, pa, mslot, ps0 + u_pos, 0u, sr, lane)
+                                          : request_head(p.g, pa, mslot, ps0 + u_pos / tiles, u_pos % tiles, sr, lane);
                     }
                 };
                 uint32_t gb = gbuf0;
                 cp_async_wait<0>();
                 __syncwarp();
                 uint32_t cur_m = mslot;
-                bool first_unit = true;
-                unsigned long long* ts = (!CLUSTER && p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + cta) * 8 : nullptr;
-                if (ts && threadIdx.x == 0) ts[2] = (unsigned long long)clock64();
                 stage_next(gb);
                 while (true) {
                     const SliceDesc cur_d = pend_d;
@@ -938,9 +889,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                                             : make_ctx(state(), state(), bestp(), s_mask[tile], p.tile_stride, tile, half, rep0(),
                                                        thr, T, p.tie_rule);
                     if (CLUSTER) x.tile += tile0;   // hub accumulators are indexed by the global tile
-                    if (first_unit && ts && threadIdx.x == 0) { x.stamp = ts; ts[3] = (unsigned long long)clock64(); }
-                    first_unit = false;
-                    slice_compute(p.g, x, cur_d, pa.meta(cur_m, 0), sr, acc, p.keys, gb);
+                    slice_compute(p.g, x, cur_d, pa.meta(cur_m, 0), sr, acc, p.keys, gb, bulk, bd);
                     if (++rows_acc >= p.flush_rows) {
                         flush_warp(acc, s_wacc[warp], lane);
                         rows_acc = 0;
@@ -952,20 +901,20 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             }
 
             // static data of this warp's first slice of the next phase: issued before the barrier
-            pr = prn;
-            nu = (pr.s1 - pr.s0) * tiles;
+            ps0 = psn0;
+            nu = (psn1 - psn0) * tiles;
             have = !very_last && u_static < nu;
-            if (have && p.ticket_mode != 2u && u_static + n_static < nu) {   // this warp's second unit: head towards L2
+            if (have && u_static + n_static < nu) {   // this warp's second unit: head towards L2
                 const uint32_t u2 = u_static + n_static;
-                const uint32_t s2 = pr.s0 + (tiles == 1u ? u2 : u2 / tiles);
+                const uint32_t s2 = ps0 + (tiles == 1u ? u2 : u2 / tiles);
                 const size_t at2 = (size_t)s2 * (kHeadGroups * kSubRows) + sr;
                 prefetch_l2(half == 0 ? p.g.col4 + at2 : p.g.col4 + at2 + kSubRows);
                 if (lane == 0) { prefetch_l2(p.g.w4 + at2); prefetch_l2(p.g.sorig + (size_t)s2 * kSubRows); prefetch_l2(p.g.slices + s2); }
             }
             if (have) {
                 mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
-                nxt = tiles == 1u ? request_head(p.g, pa, mslot, pr.s0 + u_static, 0u, sr, lane)
-                              : request_head(p.g, pa, mslot, pr.s0 + u_static / tiles, u_static % tiles, sr, lane);
+                nxt = tiles == 1u ? request_head(p.g, pa, mslot, ps0 + u_static, 0u, sr, lane)
+                              : request_head(p.g, pa, mslot, ps0 + u_static / tiles, u_static % tiles, sr, lane);
             }
 
             if (last_phase) {   // a7: this sweep's energy increments -> accum slot t % 3
@@ -1001,8 +950,37 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                     }
                 }
             }
-            grid_barrier<CLUSTER>(p.barrier, epoch, n_cta,
-                         (!CLUSTER && p.timing && t == p.timing_sweep) ? p.timing + ((size_t)ph * n_cta + cta) * 8 : nullptr, &s_next);
+            grid_barrier<CLUSTER>(p.barrier, epoch, n_cta, tsw ? tsw + (size_t)vp * n_cta * 8 : nullptr);
+        }
+
+        if constexpr (!CLUSTER) if (chain_on) {
+            // the chain: the last colour classes level by level inside one CTA per word of four replicas
+            if (chain_cta) {
+                const ChainView& v = p.chain;
+                ChainRt rt;
+                rt.thr = thr; rt.T = T; rt.rl0 = p.rep0 + ctile * kTile + 4u * cgrp; rt.tie_rule = p.tie_rule;
+                ChainGlobal cgl;
+                const size_t o = (size_t)ctile * p.tile_stride + (size_t)v.row_lo * kTile + 4u * cgrp;
+                cgl.state = p.state + o;
+                cgl.best = p.best + o;
+                cgl.old = v.old + (size_t)cta * v.n_t_pad;
+                cgl.cap4 = (s_mask[ctile] >> (4u * cgrp)) & 15u;
+                long long cdE[4] = {0, 0, 0, 0};
+                const uint32_t cflip = gbuf_base + chain_align16(4u * v.n_t_pad);
+                chain_pass_streamed<true>(v, s_chunks, s_segs, gbuf_base, cflip, cflip + chain_align16(v.n_t_pad), cta, rt,
+                                          p.keys, cdE, cgl, threadIdx.x, (uint32_t)kSweepThreads, false,
+                                          (tsw && cta == 0 && threadIdx.x == 0) ? p.timing : nullptr, n_cta * 8u);
+                chain_reduce_dE(cdE, s_cdE, threadIdx.x, v.narrow != 0u);
+                __syncthreads();
+                if (threadIdx.x < 4) {
+                    const long long v4 = s_cdE[threadIdx.x];
+                    if (v4 != 0)
+                        atomicAdd(reinterpret_cast<unsigned long long*>(p.accum + (size_t)(t % 3u) * nR + ctile * kTile +
+                                                                         4u * cgrp + threadIdx.x), (unsigned long long)v4);
+                    s_cdE[threadIdx.x] = 0;
+                }
+            }
+            grid_barrier<CLUSTER>(p.barrier, epoch, n_cta, tsw ? tsw + (size_t)VP * n_cta * 8 : nullptr);
         }
 
         // sweep end (every CTA redundantly): E, cut = (W - E)/2 (eq. 4), improved mask

@@ -1,5 +1,5 @@
 """C-ABI boundary checks that need no GPU (`-m "not gpu"`): the shared library loads, exports
-every symbol include/ising.h declares, and its host-only entry points behave."""
+every symbol include/*.h declares, and its host-only entry points behave."""
 import ctypes
 import os
 import re
@@ -12,9 +12,14 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def declared_symbols():
-    src = open(os.path.join(ROOT, "include", "ising.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(ising_[a-z_]+)\s*\(", src)))
+    names = set()
+    for header in sorted(os.listdir(os.path.join(ROOT, "include"))):
+        if not header.endswith(".h"):
+            continue
+        src = open(os.path.join(ROOT, "include", header)).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names |= set(re.findall(r"\b(ising_[a-z_]+)\s*\(", src))
+    return sorted(names)
 
 
 def test_library_builds_and_exports_every_declared_symbol():

@@ -367,32 +367,57 @@ def test_config5_midsize_uses_both_sub_row_lengths():
     assert_same(g, o, best_spins=False)
 
 
-@pytest.mark.parametrize("ticket_mode", ["1", "2"])
-def test_ticket_scheduling_knob_gives_identical_results(ticket_mode, monkeypatch):
-    """ISING_TICKET_MODE (tuning knob of the persistent kernel: units handed out by a CTA-local or a grid-wide
-    ticket counter instead of the static stride) must not change any result."""
-    wl = W.config5(n=300000, sweeps=4, replicas=32)
-    monkeypatch.setenv("ISING_TICKET_MODE", ticket_mode)
-    g = gpu_anneal(wl, want_best_spins=False)
-    monkeypatch.delenv("ISING_TICKET_MODE")
-    o = oracle_anneal(wl)
-    assert_same(g, o, best_spins=False)
+ENGINE_FLAGS = {
+    "small": 0,                                                     # whole graph inside one CTA per four replicas
+    "cluster": P.ISING_LOAD_NO_SMALL,                                # one thread-block cluster per replica tile
+    "grid": P.ISING_LOAD_NO_SMALL | P.ISING_LOAD_NO_CLUSTER | P.ISING_LOAD_NO_TAIL_CHAIN,   # cooperative grid, every class a phase
+    "grid+tail": P.ISING_LOAD_NO_SMALL | P.ISING_LOAD_NO_CLUSTER,    # cooperative grid, last classes as a shared-memory chain
+}
+ENGINE_CODE = {"small": P.ENGINE_SMALL, "cluster": P.ENGINE_CLUSTER, "grid": P.ENGINE_GRID, "grid+tail": P.ENGINE_GRID_TAIL_CHAIN}
 
 
-@pytest.mark.parametrize("cluster", ["0", "1"])
-def test_small_graph_through_grid_and_cluster_kernels(cluster, monkeypatch):
-    """Small graphs run the persistent kernel as one thread-block cluster per replica tile (hardware cluster barrier
-    between colour phases); ISING_CLUSTER=0 forces the cooperative-grid variant.  Both must match the oracle, also
-    with several tiles, a ragged replica count, KEEP ties and a continued run."""
-    monkeypatch.setenv("ISING_CLUSTER", cluster)
+@pytest.mark.parametrize("engine", ["small", "cluster", "grid"])
+def test_small_graph_through_every_gauss_seidel_engine(engine):
+    """A small graph runs wholly inside one CTA per four replicas (shared-memory chain); load flags force the
+    cluster and the cooperative-grid variants of the persistent kernel.  All must match the oracle, also with several
+    tiles, a ragged replica count, KEEP ties and a continued run."""
     wl = er_workload(900, 0.015, 67, "pm4", np.int8, 75, 40, seed=6, p0=0.2)
-    g = gpu_anneal(wl, tie_rule=1)
+    g = gpu_anneal(wl, tie_rule=1, flags=ENGINE_FLAGS[engine])
+    assert g["problem"].engine == ENGINE_CODE[engine]
     o = oracle_anneal(wl, tie_rule=1)
     assert_same(g, o)
     g1 = gpu_anneal(wl, thr=wl.thr[:15], problem=g["problem"])
     g2 = gpu_anneal(wl, thr=wl.thr[15:], sweep_offset=15, init_mode=P.ISING_INIT_CONTINUE, problem=g["problem"])
     np.testing.assert_array_equal(g2["final"], oracle_anneal(wl)["final"])
-    monkeypatch.delenv("ISING_CLUSTER")
+
+
+@pytest.mark.parametrize("engine", ["grid", "grid+tail"])
+@pytest.mark.parametrize("replicas,first", [(32, 0), (70, 5)])
+def test_power_law_graph_with_and_without_tail_chain(engine, replicas, first):
+    """Config-5-shaped graph: the last colour classes (few hub rows each) run as a shared-memory chain after one bulk
+    pseudo-phase, or as grid-wide phases.  Ragged replica count over several tiles, a first replica that is not a
+    multiple of four (two Philox calls per word), KEEP ties, trace / best state, and a continued run."""
+    wl = W.config5(n=120000, sweeps=9, replicas=replicas)
+    g = gpu_anneal(wl, first_replica=first, tie_rule=1, flags=ENGINE_FLAGS[engine])
+    assert g["problem"].engine == ENGINE_CODE[engine]
+    if engine == "grid+tail":
+        assert 0 < g["problem"].info(14) <= 12288 and g["problem"].info(15) < wl.n_colours
+    o = oracle_anneal(wl, first_replica=first, tie_rule=1, n_threads=16)
+    assert_same(g, o)
+    g1 = gpu_anneal(wl, thr=wl.thr[:4], first_replica=first, problem=g["problem"], want_best_spins=False)
+    g2 = gpu_anneal(wl, thr=wl.thr[4:], sweep_offset=4, first_replica=first, init_mode=P.ISING_INIT_CONTINUE,
+                    problem=g["problem"], want_best_spins=False)
+    np.testing.assert_array_equal(g2["final"], oracle_anneal(wl, first_replica=first, n_threads=16)["final"])
+
+
+def test_small_graph_streamed_through_shared_memory():
+    """A graph whose packed edges do not fit one CTA's shared memory but whose spins do: the chain engine streams the
+    edge chunks through two buffers every sweep (several chunks, levels cut across chunks)."""
+    wl = er_workload(6000, 0.008, 71, "pm4", np.int8, 8, 12, seed=9, p0=0.2)    # ~290k directed edges: ~0.9 MB of cells
+    g = gpu_anneal(wl)
+    assert g["problem"].engine == P.ENGINE_SMALL and g["problem"].info(17) == 0 and g["problem"].info(16) > 2
+    o = oracle_anneal(wl, n_threads=8)
+    assert_same(g, o)
 
 
 def test_more_replicas_than_one_persistent_launch():
@@ -413,14 +438,15 @@ def test_schedule_longer_than_one_threshold_chunk():
 
 def test_phase_timing_diagnostics_do_not_change_results():
     wl = W.config5(n=8000, sweeps=6, replicas=32)
-    p = P.load_workload(wl)
+    p = P.load_workload(wl, flags=ENGINE_FLAGS["grid+tail"])
     stamps = p.phase_timing(2)
     g = gpu_anneal(wl, problem=p)
     o = oracle_anneal(wl)
     assert_same(g, o)
     t = stamps.cpu().numpy()
-    assert t.shape == (wl.n_colours, p.info(12), 8)   # 0/1: barrier arrive / leave, 2-6: stages of one unit
-    assert (t[:, :, 1] >= t[:, :, 0]).all() and (t[:, :, 0] > 0).all()
+    assert t.shape == (p.info(15) + 1, p.info(12), 8)   # 0/1: barrier arrive / leave, per virtual phase (+ the chain)
+    rows = p.info(15) + (1 if p.engine == P.ENGINE_GRID_TAIL_CHAIN else 0)
+    assert (t[:rows, :, 1] >= t[:rows, :, 0]).all() and (t[:rows, :, 0] > 0).all()
 
 
 def test_edge_list_file_workload(tmp_path):
