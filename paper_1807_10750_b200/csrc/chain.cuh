@@ -184,6 +184,7 @@ __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChun
             h2 = __dp4a((int)t2, (int)w, h2);
             h3 = __dp4a((int)t3, (int)w, h3);
         }
+        // (a REDUX per group member mask was measured 3x slower than the butterfly: the groups of a warp are serialised)
         for (uint32_t o = 1; o < L; o <<= 1) {
             h0 += __shfl_xor_sync(0xffffffffu, h0, o);
             h1 += __shfl_xor_sync(0xffffffffu, h1, o);
@@ -280,9 +281,10 @@ __device__ __forceinline__ void chain_pass_streamed(const ChainView& v, const Ch
     }
 }
 
-// Sum of the threads' dE[] into s_dE[4] (shared; zero before).  narrow: every partial sum of a sweep fits int32
-// (chain rows x 2 max_i sum_j |w_ij| < 2^31, checked at load): one REDUX per value and one atomic per warp.
-__device__ __forceinline__ void chain_reduce_dE(long long (&dE)[4], long long* s_dE, uint32_t tid, bool narrow) {
+// Warp sums of the threads' dE[] into s_wdE[warp][4] (plain stores; the caller adds the warps' slots up after a CTA
+// barrier).  narrow: every partial sum of a sweep fits int32 (chain rows x 2 max_i sum_j |w_ij| < 2^31, checked at load):
+// one REDUX per value instead of a 64-bit butterfly.
+__device__ __forceinline__ void chain_reduce_dE(long long (&dE)[4], long long (*s_wdE)[4], uint32_t tid, bool narrow) {
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
         long long x = dE[b];
@@ -292,10 +294,14 @@ __device__ __forceinline__ void chain_reduce_dE(long long (&dE)[4], long long* s
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
         }
-        if ((tid & 31u) == 0u && x != 0)
-            atomicAdd(reinterpret_cast<unsigned long long*>(s_dE + b), (unsigned long long)x);
+        if ((tid & 31u) == 0u) s_wdE[tid >> 5][b] = x;
         dE[b] = 0;
     }
+}
+__device__ __forceinline__ long long chain_sum_dE(const long long (*s_wdE)[4], uint32_t b, uint32_t n_warps) {
+    long long x = 0;
+    for (uint32_t w = 0; w < n_warps; ++w) x += s_wdE[w][b];
+    return x;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -331,7 +337,8 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
     extern __shared__ __align__(128) uint8_t chain_smem[];
     __shared__ ChainChunk s_chunks[kChainMaxChunks];
     __shared__ ChainSeg s_segs[kChainMaxSegs];
-    __shared__ long long s_dE[4], s_E[4], s_bc[4];
+    __shared__ long long s_wdE[kSmallThreadsMax / 32][4];
+    __shared__ long long s_E[4], s_bc[4];
     __shared__ int s_bs[4];
     __shared__ uint32_t s_imp;
     const uint32_t tid = threadIdx.x, nthr = blockDim.x;
@@ -356,7 +363,6 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
         if (p.resume) bcomp[r] = __ldcg(reinterpret_cast<const uint32_t*>(gbest + (size_t)r * kTile));
     }
     if (tid < 4u) {
-        s_dE[tid] = 0;
         s_E[tid] = p.E0[r_first + tid];
         s_bc[tid] = p.resume ? p.best_out[r_first + tid] : (long long)0x8000000000000000ull;
         s_bs[tid] = p.resume ? p.best_sweep_out[r_first + tid] : 0;
@@ -391,16 +397,15 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
         } else {
             chain_pass_streamed<false>(v, s_chunks, s_segs, val, flip, buf0, slot, rt, p.keys, dE, cg, tid, nthr, false);
         }
-        chain_reduce_dE(dE, s_dE, tid, v.narrow != 0u);
+        chain_reduce_dE(dE, s_wdE, tid, v.narrow != 0u);
         __syncthreads();
         if (ts) *ts++ = (unsigned long long)clock64();
         if (tid < 4u) {   // a7: E, cut = (W - E)/2 (eq. 4), best tracking (strictly greater: the earliest sweep wins)
-            const long long E = s_E[tid] + s_dE[tid];
+            const long long E = s_E[tid] + chain_sum_dE(s_wdE, tid, nthr >> 5);
             const long long cut = (p.W - E) / 2;
             const bool live = r_first + tid < p.n_replicas;
             const bool improved = live && cut > s_bc[tid];
             s_E[tid] = E;
-            s_dE[tid] = 0;
             if (improved) { s_bc[tid] = cut; s_bs[tid] = (int)rt.T; }
             if (live && p.trace) p.trace[(size_t)t * p.trace_stride + r_first + tid] = cut;
             const uint32_t m = __ballot_sync(0xfu, improved);

@@ -738,7 +738,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     __shared__ uint32_t s_ps[kPhaseCache + 1];                // first slice of every virtual phase
     __shared__ ChainChunk s_chunks[CLUSTER ? 1 : kChainMaxChunks];
     __shared__ ChainSeg s_segs[CLUSTER ? 1 : kChainMaxSegs];
-    __shared__ long long s_cdE[4];
+    __shared__ long long s_cdE[kWarpsPerCta][4];
     // 128-byte alignment matters: a warp's 512-byte row of 16-byte slots must not straddle a fifth 128-byte line
     // (measured: +18 % time when the static arrays happened to end 16 bytes past a line)
     extern __shared__ __align__(128) int s_dE_raw[];         // dynamic: [16][kSweepThreads] per-thread energy increments (SmemAcc)
@@ -787,7 +787,6 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
         s_bsweep[i] = p.resume ? best_sweep_out()[i] : 0;
     }
     if (threadIdx.x < kMaxPersistReplicas / kTile) s_mask[threadIdx.x] = 0u;
-    if (threadIdx.x < 4) s_cdE[threadIdx.x] = 0;
     s_wacc[threadIdx.x >> 5][threadIdx.x & 31] = 0;
     for (uint32_t i = threadIdx.x; i <= min(VP, (uint32_t)kPhaseCache); i += blockDim.x) s_ps[i] = __ldg(p.vphase_slices + i);
     // chain CTA (cta = 8 * tile + g owns the word of replicas 4 g .. 4 g + 3 of every chain row of its tile): tables
@@ -973,11 +972,10 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 chain_reduce_dE(cdE, s_cdE, threadIdx.x, v.narrow != 0u);
                 __syncthreads();
                 if (threadIdx.x < 4) {
-                    const long long v4 = s_cdE[threadIdx.x];
+                    const long long v4 = chain_sum_dE(s_cdE, threadIdx.x, (uint32_t)kWarpsPerCta);
                     if (v4 != 0)
                         atomicAdd(reinterpret_cast<unsigned long long*>(p.accum + (size_t)(t % 3u) * nR + ctile * kTile +
                                                                          4u * cgrp + threadIdx.x), (unsigned long long)v4);
-                    s_cdE[threadIdx.x] = 0;
                 }
             }
             grid_barrier<CLUSTER>(p.barrier, epoch, n_cta, tsw ? tsw + (size_t)VP * n_cta * 8 : nullptr);
