@@ -95,9 +95,9 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def measured_int8_peak():
-    """Dense int8 tensor peak in TOP/s: the measured bf16 cuBLAS figure x the nominal int8:bf16 ratio of 2
-    (B200_PROFILING.md: 4.5 vs 2.25 PFLOP/s dense); sustained figure, the kernel runs inside a long step."""
+def derived_int8_peak():
+    """Dense int8 tensor peak in TOP/s derived from the driver's figure: measured sustained bf16 x the nominal
+    int8:bf16 ratio of 2 (B200_PROFILING.md: 4.5 vs 2.25 PFLOP/s dense)."""
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
         try:
@@ -106,6 +106,77 @@ def measured_int8_peak():
         except Exception:
             pass
     return 2.0 * 1400.0, "2 x fallback sustained bf16 1.4 PFLOP/s (B200_PROFILING.md)"
+
+
+def probe_int8_peak(torch, seconds: float = 1.5):
+    """PROBE ONLY (never on the product path): what the library int8 GEMM of this box sustains, in TOP/s
+    (torch._int_mm = cuBLASLt int8 x int8 -> int32, 8192^3, back to back for `seconds`)."""
+    try:
+        n = 8192
+        a = torch.randint(-8, 9, (n, n), dtype=torch.int8, device="cuda")
+        b = torch.randint(-8, 9, (n, n), dtype=torch.int8, device="cuda")
+        for _ in range(3):
+            torch._int_mm(a, b)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps, t_ms, best = 0, 0.0, 0.0
+        while t_ms < seconds * 1e3:
+            e0.record()
+            for _ in range(10):
+                torch._int_mm(a, b)
+            e1.record()
+            torch.cuda.synchronize()
+            dt = e0.elapsed_time(e1)
+            t_ms += dt
+            reps += 10
+            best = max(best, 10 * 2.0 * n ** 3 / (dt * 1e-3) / 1e12)
+        return {"sustained_tops": reps * 2.0 * n ** 3 / (t_ms * 1e-3) / 1e12, "burst_tops": best,
+                "how": "torch._int_mm 8192^3 int8 (cuBLASLt), %d calls back to back" % reps}
+    except Exception as ex:   # no int8 GEMM in this torch build: the derived figure stands alone
+        return {"error": repr(ex)}
+
+
+# A colour class of a small graph costs at least one CTA barrier plus one dependent chain
+# "shared-memory index -> shared-memory spin -> dp4a -> butterfly -> sign -> store" (DESIGN.md 7): ~200 SM cycles.
+LEVEL_FLOOR_US = 0.10
+
+
+def workload_roofline(wl, us_per_sweep, engine, hbm_peak, l2, int8):
+    """SURVEY 8(d) 'which roofline bounds the path', per workload, from the measured time per sweep."""
+    R, n, nnz = wl.n_replicas, wl.n, wl.nnz
+    alg = algorithmic_bytes_per_sweep(n, nnz, R)
+    t = us_per_sweep * 1e-6
+    if wl.mode == "jacobi" and engine == "dense":
+        ops = 2.0 * n * n * R
+        ach = ops / t / 1e12
+        out = {"bound": "tensor", "achieved": ach, "unit": "TOP/s (int8 MAC = 2 ops)",
+               "peak": int8.get("peak"), "frac": ach / int8["peak"], "peak_source": int8.get("peak_source"),
+               "peak_derived_2x_bf16": int8.get("derived"), "frac_of_derived": ach / int8["derived"]}
+        return out
+    if n >= 200_000:   # graph streamed from HBM, 32 MB of spins gathered from L2 (config 5)
+        b_hbm = nnz * 5 + 4 * (n + 1)
+        b_l2 = (nnz * 32 + 2 * n * 32) * ((R + 31) // 32)
+        t_roof = max(b_hbm * ((R + 31) // 32) / (hbm_peak * 1e9), b_l2 / (l2["gather_gbs"] * 1e9)) if l2.get("gather_gbs") else None
+        out = {"bound": "hbm", "achieved": alg / t / 1e9, "unit": "GB/s", "peak": hbm_peak, "frac": alg / t / 1e9 / hbm_peak,
+               "l2": {"gather_peak_gbs": l2.get("gather_gbs"), "stream_peak_gbs": l2.get("stream_gbs"),
+                      "gather_bytes_per_sweep": b_l2, "hbm_stream_bytes_per_sweep": b_hbm * ((R + 31) // 32),
+                      "t_roof_us": None if t_roof is None else t_roof * 1e6,
+                      "frac_of_t_roof": None if t_roof is None else t_roof / t,
+                      "note": "T_roof = max(B_hbm / BW_hbm, B_l2 / BW_l2) (SURVEY 8(d)): the gathers are L2 hits, so this -- not "
+                              "the HBM-normalised frac the contract asks for -- says how far the sweep is from the memory system's limit"}}
+        return out
+    levels = max(1, wl.n_colours)
+    if n * ((R + 31) // 32) <= 4000:   # one replica's state is a few KB: a dependent level per colour class (configs 1, 2)
+        us_level = us_per_sweep / levels
+        return {"bound": "latency", "achieved": us_level, "unit": "us per colour class", "peak": LEVEL_FLOOR_US,
+                "frac": LEVEL_FLOOR_US / us_level, "levels_per_sweep": levels,
+                "effective_gbs": alg / t / 1e9,
+                "note": "floor = one CTA barrier + one dependent shared-memory chain per colour class (DESIGN.md 7)"}
+    ach = alg / t / 1e9   # everything on chip (config 3): algorithmic bytes against what L2 streams
+    return {"bound": "l2", "achieved": ach, "unit": "GB/s", "peak": l2.get("stream_gbs"),
+            "frac": None if not l2.get("stream_gbs") else ach / l2["stream_gbs"], "levels_per_sweep": levels,
+            "note": "graph and spins live in shared memory for the whole call (no L2 traffic inside a sweep); the figure is "
+                    "SURVEY 8(d)'s algorithmic bytes over the measured L2 streaming bandwidth"}
 
 
 # --------------------------------------------------------------------------------------------

@@ -21,6 +21,16 @@ extern "C" {
  */
 ising_status ising_debug_phase_timing(ising_problem* p, uint64_t* stamps, int32_t sweep);
 
+/*
+ * Bandwidth probe (measurement only): what this GPU's L2 sustains for the access patterns of the sparse sweep.
+ *   scratch        DEVICE memory, at least `bytes` long (a power of two >= 1 MiB is used: the largest that fits)
+ *   gather_gbs     HOST out: random 32-byte sector gathers (two 16-byte loads per lane pair, eight in flight per lane)
+ *                  from the buffer, GB/s of sectors delivered
+ *   stream_gbs     HOST out: grid-strided 16-byte streaming reads of the same buffer, GB/s
+ * Pick `bytes` = the state size of interest (config 5: 32 MiB, L2-resident).  Synchronises `stream`.
+ */
+ising_status ising_debug_probe_l2(void* scratch, size_t bytes, double* gather_gbs, double* stream_gbs, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -78,6 +78,8 @@ def lib():
     L.ising_problem_info.argtypes = [_vp, _i32, ctypes.POINTER(_i64)]
     L.ising_debug_phase_timing.restype = _i32
     L.ising_debug_phase_timing.argtypes = [_vp, _vp, _i32]
+    L.ising_debug_probe_l2.restype = _i32
+    L.ising_debug_probe_l2.argtypes = [_vp, _sz, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), _vp]
     L.ising_free.restype = _i32
     L.ising_free.argtypes = [_vp]
     _lib = L
@@ -275,6 +277,16 @@ def ising_current_state(p: Problem, n_replicas: int, out=None, stream=None):
         out = torch.zeros((n_replicas, p.n), dtype=torch.int8, device="cuda")
     _check(lib().ising_current_state(p.handle, _ptr(out), n_replicas, _stream(stream)), "ising_current_state")
     return out
+
+
+def probe_l2(nbytes: int = 32 << 20, stream=None):
+    """include/ising_debug.h: (random 32-byte sector gather GB/s, streaming read GB/s) of an nbytes buffer on this GPU."""
+    t = _torch()
+    buf = t.zeros(nbytes, dtype=t.uint8, device="cuda")
+    g, s_ = ctypes.c_double(0), ctypes.c_double(0)
+    _check(lib().ising_debug_probe_l2(buf.data_ptr(), nbytes, ctypes.byref(g), ctypes.byref(s_), _stream(stream)),
+           "ising_debug_probe_l2")
+    return float(g.value), float(s_.value)
 
 
 def ising_free(p: Problem):

@@ -18,6 +18,7 @@
 #include "builder.cuh"
 #include "common.cuh"
 #include "dense_tcgen05.cuh"
+#include "probe.cuh"
 #include "sparse_sweep.cuh"
 
 using namespace ising;
@@ -1016,10 +1017,12 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
     if (use_dense) {
         DenseAnnealArgs a{};
         a.tie_rule = tie_rule; a.n_replicas = n_replicas; a.first_replica = first_replica; a.keys = keys;
-        a.thresholds = thresholds; a.n_sweeps = n_sweeps; a.sweep_offset = sweep_offset; a.cut_trace = cut_trace;
+        a.thresholds = p->thr_host.data(); a.n_sweeps = n_sweeps; a.sweep_offset = sweep_offset; a.cut_trace = cut_trace;
         a.W = p->W;
         a.import_from_sparse = !(p->state_in_dense && init_mode == ISING_INIT_CONTINUE);
         a.sparse_state = p->state[p->cur]; a.perm = p->perm; a.io_stage = p->io_stage;
+        a.thr_dev = p->sm.thr; a.thr_host = p->thr_host.data(); a.thr_cap = kThrCap;
+        a.timing = p->timing; a.timing_pass = p->timing_sweep;
         ising_status s = dense_anneal(p->dense, a, st, &p->launches);
         if (s) return s;
         p->state_in_dense = true;
@@ -1371,6 +1374,45 @@ ising_status ising_debug_phase_timing(ising_problem* p, uint64_t* stamps, int32_
     if (sweep < 0 || (stamps && !is_device_ptr(stamps))) return ISING_ERR_BAD_SHAPE;
     p->timing = (unsigned long long*)stamps;
     p->timing_sweep = (uint32_t)sweep;
+    return ISING_OK;
+}
+
+ising_status ising_debug_probe_l2(void* scratch, size_t bytes, double* gather_gbs, double* stream_gbs, void* stream) {
+    if (!scratch || !gather_gbs || !stream_gbs) return ISING_ERR_NULL_ARG;
+    if (bytes < (1u << 20) || !is_device_ptr(scratch)) return ISING_ERR_BAD_SHAPE;
+    if (ising_status s = check_device()) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    size_t use = 1u << 20;
+    while (use * 2 <= bytes && use < ((size_t)1 << 31)) use *= 2;
+    int sm = 148;
+    {
+        int dev = 0;
+        CK(cudaGetDevice(&dev));
+        CK(cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev));
+    }
+    uint32_t* sink = reinterpret_cast<uint32_t*>(scratch);   // (never written: the kernels' results cannot match the magic value)
+    const uint32_t sectors_mask = (uint32_t)(use / 32) - 1u, per_pair = 2048, blocks = (unsigned)sm * 4, passes = 16;
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    float ms_g = 0, ms_s = 0;
+    for (int rep = 0; rep < 3; ++rep) {   // the last of three runs counts (the first brings the buffer into L2)
+        CK(cudaEventRecord(e0, st));
+        k_probe_gather<<<blocks, 512, 0, st>>>((const uint4*)scratch, sectors_mask, per_pair, sink);
+        CK(cudaEventRecord(e1, st));
+        CK(cudaEventSynchronize(e1));
+        CK(cudaEventElapsedTime(&ms_g, e0, e1));
+        CK(cudaEventRecord(e0, st));
+        k_probe_stream<<<blocks, 512, 0, st>>>((const uint4*)scratch, (uint32_t)(use / 16), passes, sink);
+        CK(cudaEventRecord(e1, st));
+        CK(cudaEventSynchronize(e1));
+        CK(cudaEventElapsedTime(&ms_s, e0, e1));
+    }
+    CK(cudaEventDestroy(e0));
+    CK(cudaEventDestroy(e1));
+    CK(cudaGetLastError());
+    *gather_gbs = (double)blocks * 256.0 * per_pair * 32.0 / (ms_g * 1e-3) / 1e9;
+    *stream_gbs = (double)use * passes / (ms_s * 1e-3) / 1e9;
     return ISING_OK;
 }
 
