@@ -158,10 +158,13 @@ def workload_roofline(wl, us_per_sweep, engine, hbm_peak, l2, int8):
         b_l2 = (nnz * 32 + 2 * n * 32) * ((R + 31) // 32)
         t_roof = max(b_hbm * ((R + 31) // 32) / (hbm_peak * 1e9), b_l2 / (l2["gather_gbs"] * 1e9)) if l2.get("gather_gbs") else None
         out = {"bound": "hbm", "achieved": alg / t / 1e9, "unit": "GB/s", "peak": hbm_peak, "frac": alg / t / 1e9 / hbm_peak,
-               "l2": {"gather_peak_gbs": l2.get("gather_gbs"), "stream_peak_gbs": l2.get("stream_gbs"),
+               "l2": {"gather_peak_gbs": l2.get("gather_gbs"), "gather_peak_16B_lane_pair_gbs": l2.get("gather_16B_lane_pair_gbs"),
+                      "stream_peak_gbs": l2.get("stream_gbs"),
                       "gather_bytes_per_sweep": b_l2, "hbm_stream_bytes_per_sweep": b_hbm * ((R + 31) // 32),
                       "t_roof_us": None if t_roof is None else t_roof * 1e6,
                       "frac_of_t_roof": None if t_roof is None else t_roof / t,
+                      "frac_of_own_shape_ceiling": None if not l2.get("gather_16B_lane_pair_gbs") else
+                      (b_l2 / (l2["gather_16B_lane_pair_gbs"] * 1e9)) / t,
                       "note": "T_roof = max(B_hbm / BW_hbm, B_l2 / BW_l2) (SURVEY 8(d)): the gathers are L2 hits, so this -- not "
                               "the HBM-normalised frac the contract asks for -- says how far the sweep is from the memory system's limit"}}
         return out
@@ -263,6 +266,26 @@ def oracle_calibrate(wl, threads: int, target_s: float):
     return reps, sweeps
 
 
+def oracle_matches_trace(wl, trace, first_replica, replicas, sweeps, threads):
+    """The timed run's cut trace of a few replicas over the first sweeps against the oracle (outside the timed region)."""
+    from oracle import ising_oracle as O
+    ok = True
+    tr = trace[:sweeps].cpu().numpy()
+    for r in replicas:
+        o = O.anneal_workload(wl, n_replicas=1, first_replica=first_replica + r, thr=wl.thr[:sweeps], n_threads=1)
+        ok = ok and bool((o["trace"][:, 0] == tr[:, r]).all())
+    return ok
+
+
+def oracle_energy_seconds(wl, states=4):
+    """Seconds the oracle's from-scratch energy takes per state (it is evaluated after every sweep of every replica)."""
+    from oracle import ising_oracle as O
+    spins = W.random_spins(7, states, wl.n)
+    t0 = time.perf_counter()
+    O.energy_cut(wl.n, wl.row_ptr, wl.col, wl.w, spins)
+    return (time.perf_counter() - t0) / states
+
+
 def run_reference(args, wl, rank):
     if rank != 0:
         return 0
@@ -319,8 +342,8 @@ def time_workload(P, torch, wl, first_replica, steps, warmup, flush_buf, dist=No
         torch.cuda.synchronize()
         times.append(e0.elapsed_time(e1) * 1e-3)
         best.append(P.ising_best_state(p, -1, want_spins=False)[1])
-    launches = p.launches - launches0 - steps * 0
-    return p, times, best, launches
+    launches = p.launches - launches0
+    return p, times, best, launches, trace
 
 
 def time_e2e(P, torch, wl, first_replica, steps, warmup, dist=None):
@@ -403,8 +426,8 @@ def main():
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
-    p, times, best, launches = time_workload(P, torch, wl, first_replica, args.steps, args.warmup, flush_buf,
-                                             dist, None)
+    p, times, best, launches, trace = time_workload(P, torch, wl, first_replica, args.steps, args.warmup, flush_buf,
+                                                    dist, None)
     clocks = sampler.stop() if rank == 0 else None
     t_total = max_over_ranks(sum(times), dist, "cuda")
     deterministic = len(set(best)) == 1
@@ -413,49 +436,60 @@ def main():
     edge_visits = wl.nnz * R * M * args.steps * world
     value = spin_updates / t_total
 
-    # roofline of the dominant kernel: k_anneal_gs, the persistent Gauss-Seidel kernel -- ONE launch
-    # per ising_anneal call (per <= 1024 replicas) runs all M sweeps x colour phases.  Its duration is
-    # taken as the CUDA-event time of the whole ising_anneal call (which also holds the spin init,
-    # the initial-energy pass and two tiny kernels), so `achieved` is a lower bound for the kernel.
+    # roofline of the dominant kernel.  Config 5: k_anneal_gs, the persistent Gauss-Seidel kernel -- ONE launch
+    # per ising_anneal call runs all M sweeps.  Its duration is taken as the CUDA-event time of the whole ising_anneal call
+    # (which also holds the spin init, the initial-energy pass and two tiny kernels: 0.2 % of the call), so `achieved` is a
+    # lower bound for the kernel.
+    from paper_1807_10750_b200 import binding as B
     peak, peak_src = measured_peaks()
+    l2 = {}
+    try:
+        g_gbs, g16_gbs, s_gbs = B.probe_l2(32 << 20)
+        l2 = {"gather_gbs": g_gbs, "gather_16B_lane_pair_gbs": g16_gbs, "stream_gbs": s_gbs,
+              "how": "ising_debug_probe_l2 on a 32 MiB buffer: random 32-byte sector gathers, the better of 4-byte lanes (4 sectors "
+                     "per warp instruction) and the sweep's 16-byte lane pairs (16 sectors per instruction), eight loads in flight "
+                     "per lane / grid-strided 16-byte streaming reads"}
+    except Exception as ex:
+        l2 = {"error": repr(ex)}
+    int8 = {}
+    int8["derived"], int8["derived_source"] = derived_int8_peak()
+    int8["probe"] = probe_int8_peak(torch) if rank == 0 else {}
+    if int8["probe"].get("sustained_tops"):
+        int8["peak"], int8["peak_source"] = int8["probe"]["sustained_tops"], "measured: " + int8["probe"]["how"]
+    else:
+        int8["peak"], int8["peak_source"] = int8["derived"], int8["derived_source"]
+    engine_names = {0: "k_sweep (one launch per colour phase)", 1: "k_anneal_gs (persistent cooperative grid)",
+                    2: "k_anneal_gs<cluster> (one thread-block cluster per replica tile)",
+                    3: "k_anneal_gs (persistent cooperative grid + shared-memory tail chain)",
+                    4: "k_anneal_small (whole graph in one CTA per four replicas)"}
+
+    def kernel_of(pp, w_):
+        if pp.has_dense_engine and w_.mode == "jacobi":
+            return "dense", "k_dense_anneal (tcgen05.mma kind::i8, all sweeps in one cooperative launch)"
+        if w_.mode == "jacobi":
+            return "sparse-jacobi", "k_sweep<Jacobi> (one launch per sweep)"
+        return "gs", engine_names.get(pp.engine, "?")
+
     n_phase = max(1, wl.n_colours) if wl.mode == "gs" else 1
-    persistent = wl.mode == "gs"
-    launches_per_step = 1 if persistent else M
-    avg_launch_s = sum(times) / (args.steps * launches_per_step)
-    bytes_per_launch = algorithmic_bytes_per_sweep(wl.n, wl.nnz, R) * (M if persistent else 1)
-    achieved = bytes_per_launch / avg_launch_s / 1e9
-    traffic = None
+    us_per_sweep = 1e6 * sum(times) / (args.steps * M)
+    eng, kname = kernel_of(p, wl)
+    roofline = workload_roofline(wl, us_per_sweep, eng, peak, l2, int8)
+    avg_call_s = sum(times) / args.steps
+    roofline.update({"kernel": kname, "us_per_sweep": us_per_sweep, "avg_call_us": avg_call_s * 1e6,
+                     "bytes_per_launch": algorithmic_bytes_per_sweep(wl.n, wl.nnz, R) * M,
+                     "peak_source": roofline.get("peak_source", peak_src), "traffic": None,
+                     "note": "algorithmic bytes = (nnz*37 + n*68) per 32-replica tile per sweep (SURVEY 8(d)) x sweeps per launch; "
+                             "avg_call_us is the CUDA-event time of the whole ising_anneal call, a lower bound for the kernel; "
+                             "traffic = ncu dram bytes per sweep of this build (profiles/traffic.json) x sweeps per launch"})
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         try:
             tj = json.load(open(tpath)).get(wl.name)
             if tj:
-                traffic = tj["dram_bytes_per_sweep"] * (M if persistent else 1)
+                roofline["traffic"] = tj["dram_bytes_per_sweep"] * M
+                roofline["traffic_source"] = tj.get("source")
         except Exception:
-            traffic = None
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic,
-                "kernel": "k_anneal_gs (persistent cooperative kernel: %d sweeps x %d colour phases per launch)" % (
-                    M, n_phase) if persistent else "k_sweep<Jacobi> (one launch per sweep)",
-                "bytes_per_launch": bytes_per_launch, "avg_launch_us": avg_launch_s * 1e6,
-                "us_per_sweep": 1e6 * sum(times) / (args.steps * M),
-                "peak_source": peak_src,
-                "note": "algorithmic bytes = (nnz*37 + n*68) per 32-replica tile per sweep (SURVEY 8(d)) x sweeps per "
-                        "launch; the 32 B gathered per edge come from L2 (spin state is L2-resident), so frac can "
-                        "exceed what HBM alone would allow; traffic = ncu dram bytes per sweep (profiles/traffic.json) "
-                        "x sweeps per launch"}
-
-    if p.has_dense_engine and wl.mode == "jacobi":
-        # fully connected instance: the local fields are an int8 contraction on tcgen05 (a8)
-        tpeak, tsrc = measured_int8_peak()
-        ops_per_launch = 2.0 * wl.n * wl.n * R
-        achieved = ops_per_launch / avg_launch_s / 1e12
-        roofline = {"bound": "tensor", "achieved": achieved, "peak": tpeak, "unit": "TFLOP/s", "frac": achieved / tpeak,
-                    "traffic": None, "kernel": "k_dense_sweep (tcgen05.mma kind::i8, one launch per Jacobi sweep)",
-                    "ops_per_launch": ops_per_launch, "avg_launch_us": avg_launch_s * 1e6,
-                    "us_per_sweep": 1e6 * sum(times) / (args.steps * M), "peak_source": tsrc,
-                    "note": "int8 multiply-adds counted as 2 ops (unit reads TOP/s); algorithmic ops = 2 n^2 R per sweep; "
-                            "duration = whole ising_anneal time / sweeps (includes the per-sweep cut/best kernel)"}
+            pass
 
     e2e = None
     if not args.no_e2e:
@@ -467,28 +501,54 @@ def main():
 
     extra = {}
     cpu_baseline = None
+    check = {"deterministic_across_steps": deterministic, "best_cut": best[-1]}
     if rank == 0 and world == 1 and not args.no_extra:
-        for name in ("cfg1", "cfg2", "cfg3", "cfg4"):
+        for name in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5"):
             if name == args.workload:
                 continue
             try:
                 w2 = make_workload(name)
-                _, t2, b2, l2 = time_workload(P, torch, w2, 0, 2, 1, flush_buf)
+                p2, t2, b2, l2n, tr2 = time_workload(P, torch, w2, 0, 2, 3, flush_buf)
                 tt = sum(t2)
+                eng2, k2 = kernel_of(p2, w2)
+                us2 = 1e6 * tt / (2 * w2.n_sweeps)
+                m2 = min(w2.n_sweeps, 30)
                 extra[name] = {"workload": w2.name, "n": w2.n, "nnz": w2.nnz, "replicas": w2.n_replicas,
-                               "sweeps": w2.n_sweeps, "mode": w2.mode, "ms_per_step": 1e3 * tt / 2,
+                               "sweeps": w2.n_sweeps, "colours": w2.n_colours, "mode": w2.mode, "ms_per_step": 1e3 * tt / 2,
+                               "us_per_sweep": us2,
                                "spin_updates_per_s": w2.n * w2.n_replicas * w2.n_sweeps * 2 / tt,
                                "edge_visits_per_s": w2.nnz * w2.n_replicas * w2.n_sweeps * 2 / tt,
-                               "best_cut": b2[-1], "gpu_launches": l2}
+                               "best_cut": b2[-1], "gpu_launches": l2n, "kernel": k2,
+                               "roofline": workload_roofline(w2, us2, eng2, peak, l2, int8),
+                               "matches_oracle": oracle_matches_trace(w2, tr2, 0, sorted({0, w2.n_replicas - 1}), m2, 1),
+                               "matches_oracle_sample": "cut trace of replicas 0 and R-1, first %d sweeps of the timed run" % m2}
+                p2.free()
             except Exception as ex:  # keep the headline line alive
                 extra[name] = {"error": repr(ex)}
+        # the timed run of the headline workload against the oracle (outside the timed region)
+        mo = min(M, 24 if wl.n >= 200_000 else 200)
+        check["matches_oracle"] = oracle_matches_trace(wl, trace, first_replica, sorted({0, R - 1}), mo, 1)
+        check["matches_oracle_sample"] = "cut trace of replicas 0 and R-1, first %d sweeps of the last timed step" % mo
+        # the oracle, as it stands, on this box's host cores: all cores (threads over replicas) and one thread;
+        # it evaluates the energy from the definition after every sweep, timed separately
         cores = os.cpu_count() or 1
         threads = max(1, min(cores, wl.n_replicas))
-        reps, sweeps = oracle_calibrate(wl, threads, target_s=15.0)
-        t = oracle_sample(wl, reps, sweeps, threads)
-        cpu_baseline = {"value": wl.n * reps * sweeps / t, "unit": UNIT, "cores": threads, "kind": "oracle",
+        reps, sweeps = oracle_calibrate(wl, threads, target_s=12.0)
+        t_all = oracle_sample(wl, reps, sweeps, threads)
+        s1 = max(1, sweeps // 2)
+        t_one = oracle_sample(wl, 1, s1, 1)
+        t_e = oracle_energy_seconds(wl)
+        cpu_baseline = {"value": wl.n * reps * sweeps / t_all, "unit": UNIT, "cores": threads, "nproc": cores, "kind": "oracle",
                         "sample": "%d replicas x first %d sweeps of %s (%.1f s wall, %d threads over replicas)" % (
-                            reps, sweeps, wl.name, t, threads)}
+                            reps, sweeps, wl.name, t_all, threads),
+                        "single_thread": {"value": wl.n * s1 / t_one, "unit": UNIT,
+                                          "sample": "1 replica x first %d sweeps (%.1f s wall, 1 thread)" % (s1, t_one)},
+                        "sweep_plus_energy_s_per_replica_sweep": t_one / s1,
+                        "energy_s_per_replica_sweep": t_e,
+                        "sweep_only_s_per_replica_sweep": max(0.0, t_one / s1 - t_e),
+                        "note": "the oracle recomputes the energy from the definition after every sweep (it is a correctness "
+                                "reference, not a tuned CPU baseline): sweep-only = measured sweep+energy minus the separately "
+                                "timed from-scratch energy"}
 
     if rank == 0:
         line = {
@@ -499,11 +559,12 @@ def main():
             "config": {"workload": wl.name, "n": wl.n, "nnz": wl.nnz, "replicas_per_gpu": R, "sweeps": M,
                        "colours": wl.n_colours, "mode": wl.mode, "parallelism": "replicas-only x%d" % world,
                        "l2": "256 MiB buffer rewritten between timed steps (L2 flush); working set 148 MB > L2",
-                       "step": "one ising_anneal call: init + %d sweeps x %d colour phases + per-sweep cut/trace/best capture" % (
+                       "engine": kname,
+                       "step": "one ising_anneal call: init + %d sweeps x %d colour classes + per-sweep cut/trace/best capture" % (
                            M, n_phase)},
             "edge_visits_per_s": edge_visits / t_total,
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches,
-            "clocks": clocks, "check": {"deterministic_across_steps": deterministic, "best_cut": best[-1]},
+            "clocks": clocks, "check": check, "peaks": {"hbm_gbs": peak, "l2": l2, "int8": int8},
             "workloads": extra,
         }
         print(json.dumps(line))

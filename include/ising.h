@@ -60,7 +60,8 @@ typedef int32_t ising_status;
 enum {
     ISING_OK = 0,
     ISING_ERR_NULL_ARG = 1,
-    ISING_ERR_BAD_SHAPE = 2,          /* n<=0, nnz<0, row_ptr not monotone / wrong ends, col out of range, bad enum */
+    ISING_ERR_BAD_SHAPE = 2,          /* n<=0, nnz<0, row_ptr not monotone / wrong ends, col out of range, bad enum,
+                                         workspace not 256-byte aligned device memory */
     ISING_ERR_UNSORTED_OR_DUP = 3,    /* a row's columns are not strictly ascending */
     ISING_ERR_SELF_LOOP = 4,
     ISING_ERR_ASYMMETRIC = 5,         /* (i,j) present without (j,i), or w(i,j) != w(j,i) */
@@ -114,7 +115,8 @@ ising_status ising_workspace_bytes(int32_t n, int64_t nnz, int32_t wtype, int32_
  *   colour       int32 [n] proper colouring with values in [0, n_colours), host|device;
  *                NULL (and n_colours = 0) -> the problem supports Jacobi / racy modes only
  *   max_replicas largest n_replicas any later call will pass (1 .. 65536)
- *   workspace    DEVICE memory, 256-byte aligned, workspace_bytes long, borrowed until ising_free
+ *   workspace    DEVICE memory, 256-byte aligned (else ISING_ERR_BAD_SHAPE), workspace_bytes long (else
+ *                ISING_ERR_WORKSPACE_TOO_SMALL), borrowed until ising_free
  *   flags        ISING_LOAD_*
  *   out          receives the handle (host object; free with ising_free)
  *

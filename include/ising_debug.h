@@ -24,12 +24,15 @@ ising_status ising_debug_phase_timing(ising_problem* p, uint64_t* stamps, int32_
 /*
  * Bandwidth probe (measurement only): what this GPU's L2 sustains for the access patterns of the sparse sweep.
  *   scratch        DEVICE memory, at least `bytes` long (a power of two >= 1 MiB is used: the largest that fits)
- *   gather_gbs     HOST out: random 32-byte sector gathers (two 16-byte loads per lane pair, eight in flight per lane)
- *                  from the buffer, GB/s of sectors delivered
+ *   gather_gbs     HOST out: random 32-byte sector gathers from the buffer, GB/s of sectors delivered: the better of two
+ *                  access shapes (two 16-byte loads per lane pair = 16 sectors per warp instruction, the sweep's shape;
+ *                  4-byte loads by eight lanes per sector = 4 sectors per instruction), eight loads in flight per lane
+ *   gather16_gbs   HOST out: the same for the 16-byte shape alone (what the sweep kernel's gathers can reach)
  *   stream_gbs     HOST out: grid-strided 16-byte streaming reads of the same buffer, GB/s
  * Pick `bytes` = the state size of interest (config 5: 32 MiB, L2-resident).  Synchronises `stream`.
  */
-ising_status ising_debug_probe_l2(void* scratch, size_t bytes, double* gather_gbs, double* stream_gbs, void* stream);
+ising_status ising_debug_probe_l2(void* scratch, size_t bytes, double* gather_gbs, double* gather16_gbs, double* stream_gbs,
+                                  void* stream);
 
 #ifdef __cplusplus
 }

@@ -79,7 +79,8 @@ def lib():
     L.ising_debug_phase_timing.restype = _i32
     L.ising_debug_phase_timing.argtypes = [_vp, _vp, _i32]
     L.ising_debug_probe_l2.restype = _i32
-    L.ising_debug_probe_l2.argtypes = [_vp, _sz, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), _vp]
+    L.ising_debug_probe_l2.argtypes = [_vp, _sz, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                                       ctypes.POINTER(ctypes.c_double), _vp]
     L.ising_free.restype = _i32
     L.ising_free.argtypes = [_vp]
     _lib = L
@@ -280,13 +281,14 @@ def ising_current_state(p: Problem, n_replicas: int, out=None, stream=None):
 
 
 def probe_l2(nbytes: int = 32 << 20, stream=None):
-    """include/ising_debug.h: (random 32-byte sector gather GB/s, streaming read GB/s) of an nbytes buffer on this GPU."""
+    """include/ising_debug.h: (random 32-byte sector gather GB/s with the best access shape, the same with the sweep's
+    16-byte lane-pair shape, streaming read GB/s) of an nbytes buffer on this GPU."""
     t = _torch()
     buf = t.zeros(nbytes, dtype=t.uint8, device="cuda")
-    g, s_ = ctypes.c_double(0), ctypes.c_double(0)
-    _check(lib().ising_debug_probe_l2(buf.data_ptr(), nbytes, ctypes.byref(g), ctypes.byref(s_), _stream(stream)),
-           "ising_debug_probe_l2")
-    return float(g.value), float(s_.value)
+    g, g16, s_ = ctypes.c_double(0), ctypes.c_double(0), ctypes.c_double(0)
+    _check(lib().ising_debug_probe_l2(buf.data_ptr(), nbytes, ctypes.byref(g), ctypes.byref(g16), ctypes.byref(s_),
+                                      _stream(stream)), "ising_debug_probe_l2")
+    return float(g.value), float(g16.value), float(s_.value)
 
 
 def ising_free(p: Problem):

@@ -444,10 +444,13 @@ ising_status ising_workspace_bytes(int32_t n, int64_t nnz, int32_t wtype, int32_
     return ISING_OK;
 }
 
-ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
-                            const void* weights, int32_t wtype, const int32_t* colour, int32_t n_colours,
-                            int32_t max_replicas, void* workspace, size_t workspace_bytes, int32_t flags,
-                            void* stream, ising_problem** out) {
+}  // extern "C"
+
+namespace {
+ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
+                           const void* weights, int32_t wtype, const int32_t* colour, int32_t n_colours,
+                           int32_t max_replicas, void* workspace, size_t workspace_bytes, int32_t flags,
+                           void* stream, ising_problem** out) {
     if (!out || !row_ptr || !workspace || (nnz > 0 && (!col_idx || !weights))) return ISING_ERR_NULL_ARG;
     if (n <= 0 || nnz < 0 || n_colours < 0 || (wtype != ISING_W_INT8 && wtype != ISING_W_INT32))
         return ISING_ERR_BAD_SHAPE;
@@ -455,7 +458,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     if (max_replicas < 1 || max_replicas > 65536) return ISING_ERR_TOO_MANY_REPLICAS;
     if (ising_status s = check_device()) return s;
     if ((reinterpret_cast<uintptr_t>(workspace) & (kAlign - 1)) != 0 || !is_device_ptr(workspace))
-        return ISING_ERR_WORKSPACE_TOO_SMALL;
+        return ISING_ERR_BAD_SHAPE;   // not 256-byte aligned device memory
     cudaStream_t st = (cudaStream_t)stream;
 
     Bump ws{(uint8_t*)workspace, workspace_bytes, 0, false};
@@ -501,7 +504,7 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     if (plan_early) {
         const int64_t* rp = row_ptr;
         bool bad = rp[0] != 0 || rp[n] != nnz;
-        for (int32_t i = 0; i < n && !bad; ++i) bad = rp[i + 1] < rp[i] || rp[i] < 0 || rp[i + 1] > nnz;
+        for (int32_t i = 0; i < n && !bad; ++i) bad = rp[i + 1] < rp[i] || rp[i] < 0 || rp[i + 1] > nnz || rp[i + 1] - rp[i] > (int64_t)n - 1;
         if (bad) return ISING_ERR_BAD_SHAPE;
         if (colour)
             for (int32_t i = 0; i < n; ++i)
@@ -940,6 +943,27 @@ ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, cons
     return ISING_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
+ising_status ising_load_csr(int32_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
+                            const void* weights, int32_t wtype, const int32_t* colour, int32_t n_colours,
+                            int32_t max_replicas, void* workspace, size_t workspace_bytes, int32_t flags,
+                            void* stream, ising_problem** out) {
+    ising_status s;
+    try {
+        s = load_csr_impl(n, nnz, row_ptr, col_idx, weights, wtype, colour, n_colours, max_replicas, workspace,
+                          workspace_bytes, flags, stream, out);
+    } catch (...) {   // std::bad_alloc of the host-side planning: no exception crosses the C ABI
+        s = ISING_ERR_CUDA;
+    }
+    // on error, copies enqueued from the caller's (possibly pinned) arrays have finished before the call returns:
+    // the inputs may be freed on return either way
+    if (s != ISING_OK) { (void)cudaStreamSynchronize((cudaStream_t)stream); (void)cudaGetLastError(); }
+    return s;
+}
+
 ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int32_t n_replicas,
                           int32_t first_replica, uint64_t seed, const uint32_t* thresholds, int32_t n_sweeps,
                           int32_t sweep_offset, int32_t init_mode, const int8_t* init_spins, int64_t* cut_trace,
@@ -1080,7 +1104,7 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
         p->parity = 0;
     } else if (mode == ISING_MODE_GS && !p->wide && p->cooperative) {
         // the hot path: initial energy from the definition (evaluation pass), then ONE persistent
-        // cooperative launch per batch of <= 1024 replicas and chunk of <= kThrCap sweeps
+        // cooperative launch per batch of <= kMaxPersistReplicas (512) replicas and chunk of <= kThrCap sweeps
         CK(cudaMemsetAsync(p->sm.accum_eval, 0, small_bytes, st));
         SweepParams ev = sp;
         ev.src = p->state[p->cur]; ev.dst = p->state[p->cur]; ev.accum = p->sm.accum_eval;
@@ -1285,8 +1309,14 @@ ising_status ising_best_state(ising_problem* p, int32_t replica, int8_t* spins_o
     if (replica < -1 || replica >= p->last_R) return ISING_ERR_BAD_SHAPE;
     cudaStream_t st = (cudaStream_t)stream;
     const int R = p->last_R;
-    std::vector<long long> bc(R);
-    std::vector<int32_t> bs(R);
+    std::vector<long long> bc;
+    std::vector<int32_t> bs;
+    try {
+        bc.resize((size_t)R);
+        bs.resize((size_t)R);
+    } catch (...) {
+        return ISING_ERR_CUDA;
+    }
     if (p->state_in_dense) {
         if (ising_status s = dense_best_arrays(p->dense, bc.data(), bs.data(), R, st)) return s;
     } else {
@@ -1377,8 +1407,9 @@ ising_status ising_debug_phase_timing(ising_problem* p, uint64_t* stamps, int32_
     return ISING_OK;
 }
 
-ising_status ising_debug_probe_l2(void* scratch, size_t bytes, double* gather_gbs, double* stream_gbs, void* stream) {
-    if (!scratch || !gather_gbs || !stream_gbs) return ISING_ERR_NULL_ARG;
+ising_status ising_debug_probe_l2(void* scratch, size_t bytes, double* gather_gbs, double* gather16_gbs, double* stream_gbs,
+                                  void* stream) {
+    if (!scratch || !gather_gbs || !gather16_gbs || !stream_gbs) return ISING_ERR_NULL_ARG;
     if (bytes < (1u << 20) || !is_device_ptr(scratch)) return ISING_ERR_BAD_SHAPE;
     if (ising_status s = check_device()) return s;
     cudaStream_t st = (cudaStream_t)stream;
@@ -1395,13 +1426,20 @@ ising_status ising_debug_probe_l2(void* scratch, size_t bytes, double* gather_gb
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0));
     CK(cudaEventCreate(&e1));
-    float ms_g = 0, ms_s = 0;
+    float ms_g = 0, ms_s = 0, ms_g4 = 0;
     for (int rep = 0; rep < 3; ++rep) {   // the last of three runs counts (the first brings the buffer into L2)
         CK(cudaEventRecord(e0, st));
         k_probe_gather<<<blocks, 512, 0, st>>>((const uint4*)scratch, sectors_mask, per_pair, sink);
         CK(cudaEventRecord(e1, st));
         CK(cudaEventSynchronize(e1));
         CK(cudaEventElapsedTime(&ms_g, e0, e1));
+        float ms_4 = 0;
+        CK(cudaEventRecord(e0, st));
+        k_probe_gather4<<<blocks, 512, 0, st>>>((const uint32_t*)scratch, sectors_mask, per_pair, sink);
+        CK(cudaEventRecord(e1, st));
+        CK(cudaEventSynchronize(e1));
+        CK(cudaEventElapsedTime(&ms_4, e0, e1));
+        ms_g4 = ms_4;
         CK(cudaEventRecord(e0, st));
         k_probe_stream<<<blocks, 512, 0, st>>>((const uint4*)scratch, (uint32_t)(use / 16), passes, sink);
         CK(cudaEventRecord(e1, st));
@@ -1411,7 +1449,9 @@ ising_status ising_debug_probe_l2(void* scratch, size_t bytes, double* gather_gb
     CK(cudaEventDestroy(e0));
     CK(cudaEventDestroy(e1));
     CK(cudaGetLastError());
-    *gather_gbs = (double)blocks * 256.0 * per_pair * 32.0 / (ms_g * 1e-3) / 1e9;
+    *gather16_gbs = (double)blocks * 256.0 * per_pair * 32.0 / (ms_g * 1e-3) / 1e9;   // 16-byte lanes: 256 pairs per CTA
+    const double g4 = (double)blocks * 64.0 * per_pair * 32.0 / (ms_g4 * 1e-3) / 1e9;      // 4-byte lanes: 64 groups per CTA
+    *gather_gbs = std::max(*gather16_gbs, g4);
     *stream_gbs = (double)use * passes / (ms_s * 1e-3) / 1e9;
     return ISING_OK;
 }

@@ -68,3 +68,58 @@ def test_config3_full_schedule_on_a_replica_subset():
     g = gpu_anneal(wl, n_replicas=16, first_replica=120)
     o = oracle_anneal(wl, n_replicas=16, first_replica=120, n_threads=16)
     assert_same(g, o)
+
+
+def _oracle_replica_groups(wl, groups, thr, n_threads):
+    """Oracle runs of contiguous replica ranges [(first, count), ...] -> {replica: (trace column, final spins, best cut, best sweep)}."""
+    out = {}
+    for first, count in groups:
+        o = oracle_anneal(wl, thr=thr, n_replicas=count, first_replica=first, n_threads=min(n_threads, count))
+        for k in range(count):
+            out[first + k] = (o["trace"][:, k], o["final"][k], int(o["best_cut"][k]), int(o["best_sweep"][k]))
+    return out
+
+
+def test_config5_bench_configuration_full_schedule_sampled_replicas(cfg5):
+    """SURVEY 8(c) sampling plan: the run bench.py times (all 32 replicas x all 500 sweeps, one ising_anneal call) compared
+    with the oracle on replicas {0, 3, 4, 31}: every cut of the trace, the final spins, best cut and sweep."""
+    import concurrent.futures as cf
+    import torch
+    wl = cfg5
+    p = P.load_workload(wl)
+    assert p.engine == P.ENGINE_GRID_TAIL_CHAIN
+    trace = P.anneal_workload(p, wl, cut_trace=True)
+    final = P.ising_current_state(p, wl.n_replicas)
+    torch.cuda.synchronize()
+    trace, final = trace.cpu().numpy(), final.cpu().numpy()
+    reps = (0, 3, 4, 31)
+    with cf.ThreadPoolExecutor(len(reps)) as ex:     # four single-thread oracle runs side by side (ctypes drops the GIL)
+        res = list(ex.map(lambda r: _oracle_replica_groups(wl, [(r, 1)], wl.thr, 1)[r], reps))
+    for r, (tr, fin, bc, bs) in zip(reps, res):
+        np.testing.assert_array_equal(trace[:, r], tr)
+        np.testing.assert_array_equal(final[r], fin)
+        s, cut, sweep, rep = P.ising_best_state(p, r, want_spins=False)
+        assert (cut, sweep) == (bc, bs)
+
+
+def test_config4_bench_configuration_full_schedule_sampled_replicas():
+    """K_4096 x 1024 replicas x 1000 Jacobi sweeps on the tcgen05 engine exactly as bench.py runs it (one cooperative launch):
+    every replica for the first 3 sweeps, and replicas {0-7, 127, 128, 255, 256, 511, 512, 1016-1023} (tile and Philox-group
+    edges) for the complete schedule (SURVEY 8(c) plan)."""
+    import torch
+    wl = W.config4()
+    g3 = gpu_anneal(wl, thr=wl.thr[:3], want_best_spins=False)
+    assert g3["problem"].has_dense_engine
+    assert_same(g3, oracle_anneal(wl, thr=wl.thr[:3], n_threads=16), best_spins=False)
+    p = g3["problem"]
+    trace = P.anneal_workload(p, wl, cut_trace=True)
+    final = P.ising_current_state(p, wl.n_replicas)
+    torch.cuda.synchronize()
+    trace, final = trace.cpu().numpy(), final.cpu().numpy()
+    groups = [(0, 8), (127, 2), (255, 2), (511, 2), (1016, 8)]
+    res = _oracle_replica_groups(wl, groups, wl.thr, 16)
+    for r, (tr, fin, bc, bs) in res.items():
+        np.testing.assert_array_equal(trace[:, r], tr)
+        np.testing.assert_array_equal(final[r], fin)
+        s, cut, sweep, rep = P.ising_best_state(p, r, want_spins=(r in (0, 1023)))
+        assert (cut, sweep) == (bc, bs)
