@@ -389,6 +389,7 @@ def main():
     ap.add_argument("--workload", default="cfg5")
     ap.add_argument("--no-extra", action="store_true", help="skip the other four configs and cpu_baseline")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-probes", action="store_true", help="skip the L2 / int8 peak probes (profiling runs: keeps the launch list short)")
     ap.add_argument("--sweeps", type=int, default=0, help="truncate the schedule to its first SWEEPS sweeps "
                     "(profiling runs only; the default 0 keeps the workload's full schedule)")
     args = ap.parse_args()
@@ -444,6 +445,8 @@ def main():
     peak, peak_src = measured_peaks()
     l2 = {}
     try:
+        if args.no_probes:
+            raise RuntimeError("skipped (--no-probes)")
         g_gbs, g16_gbs, s_gbs = B.probe_l2(32 << 20)
         l2 = {"gather_gbs": g_gbs, "gather_16B_lane_pair_gbs": g16_gbs, "stream_gbs": s_gbs,
               "how": "ising_debug_probe_l2 on a 32 MiB buffer: random 32-byte sector gathers, the better of 4-byte lanes (4 sectors "
@@ -453,7 +456,7 @@ def main():
         l2 = {"error": repr(ex)}
     int8 = {}
     int8["derived"], int8["derived_source"] = derived_int8_peak()
-    int8["probe"] = probe_int8_peak(torch) if rank == 0 else {}
+    int8["probe"] = probe_int8_peak(torch) if rank == 0 and not args.no_probes else {}
     if int8["probe"].get("sustained_tops"):
         int8["peak"], int8["peak_source"] = int8["probe"]["sustained_tops"], "measured: " + int8["probe"]["how"]
     else:
