@@ -90,7 +90,8 @@ enum {
     ISING_LOAD_NO_DENSE = 1,      /* never build the dense tcgen05 engine, even for a complete graph */
     /* Gauss-Seidel engine selection (results never depend on it; the default picks the fastest that applies):       */
     ISING_LOAD_NO_SMALL = 2,      /* do not run a small graph wholly inside one CTA per four replicas (shared memory)   */
-    ISING_LOAD_NO_CLUSTER = 4,    /* do not run a small graph on one thread-block cluster per replica tile              */
+    ISING_LOAD_NO_CLUSTER = 4,    /* no thread-block clusters: neither one per replica tile, nor pairs of CTAs sharing   */
+                                  /* the rows of a small graph in the shared-memory engine                               */
     ISING_LOAD_NO_TAIL_CHAIN = 8  /* big graph: every colour class is a grid-wide phase (no shared-memory tail chain)    */
 };
 
@@ -203,7 +204,8 @@ ising_status ising_current_state(ising_problem* p, int8_t* spins_out, int32_t n_
  *         12 CTAs of the persistent grid, 13 Gauss-Seidel engine (0 launch per phase, 1 persistent grid, 2 persistent
  *         clusters, 3 persistent grid + shared-memory tail chain, 4 shared-memory chain for the whole graph),
  *         14 rows of the shared-memory chain, 15 virtual phases of the persistent kernel,
- *         16 chunks of the chain, 17 1 if the chain is resident in shared memory
+ *         16 chunks of the chain, 17 1 if the chain is resident in shared memory,
+ *         18 CTAs per word of four replicas of the small-graph engine (cluster size)
  */
 ising_status ising_problem_info(const ising_problem* p, int32_t what, int64_t* value_out);
 

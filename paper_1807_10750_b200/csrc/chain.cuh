@@ -150,20 +150,45 @@ struct ChainGlobal {
     uint8_t* best;       // same position in the captured best state
     uint32_t* old;       // compact copy [n_t_pad] of this CTA
     uint32_t cap4;       // capture mask of this CTA's four replicas (improved in the previous sweep)
+    // FULL chain split over a cluster of `csplit` CTAs (throughput-bound small graphs): CTA `crank` updates its share of
+    // every segment's rows and mirrors the new word into the peers' copies of val[] (distributed shared memory)
+    uint32_t csplit, crank;
 };
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t smem_addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_cluster_u32(uint32_t cluster_addr, uint32_t v) {
+    asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void cluster_barrier() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// this CTA's share [lo, hi) of the rows [r0, r1) of a segment
+__device__ __forceinline__ void chain_share(const ChainGlobal& cg, uint32_t r0, uint32_t r1, uint32_t& lo, uint32_t& hi) {
+    lo = r0; hi = r1;
+    if (cg.csplit > 1u) {
+        const uint32_t part = (r1 - r0 + cg.csplit - 1u) / cg.csplit;
+        lo = min(r1, r0 + cg.crank * part);
+        hi = min(r1, lo + part);
+    }
+}
 
 // One segment: every row takes its energy-minimising value (L47-49, Q1/Q3), the scheduled flip (L177), and its
 // energy increment dE = (a - s) h is added to dE[] (a7; exact because a colour class is an independent set).
-template <bool DELTA>
+template <bool DELTA, bool SPLIT = false>
 __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChunk& ck, uint32_t buf, uint32_t val,
                                               uint32_t flip, const ChainRt& rt, const PhiloxKeys& keys, long long (&dE)[4],
                                               const ChainGlobal& cg, uint32_t tid, uint32_t nthr) {
     const uint32_t logL = sg.info & 0xffu, L = 1u << logL, q = tid & (L - 1u);
     const uint32_t rpi = nthr >> logL;
     const ChunkLayout l = chunk_layout(ck.r1 - ck.r0, ck.c1 - ck.c0, DELTA);
-    uint32_t r = sg.r0 + (tid >> logL);
-    for (uint32_t rw = sg.r0 + ((tid & ~31u) >> logL); rw < sg.r1; rw += rpi, r += rpi) {   // warp-uniform trip count
-        const bool act = r < sg.r1;
+    uint32_t s_lo = sg.r0, s_hi = sg.r1;
+    if (SPLIT) chain_share(cg, sg.r0, sg.r1, s_lo, s_hi);
+    uint32_t r = s_lo + (tid >> logL);
+    for (uint32_t rw = s_lo + ((tid & ~31u) >> logL); rw < s_hi; rw += rpi, r += rpi) {   // warp-uniform trip count
+        const bool act = r < s_hi;
         const uint32_t lr = act ? r - ck.r0 : 0u;
         uint32_t p0 = 0, p1 = 0, f4 = 0;
         if (act) {
@@ -232,6 +257,10 @@ __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChun
                 }
             } else {
                 sts32(val + 4u * r, a);
+                if (SPLIT) {
+                    for (uint32_t pr = 0; pr < cg.csplit; ++pr)   // the peers' copies of val[]
+                        if (pr != cg.crank) st_cluster_u32(mapa_u32(val + 4u * r, pr), a);
+                }
             }
         }
     }
@@ -327,6 +356,7 @@ struct SmallParams {
     long long* best_out;
     int32_t* best_sweep_out;
     int32_t resume;
+    uint32_t csplit;                // CTAs per word (cluster size): 1, or 2 for throughput-bound graphs (resident chain only)
     unsigned long long* timing;     // diagnostics (resident chain only): SM-clock stamps of CTA 0 in sweep timing_sweep: sweep start,
                                     // flips drawn, after every segment, dE reduced, cut / best done, capture done; or nullptr
     uint32_t timing_sweep;
@@ -342,7 +372,8 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
     __shared__ int s_bs[4];
     __shared__ uint32_t s_imp;
     const uint32_t tid = threadIdx.x, nthr = blockDim.x;
-    const uint32_t tile = blockIdx.x / kChainGroups, g = blockIdx.x % kChainGroups, slot = blockIdx.x;
+    const uint32_t csplit = p.csplit, crank = blockIdx.x % csplit, slot = blockIdx.x / csplit;   // slot = word index
+    const uint32_t tile = slot / kChainGroups, g = slot % kChainGroups;
     const uint32_t r_first = tile * kTile + 4u * g;      // first replica of this CTA within the call
     if (r_first >= p.n_replicas) return;                 // no live replica in this word
     const ChainView& v = p.v;
@@ -374,6 +405,9 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
         __syncthreads();
     }
     ChainGlobal cg{};
+    cg.csplit = csplit;
+    cg.crank = crank;
+    __shared__ long long s_part[4][4];   // [CTA of the cluster][replica]: the sweep's energy increments of that CTA's rows
     ChainRt rt;
     rt.rl0 = p.rep0 + r_first;
     rt.tie_rule = p.tie_rule;
@@ -384,14 +418,27 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
         unsigned long long* ts = (p.timing && t == p.timing_sweep && blockIdx.x == 0 && tid == 0) ? p.timing : nullptr;
         if (ts) *ts++ = (unsigned long long)clock64();
         if (v.resident) {
-            chain_draw_flips(v, flip, 0u, n, rt, p.keys, tid, nthr);
+            if (csplit == 1u) {
+                chain_draw_flips(v, flip, 0u, n, rt, p.keys, tid, nthr);
+            } else {   // only the rows this CTA will update
+                for (uint32_t s = 0; s < v.n_segs; ++s) {
+                    uint32_t lo, hi;
+                    chain_share(cg, s_segs[s].r0, s_segs[s].r1, lo, hi);
+                    chain_draw_flips(v, flip, lo, hi, rt, p.keys, tid, nthr);
+                }
+            }
             __syncthreads();
             if (ts) *ts++ = (unsigned long long)clock64();
             const ChainChunk ck = s_chunks[0];
             for (uint32_t s = 0; s < v.n_segs; ++s) {
                 const ChainSeg sg = s_segs[s];
-                chain_segment<false>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
-                if (sg.info & 0x100u) __syncthreads();
+                if (csplit > 1u) {
+                    chain_segment<false, true>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
+                    if (sg.info & 0x100u) cluster_barrier();
+                } else {
+                    chain_segment<false>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
+                    if (sg.info & 0x100u) __syncthreads();
+                }
                 if (ts) *ts++ = (unsigned long long)clock64();
             }
         } else {
@@ -399,9 +446,24 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
         }
         chain_reduce_dE(dE, s_wdE, tid, v.narrow != 0u);
         __syncthreads();
+        if (csplit > 1u) {   // every CTA of the cluster gets every CTA's partial sums, then all keep the same books
+            if (tid < 4u) {
+                const long long part = chain_sum_dE(s_wdE, tid, nthr >> 5);
+                const uint32_t at = (uint32_t)__cvta_generic_to_shared(&s_part[crank][tid]);
+                for (uint32_t pr = 0; pr < csplit; ++pr) {
+                    const uint32_t ra = mapa_u32(at, pr);
+                    st_cluster_u32(ra, (uint32_t)(unsigned long long)part);
+                    st_cluster_u32(ra + 4u, (uint32_t)((unsigned long long)part >> 32));
+                }
+            }
+            cluster_barrier();
+        }
         if (ts) *ts++ = (unsigned long long)clock64();
         if (tid < 4u) {   // a7: E, cut = (W - E)/2 (eq. 4), best tracking (strictly greater: the earliest sweep wins)
-            const long long E = s_E[tid] + chain_sum_dE(s_wdE, tid, nthr >> 5);
+            long long dsum = 0;
+            if (csplit > 1u) { for (uint32_t pr = 0; pr < csplit; ++pr) dsum += s_part[pr][tid]; }
+            else dsum = chain_sum_dE(s_wdE, tid, nthr >> 5);
+            const long long E = s_E[tid] + dsum;
             const long long cut = (p.W - E) / 2;
             const bool live = r_first + tid < p.n_replicas;
             const bool improved = live && cut > s_bc[tid];
@@ -416,20 +478,21 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
         const uint32_t imp = s_imp;
         if (imp != 0u) {   // capture the improved replicas' bytes of every row
             const uint32_t km = nibble_to_bytemask(imp);
-            for (uint32_t r = tid; r < n; r += nthr) {
+            for (uint32_t r = tid + crank * nthr; r < n; r += nthr * csplit) {   // (a cluster's CTAs share the rows)
                 const uint32_t s = lds32(val + 4u * r);
                 bcomp[r] = imp == 15u ? s : ((s & km) | (bcomp[r] & ~km));
             }
-            __syncthreads();   // the next sweep rewrites val
+            if (csplit > 1u) cluster_barrier(); else __syncthreads();   // the next sweep rewrites val (also the peers' copies)
         }
         if (ts) *ts++ = (unsigned long long)clock64();
     }
     // final state and best state back to the standard layout
-    for (uint32_t r = tid; r < n; r += nthr) {
+    for (uint32_t r = tid + crank * nthr; r < n; r += nthr * csplit) {
         *reinterpret_cast<uint32_t*>(gstate + (size_t)r * kTile) = lds32(val + 4u * r);
         *reinterpret_cast<uint32_t*>(gbest + (size_t)r * kTile) = bcomp[r];
     }
-    if (tid < 4u) {
+    if (csplit > 1u) cluster_barrier();   // no CTA leaves while a peer may still write into its shared memory
+    if (tid < 4u && crank == 0u) {
         p.E_out[r_first + tid] = s_E[tid];
         p.best_out[r_first + tid] = s_bc[tid];
         p.best_sweep_out[r_first + tid] = s_bs[tid];

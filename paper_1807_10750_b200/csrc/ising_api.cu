@@ -185,6 +185,7 @@ struct ising_problem {
     bool chain_delta = false;
     uint32_t small_threads = 0;
     size_t small_dyn = 0;
+    uint32_t small_csplit = 1;              // CTAs per word of four replicas (cluster size) of k_anneal_small
     uint32_t* vphase_slices = nullptr;      // [n_vphases + 1] slice ranges of the persistent kernel's virtual phases
     std::vector<uint32_t> thr_host;         // the call's thresholds (pageable copy: the caller's array is free on return)
     uint32_t n_vphases = 0;
@@ -918,6 +919,11 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
                 p->chain_small = true;
                 p->small_threads = threads;
                 p->small_dyn = (size_t)val_bytes + (size_t)buf_bytes * (resident ? 1u : 2u);
+                // a throughput-bound small graph (its widest class gives every thread several rows) runs on a cluster of two
+                // CTAs per word: each updates half of every class and mirrors its words into the peer's shared memory
+                uint32_t widest = 0;
+                for (size_t j = 0; j + 1 < lvl.size(); ++j) widest = std::max(widest, lvl[j + 1] - lvl[j]);
+                p->small_csplit = (resident && widest >= 2u * threads && !(flags & ISING_LOAD_NO_CLUSTER)) ? 2u : 1u;
             }
             CKP(cudaStreamSynchronize(st));   // the plan's host vectors die here
         }
@@ -1098,7 +1104,20 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
             a.timing = s0 == 0 ? p->timing : nullptr;
             a.timing_sweep = p->timing_sweep;
             a.keys = keys;
-            k_anneal_small<<<(unsigned)(tiles * kChainGroups), p->small_threads, p->small_dyn, st>>>(a);
+            a.csplit = p->small_csplit;
+            {
+                cudaLaunchConfig_t cfg{};
+                cfg.gridDim = dim3((unsigned)(tiles * kChainGroups) * p->small_csplit);
+                cfg.blockDim = dim3(p->small_threads);
+                cfg.dynamicSmemBytes = p->small_dyn;
+                cfg.stream = st;
+                cudaLaunchAttribute at[1];
+                at[0].id = cudaLaunchAttributeClusterDimension;
+                at[0].val.clusterDim.x = p->small_csplit; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+                cfg.attrs = at;
+                cfg.numAttrs = p->small_csplit > 1u ? 1 : 0;
+                CK(cudaLaunchKernelEx(&cfg, k_anneal_small, a));
+            }
             p->launches++;
         }
         p->parity = 0;
@@ -1394,6 +1413,7 @@ ising_status ising_problem_info(const ising_problem* p, int32_t what, int64_t* v
         case 15: *value_out = p->n_vphases; break;
         case 16: *value_out = (p->chain_small || p->chain_delta) ? p->chain.n_chunks : 0; break;
         case 17: *value_out = (p->chain_small || p->chain_delta) ? p->chain.resident : 0; break;
+        case 18: *value_out = p->chain_small ? p->small_csplit : 0; break;
         default: return ISING_ERR_BAD_SHAPE;
     }
     return ISING_OK;

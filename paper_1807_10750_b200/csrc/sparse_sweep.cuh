@@ -959,6 +959,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 ChainRt rt;
                 rt.thr = thr; rt.T = T; rt.rl0 = p.rep0 + ctile * kTile + 4u * cgrp; rt.tie_rule = p.tie_rule;
                 ChainGlobal cgl;
+                cgl.csplit = 1u; cgl.crank = 0u;
                 const size_t o = (size_t)ctile * p.tile_stride + (size_t)v.row_lo * kTile + 4u * cgrp;
                 cgl.state = p.state + o;
                 cgl.best = p.best + o;
