@@ -61,6 +61,7 @@ struct ChainView {
     uint32_t buf_bytes;      // capacity of one chunk buffer
     uint32_t threads;        // CTA size the segments' lanes-per-row were planned for
     uint32_t narrow;         // a sweep's energy increments of all chain rows fit int32
+    uint32_t premul;         // the cells hold byte offsets into val[] (n_t_pad <= 16384), else local ids
 };
 
 struct ChunkLayout { uint32_t ptr, h0, old, idx, w, bytes; };
@@ -150,9 +151,6 @@ struct ChainGlobal {
     uint8_t* best;       // same position in the captured best state
     uint32_t* old;       // compact copy [n_t_pad] of this CTA
     uint32_t cap4;       // capture mask of this CTA's four replicas (improved in the previous sweep)
-    // FULL chain split over a cluster of `csplit` CTAs (throughput-bound small graphs): CTA `crank` updates its share of
-    // every segment's rows and mirrors the new word into the peers' copies of val[] (distributed shared memory)
-    uint32_t csplit, crank;
 };
 __device__ __forceinline__ uint32_t mapa_u32(uint32_t smem_addr, uint32_t rank) {
     uint32_t r;
@@ -165,43 +163,68 @@ __device__ __forceinline__ void st_cluster_u32(uint32_t cluster_addr, uint32_t v
 __device__ __forceinline__ void cluster_barrier() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
-// this CTA's share [lo, hi) of the rows [r0, r1) of a segment
-__device__ __forceinline__ void chain_share(const ChainGlobal& cg, uint32_t r0, uint32_t r1, uint32_t& lo, uint32_t& hi) {
-    lo = r0; hi = r1;
-    if (cg.csplit > 1u) {
-        const uint32_t part = (r1 - r0 + cg.csplit - 1u) / cg.csplit;
-        lo = min(r1, r0 + cg.crank * part);
-        hi = min(r1, lo + part);
-    }
+// mbarrier hand-off between the two CTAs of a cluster (k_anneal_small, flip producer / level consumer)
+__device__ __forceinline__ void mbar_init_cta(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_bar) {   // release at cluster scope
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+// (no data is published: the arriving CTA only says that its loads of a buffer have returned, which the CTA barrier before
+// the call has already made certain; a release here would cost a device-wide fence on the critical path)
+__device__ __forceinline__ void mbar_arrive_remote_relaxed(uint32_t cluster_bar) {
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {   // acquire at cluster scope
+    asm volatile(
+        "{\n\t.reg .pred p;\n"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t"
+        "@!p bra WAIT_%=;\n\t}"
+        ::"r"(bar), "r"(parity) : "memory");
 }
 
 // One segment: every row takes its energy-minimising value (L47-49, Q1/Q3), the scheduled flip (L177), and its
 // energy increment dE = (a - s) h is added to dE[] (a7; exact because a colour class is an independent set).
-template <bool DELTA, bool SPLIT = false>
+// PREMUL: the cells hold BYTE offsets into val[] (local id x 4: chains of at most 16 384 rows), not local ids.
+template <bool DELTA, bool PREMUL>
 __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChunk& ck, uint32_t buf, uint32_t val,
                                               uint32_t flip, const ChainRt& rt, const PhiloxKeys& keys, long long (&dE)[4],
                                               const ChainGlobal& cg, uint32_t tid, uint32_t nthr) {
     const uint32_t logL = sg.info & 0xffu, L = 1u << logL, q = tid & (L - 1u);
     const uint32_t rpi = nthr >> logL;
     const ChunkLayout l = chunk_layout(ck.r1 - ck.r0, ck.c1 - ck.c0, DELTA);
-    uint32_t s_lo = sg.r0, s_hi = sg.r1;
-    if (SPLIT) chain_share(cg, sg.r0, sg.r1, s_lo, s_hi);
+    const uint32_t s_lo = sg.r0, s_hi = sg.r1;
+    const uint32_t fmask = rt.thr != 0u ? 15u : 0u;
     uint32_t r = s_lo + (tid >> logL);
     for (uint32_t rw = s_lo + ((tid & ~31u) >> logL); rw < s_hi; rw += rpi, r += rpi) {   // warp-uniform trip count
-        const bool act = r < s_hi;
-        const uint32_t lr = act ? r - ck.r0 : 0u;
-        uint32_t p0 = 0, p1 = 0, f4 = 0;
-        if (act) {
-            p0 = lds16(buf + l.ptr + 2u * lr);
-            p1 = lds16(buf + l.ptr + 2u * lr + 2u);
-            if (q == 0 && rt.thr != 0u) f4 = lds8(flip + r);
-        }
+        // every lane runs the whole update on a valid row (no divergence); the first lane of a live row stores it
+        const bool storer = r < s_hi && q == 0u;
+        const uint32_t rowc = min(r, s_hi - 1u), lr = rowc - ck.r0;
+        const uint32_t p0 = lds16(buf + l.ptr + 2u * lr), p1 = lds16(buf + l.ptr + 2u * lr + 2u);
+        const uint32_t f4 = lds8(flip + rowc) & fmask;
+        uint32_t oldw;
         int h0 = 0, h1 = 0, h2 = 0, h3 = 0;
+        if (DELTA) {
+            oldw = lds32(buf + l.old + 4u * lr);
+            if (q == 0u) {
+                const uint4 hh = lds128(buf + l.h0 + 16u * lr);
+                h0 = (int)hh.x; h1 = (int)hh.y; h2 = (int)hh.z; h3 = (int)hh.w;
+            }
+        } else {
+            oldw = lds32(val + 4u * rowc);
+        }
         for (uint32_t k = p0 + q; k < p1; k += L) {
             const uint2 ix = lds64(buf + l.idx + 8u * k);
             const uint32_t w = lds32(buf + l.w + 4u * k);
-            const uint32_t e0 = lds32(val + 4u * (ix.x & 0xffffu)), e1 = lds32(val + 4u * (ix.x >> 16));
-            const uint32_t e2 = lds32(val + 4u * (ix.y & 0xffffu)), e3 = lds32(val + 4u * (ix.y >> 16));
+            uint32_t e0, e1, e2, e3;
+            if (PREMUL) {
+                e0 = lds32(val + (ix.x & 0xffffu)); e1 = lds32(val + (ix.x >> 16));
+                e2 = lds32(val + (ix.y & 0xffffu)); e3 = lds32(val + (ix.y >> 16));
+            } else {
+                e0 = lds32(val + 4u * (ix.x & 0xffffu)); e1 = lds32(val + 4u * (ix.x >> 16));
+                e2 = lds32(val + 4u * (ix.y & 0xffffu)); e3 = lds32(val + 4u * (ix.y >> 16));
+            }
             uint32_t t0, t1, t2, t3;
             transpose4x4(e0, e1, e2, e3, t0, t1, t2, t3);
             h0 = __dp4a((int)t0, (int)w, h0);
@@ -210,41 +233,36 @@ __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChun
             h3 = __dp4a((int)t3, (int)w, h3);
         }
         // (a REDUX per group member mask was measured 3x slower than the butterfly: the groups of a warp are serialised)
-        for (uint32_t o = 1; o < L; o <<= 1) {
-            h0 += __shfl_xor_sync(0xffffffffu, h0, o);
-            h1 += __shfl_xor_sync(0xffffffffu, h1, o);
-            h2 += __shfl_xor_sync(0xffffffffu, h2, o);
-            h3 += __shfl_xor_sync(0xffffffffu, h3, o);
+        if (L > 1u) {
+#pragma unroll
+            for (uint32_t o = 1; o < 32u; o <<= 1) {
+                if (o < L) {
+                    h0 += __shfl_xor_sync(0xffffffffu, h0, o);
+                    h1 += __shfl_xor_sync(0xffffffffu, h1, o);
+                    h2 += __shfl_xor_sync(0xffffffffu, h2, o);
+                    h3 += __shfl_xor_sync(0xffffffffu, h3, o);
+                }
+            }
         }
-        if (act && q == 0) {
-            uint32_t oldw;
+        uint32_t a = ~sign_bytes(h0, h1, h2, h3) | 0x01010101u;   // +1 where h < 0, else -1
+        if (rt.tie_rule == 1) {                                   // KEEP: h == 0 leaves the spin
+            const uint32_t z = (h0 == 0 ? 0xffu : 0u) | (h1 == 0 ? 0xff00u : 0u) | (h2 == 0 ? 0xff0000u : 0u) |
+                               (h3 == 0 ? 0xff000000u : 0u);
+            a = (a & ~z) | (oldw & z);
+        }
+        a ^= ((f4 * 0x00204081u) & 0x01010101u) * 0xfeu;
+        const uint32_t d2 = storer ? (a << 1) & (a ^ oldw) : 0u;  // a - s per byte: 0, +2, -2
+        asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[0]) : "r"(sbyte(d2, 0)), "r"(h0));
+        asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[1]) : "r"(sbyte(d2, 1)), "r"(h1));
+        asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[2]) : "r"(sbyte(d2, 2)), "r"(h2));
+        asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[3]) : "r"(sbyte(d2, 3)), "r"(h3));
+        if (storer) {
             if (DELTA) {
-                oldw = lds32(buf + l.old + 4u * lr);
-                const uint4 hh = lds128(buf + l.h0 + 16u * lr);
-                h0 += (int)hh.x; h1 += (int)hh.y; h2 += (int)hh.z; h3 += (int)hh.w;
-            } else {
-                oldw = lds32(val + 4u * r);
-            }
-            uint32_t a = ~sign_bytes(h0, h1, h2, h3) | 0x01010101u;   // +1 where h < 0, else -1
-            if (rt.tie_rule == 1) {                                   // KEEP: h == 0 leaves the spin
-                const uint32_t z = (h0 == 0 ? 0xffu : 0u) | (h1 == 0 ? 0xff00u : 0u) | (h2 == 0 ? 0xff0000u : 0u) |
-                                   (h3 == 0 ? 0xff000000u : 0u);
-                a = (a & ~z) | (oldw & z);
-            }
-            a ^= ((f4 * 0x00204081u) & 0x01010101u) * 0xfeu;
-            const uint32_t d2 = (a << 1) & (a ^ oldw);                // a - s per byte: 0, +2, -2
-            if (d2 != 0u) {
-                dE[0] += (long long)(sbyte(d2, 0) * h0);
-                dE[1] += (long long)(sbyte(d2, 1) * h1);
-                dE[2] += (long long)(sbyte(d2, 2) * h2);
-                dE[3] += (long long)(sbyte(d2, 3) * h3);
-            }
-            if (DELTA) {
-                sts32(val + 4u * r, d2);
-                const size_t at = (size_t)r * kTile;
+                sts32(val + 4u * rowc, d2);
+                const size_t at = (size_t)rowc * kTile;
                 if (d2 != 0u) {
                     *reinterpret_cast<uint32_t*>(cg.state + at) = a;
-                    cg.old[r] = a;
+                    cg.old[rowc] = a;
                 }
                 if (cg.cap4 != 0u) {   // fused best-state capture: the value the row held after the previous sweep
                     uint32_t* bp = reinterpret_cast<uint32_t*>(cg.best + at);
@@ -256,11 +274,7 @@ __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChun
                     }
                 }
             } else {
-                sts32(val + 4u * r, a);
-                if (SPLIT) {
-                    for (uint32_t pr = 0; pr < cg.csplit; ++pr)   // the peers' copies of val[]
-                        if (pr != cg.crank) st_cluster_u32(mapa_u32(val + 4u * r, pr), a);
-                }
+                sts32(val + 4u * rowc, a);
             }
         }
     }
@@ -268,7 +282,7 @@ __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChun
 
 // One pass over all chain levels (one sweep of the chain rows), chunks streamed through two buffers.
 // s_chunks / s_segs: the tables in shared memory.  DELTA: h0 of a chunk is cleared once it has landed.
-template <bool DELTA>
+template <bool DELTA, bool PREMUL>
 __device__ __forceinline__ void chain_pass_streamed(const ChainView& v, const ChainChunk* s_chunks, const ChainSeg* s_segs,
                                                     uint32_t val, uint32_t flip, uint32_t buf0, uint32_t slot, const ChainRt& rt,
                                                     const PhiloxKeys& keys, long long (&dE)[4], const ChainGlobal& cg,
@@ -301,7 +315,7 @@ __device__ __forceinline__ void chain_pass_streamed(const ChainView& v, const Ch
         bool synced = false;
         for (uint32_t s = ck.seg0; s < ck.seg1; ++s) {
             const ChainSeg sg = s_segs[s];
-            chain_segment<DELTA>(sg, ck, buf, val, flip, rt, keys, dE, cg, tid, nthr);
+            chain_segment<DELTA, PREMUL>(sg, ck, buf, val, flip, rt, keys, dE, cg, tid, nthr);
             synced = (sg.info & 0x100u) != 0u;
             if (synced) __syncthreads();
             stamp();
@@ -356,13 +370,19 @@ struct SmallParams {
     long long* best_out;
     int32_t* best_sweep_out;
     int32_t resume;
-    uint32_t csplit;                // CTAs per word (cluster size): 1, or 2 for throughput-bound graphs (resident chain only)
+    uint32_t csplit;                // CTAs per word (cluster size): 1, or 2 = levels + flip producer (resident chain only)
     unsigned long long* timing;     // diagnostics (resident chain only): SM-clock stamps of CTA 0 in sweep timing_sweep: sweep start,
                                     // flips drawn, after every segment, dE reduced, cut / best done, capture done; or nullptr
     uint32_t timing_sweep;
     PhiloxKeys keys;
 };
 
+// csplit == 2 (resident chain, enough SMs): every word runs on a CLUSTER of two CTAs.  CTA 0 walks the levels; CTA 1 only
+// draws the flip decisions -- they do not depend on the spins -- one sweep ahead, straight into CTA 0's shared memory
+// (two flip buffers, st.shared::cluster), and hands each buffer over through an mbarrier in CTA 0 (remote arrive, release /
+// acquire at cluster scope); CTA 0 gives a buffer back through an mbarrier in CTA 1 once its sweep is done.  The Philox
+// work (about half the instructions of a sweep of a low-degree graph) leaves the SM that runs the dependent levels.
+template <bool TIMING, bool PREMUL>
 __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const SmallParams p) {
     extern __shared__ __align__(128) uint8_t chain_smem[];
     __shared__ ChainChunk s_chunks[kChainMaxChunks];
@@ -371,16 +391,55 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
     __shared__ long long s_E[4], s_bc[4];
     __shared__ int s_bs[4];
     __shared__ uint32_t s_imp;
+    __shared__ int s_w32[kSmallThreadsMax / 32][4];   // (narrow sums: the warps' parts, added up by warp 0)
+    __shared__ __align__(8) unsigned long long s_full[2], s_empty[2];   // flip buffer b: filled (in CTA 0) / free again (in CTA 1)
     const uint32_t tid = threadIdx.x, nthr = blockDim.x;
     const uint32_t csplit = p.csplit, crank = blockIdx.x % csplit, slot = blockIdx.x / csplit;   // slot = word index
     const uint32_t tile = slot / kChainGroups, g = slot % kChainGroups;
     const uint32_t r_first = tile * kTile + 4u * g;      // first replica of this CTA within the call
-    if (r_first >= p.n_replicas) return;                 // no live replica in this word
+    if (r_first >= p.n_replicas) return;                 // no live replica in this word (both CTAs of a cluster leave)
     const ChainView& v = p.v;
     const uint32_t n = v.n_t;
-    const uint32_t val = (uint32_t)__cvta_generic_to_shared(chain_smem);
-    const uint32_t flip = val + chain_align16(4u * v.n_t_pad);
-    const uint32_t buf0 = flip + chain_align16(v.n_t_pad);
+    uint32_t val;   // (opaque to the compiler: it would otherwise re-derive the shared window address wherever it is used)
+    asm volatile("{ .reg .u64 t; cvta.to.shared.u64 t, %1; cvt.u32.u64 %0, t; }" : "=r"(val) : "l"(chain_smem));
+    const uint32_t flip_bytes = chain_align16(v.n_t_pad);
+    const uint32_t flip0 = val + chain_align16(4u * v.n_t_pad);
+    const uint32_t buf0 = flip0 + 2u * flip_bytes;
+    const uint32_t full0 = (uint32_t)__cvta_generic_to_shared(&s_full[0]), empty0 = (uint32_t)__cvta_generic_to_shared(&s_empty[0]);
+    ChainRt rt;
+    rt.rl0 = p.rep0 + r_first;
+    rt.tie_rule = p.tie_rule;
+    if (csplit > 1u) {
+        if (tid == 0) {
+            mbar_init_cta(full0, nthr); mbar_init_cta(full0 + 8u, nthr);
+            mbar_init_cta(empty0, 1u);  mbar_init_cta(empty0 + 8u, 1u);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        cluster_barrier();
+        if (crank == 1u) {   // ---- the flip producer
+            const uint32_t full_r = mapa_u32(full0, 0u), flip_r = mapa_u32(flip0, 0u);
+            uint32_t k = 0;   // sweeps with flips so far (both CTAs count alike)
+            for (uint32_t t = 0; t < p.n_sweeps; ++t) {
+                rt.thr = __ldg(p.thr + t);
+                rt.T = p.sweep_offset + t;
+                if (rt.thr == 0u) continue;
+                const uint32_t b = k & 1u;
+                if (k >= 2u) mbar_wait_cluster(empty0 + 8u * b, ((k >> 1) - 1u) & 1u);   // CTA 0 is done with sweep k - 2
+                for (uint32_t r4 = 4u * tid; r4 < n; r4 += 4u * nthr) {   // four rows per thread: one 32-bit store
+                    const uint4 o = __ldg(reinterpret_cast<const uint4*>(v.orig + r4));
+                    const uint32_t f = chain_flip4(o.x, rt, p.keys) | (chain_flip4(o.y, rt, p.keys) << 8) |
+                                       (chain_flip4(o.z, rt, p.keys) << 16) | (chain_flip4(o.w, rt, p.keys) << 24);
+                    st_cluster_u32(flip_r + b * flip_bytes + r4, f);
+                }
+                mbar_arrive_remote(full_r + 8u * b);
+                ++k;
+            }
+            cluster_barrier();   // (CTA 0 may arrive on this CTA's barriers until it is through)
+            return;
+        }
+    }
+    const uint32_t empty_r = csplit > 1u ? mapa_u32(empty0, 1u) : 0u;
+    uint32_t kf = 0;   // sweeps with flips so far
     uint8_t* const gstate = p.state + (size_t)tile * p.tile_stride + 4u * g;
     uint8_t* const gbest = p.best + (size_t)tile * p.tile_stride + 4u * g;
     uint32_t* const bcomp = p.best_compact + (size_t)slot * p.bc_stride;
@@ -405,64 +464,60 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
         __syncthreads();
     }
     ChainGlobal cg{};
-    cg.csplit = csplit;
-    cg.crank = crank;
-    __shared__ long long s_part[4][4];   // [CTA of the cluster][replica]: the sweep's energy increments of that CTA's rows
-    ChainRt rt;
-    rt.rl0 = p.rep0 + r_first;
-    rt.tie_rule = p.tie_rule;
     long long dE[4] = {0, 0, 0, 0};
     for (uint32_t t = 0; t < p.n_sweeps; ++t) {
         rt.thr = __ldg(p.thr + t);
         rt.T = p.sweep_offset + t;
-        unsigned long long* ts = (p.timing && t == p.timing_sweep && blockIdx.x == 0 && tid == 0) ? p.timing : nullptr;
-        if (ts) *ts++ = (unsigned long long)clock64();
+        unsigned long long* ts = (TIMING && p.timing && t == p.timing_sweep && blockIdx.x == 0 && tid == 0) ? p.timing : nullptr;
+        if (TIMING && ts) *ts++ = (unsigned long long)clock64();
         if (v.resident) {
+            const uint32_t fb = kf & 1u, flip = flip0 + fb * flip_bytes;
             if (csplit == 1u) {
                 chain_draw_flips(v, flip, 0u, n, rt, p.keys, tid, nthr);
-            } else {   // only the rows this CTA will update
-                for (uint32_t s = 0; s < v.n_segs; ++s) {
-                    uint32_t lo, hi;
-                    chain_share(cg, s_segs[s].r0, s_segs[s].r1, lo, hi);
-                    chain_draw_flips(v, flip, lo, hi, rt, p.keys, tid, nthr);
-                }
+                __syncthreads();
+            } else if (rt.thr != 0u) {
+                mbar_wait_cluster(full0 + 8u * fb, (kf >> 1) & 1u);   // the producer has filled this sweep's buffer
             }
-            __syncthreads();
-            if (ts) *ts++ = (unsigned long long)clock64();
+            if (TIMING && ts) *ts++ = (unsigned long long)clock64();
             const ChainChunk ck = s_chunks[0];
             for (uint32_t s = 0; s < v.n_segs; ++s) {
                 const ChainSeg sg = s_segs[s];
-                if (csplit > 1u) {
-                    chain_segment<false, true>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
-                    if (sg.info & 0x100u) cluster_barrier();
-                } else {
-                    chain_segment<false>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
-                    if (sg.info & 0x100u) __syncthreads();
-                }
-                if (ts) *ts++ = (unsigned long long)clock64();
+                chain_segment<false, PREMUL>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
+                if (sg.info & 0x100u) __syncthreads();
+                if (TIMING && ts) *ts++ = (unsigned long long)clock64();
+            }
+            if (rt.thr != 0u) {   // (every thread is past the last level: the flip buffer goes back to the producer)
+                if (csplit > 1u && tid == nthr - 32u) mbar_arrive_remote_relaxed(empty_r + 8u * fb);
+                ++kf;
             }
         } else {
-            chain_pass_streamed<false>(v, s_chunks, s_segs, val, flip, buf0, slot, rt, p.keys, dE, cg, tid, nthr, false);
+            chain_pass_streamed<false, PREMUL>(v, s_chunks, s_segs, val, flip0, buf0, slot, rt, p.keys, dE, cg, tid, nthr, false);
         }
-        chain_reduce_dE(dE, s_wdE, tid, v.narrow != 0u);
+        if (v.narrow != 0u) {
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const int x = __reduce_add_sync(0xffffffffu, (int)dE[b]);
+                if ((tid & 31u) == 0u) s_w32[tid >> 5][b] = x;
+                dE[b] = 0;
+            }
+        } else {
+            chain_reduce_dE(dE, s_wdE, tid, false);
+        }
         __syncthreads();
-        if (csplit > 1u) {   // every CTA of the cluster gets every CTA's partial sums, then all keep the same books
-            if (tid < 4u) {
-                const long long part = chain_sum_dE(s_wdE, tid, nthr >> 5);
-                const uint32_t at = (uint32_t)__cvta_generic_to_shared(&s_part[crank][tid]);
-                for (uint32_t pr = 0; pr < csplit; ++pr) {
-                    const uint32_t ra = mapa_u32(at, pr);
-                    st_cluster_u32(ra, (uint32_t)(unsigned long long)part);
-                    st_cluster_u32(ra + 4u, (uint32_t)((unsigned long long)part >> 32));
+        if (TIMING && ts) *ts++ = (unsigned long long)clock64();
+        long long dsum = 0;
+        if (v.narrow != 0u) {
+            if (tid < 32u) {
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const int y = __reduce_add_sync(0xffffffffu, tid < (nthr >> 5) ? s_w32[tid][b] : 0);
+                    if (tid == (uint32_t)b) dsum = (long long)y;
                 }
             }
-            cluster_barrier();
+        } else if (tid < 4u) {
+            dsum = chain_sum_dE(s_wdE, tid, nthr >> 5);
         }
-        if (ts) *ts++ = (unsigned long long)clock64();
         if (tid < 4u) {   // a7: E, cut = (W - E)/2 (eq. 4), best tracking (strictly greater: the earliest sweep wins)
-            long long dsum = 0;
-            if (csplit > 1u) { for (uint32_t pr = 0; pr < csplit; ++pr) dsum += s_part[pr][tid]; }
-            else dsum = chain_sum_dE(s_wdE, tid, nthr >> 5);
             const long long E = s_E[tid] + dsum;
             const long long cut = (p.W - E) / 2;
             const bool live = r_first + tid < p.n_replicas;
@@ -474,29 +529,29 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
             if (tid == 0) s_imp = m;
         }
         __syncthreads();
-        if (ts) *ts++ = (unsigned long long)clock64();
+        if (TIMING && ts) *ts++ = (unsigned long long)clock64();
         const uint32_t imp = s_imp;
         if (imp != 0u) {   // capture the improved replicas' bytes of every row
             const uint32_t km = nibble_to_bytemask(imp);
-            for (uint32_t r = tid + crank * nthr; r < n; r += nthr * csplit) {   // (a cluster's CTAs share the rows)
+            for (uint32_t r = tid; r < n; r += nthr) {
                 const uint32_t s = lds32(val + 4u * r);
                 bcomp[r] = imp == 15u ? s : ((s & km) | (bcomp[r] & ~km));
             }
-            if (csplit > 1u) cluster_barrier(); else __syncthreads();   // the next sweep rewrites val (also the peers' copies)
+            __syncthreads();   // the next sweep rewrites val
         }
-        if (ts) *ts++ = (unsigned long long)clock64();
+        if (TIMING && ts) *ts++ = (unsigned long long)clock64();
     }
     // final state and best state back to the standard layout
-    for (uint32_t r = tid + crank * nthr; r < n; r += nthr * csplit) {
+    for (uint32_t r = tid; r < n; r += nthr) {
         *reinterpret_cast<uint32_t*>(gstate + (size_t)r * kTile) = lds32(val + 4u * r);
         *reinterpret_cast<uint32_t*>(gbest + (size_t)r * kTile) = bcomp[r];
     }
-    if (csplit > 1u) cluster_barrier();   // no CTA leaves while a peer may still write into its shared memory
-    if (tid < 4u && crank == 0u) {
+    if (tid < 4u) {
         p.E_out[r_first + tid] = s_E[tid];
         p.best_out[r_first + tid] = s_bc[tid];
         p.best_sweep_out[r_first + tid] = s_bs[tid];
     }
+    if (csplit > 1u) cluster_barrier();   // no CTA leaves while its peer may still touch its shared memory
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -508,7 +563,7 @@ template <bool FILL>
 __global__ void k_chain_build(uint32_t n_t, uint32_t row_lo, int delta, const int32_t* perm, const int32_t* inv,
                               const long long* row_ptr, const int32_t* col, const void* w, int wtype,
                               const int32_t* colour, const uint32_t* cptr, uint32_t* counts, uint16_t* idx16,
-                              int8_t* w8, uint32_t* orig_out) {
+                              int8_t* w8, uint32_t* orig_out, uint32_t id_shift) {
     const uint32_t r = (uint32_t)(((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
     const uint32_t lane = threadIdx.x & 31u;
     if (r >= n_t) return;
@@ -531,7 +586,7 @@ __global__ void k_chain_build(uint32_t n_t, uint32_t row_lo, int delta, const in
         const uint32_t m = __ballot_sync(0xffffffffu, ok);
         if (FILL && ok) {
             const unsigned long long at = base_at + cnt + __popc(m & ((1u << lane) - 1u));
-            idx16[at] = (uint16_t)(u - row_lo);
+            idx16[at] = (uint16_t)((u - row_lo) << id_shift);   // (id_shift 2: byte offset into val[])
             w8[at] = (int8_t)wv;
         }
         cnt += __popc(m);
@@ -541,7 +596,7 @@ __global__ void k_chain_build(uint32_t n_t, uint32_t row_lo, int delta, const in
     } else {
         const unsigned long long end_at = 4ull * cptr[r + 1];   // padding (and the alignment gap before the next chunk)
         for (unsigned long long at = base_at + cnt + lane; at < end_at; at += 32) {
-            idx16[at] = (uint16_t)r;
+            idx16[at] = (uint16_t)(r << id_shift);
             w8[at] = 0;
         }
         if (lane == 0) orig_out[r] = (uint32_t)orig;

@@ -836,7 +836,7 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         if (ws.overflow) return fail(ISING_ERR_WORKSPACE_TOO_SMALL);
         const unsigned cb = (unsigned)(((unsigned long long)n_t * 32 + 255) / 256);
         k_chain_build<false><<<cb, 256, 0, st>>>(n_t, row_lo, delta ? 1 : 0, p->perm, p->inv, d_row_ptr, d_col, d_w, wtype,
-                                                 d_colour, nullptr, d_cnt, nullptr, nullptr, nullptr);
+                                                 d_colour, nullptr, d_cnt, nullptr, nullptr, nullptr, 0u);
         std::vector<uint32_t> counts(n_t);
         CKP(cudaMemcpyAsync(counts.data(), d_cnt, 4 * (size_t)n_t, cudaMemcpyDeviceToHost, st));
         CKP(cudaStreamSynchronize(st));
@@ -846,10 +846,12 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
             CKP(cudaGetDevice(&dev));
             CKP(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
         }
+        const bool premul = n_t_pad <= 16384u;   // 16-bit cells can hold id x 4 (the tail chain always: kTailRowsMax)
         ChainPlan pl;
         bool resident = false;
         uint32_t threads = kSweepThreads, buf_bytes = 0;
-        const uint32_t val_bytes = chain_align16(4u * n_t_pad) + chain_align16(n_t_pad);   // val[] + flip[]
+        // val[] + flip[] (k_anneal_small: two flip buffers)
+        const uint32_t val_bytes = chain_align16(4u * n_t_pad) + chain_align16(n_t_pad) * (delta ? 1u : 2u);
         if (delta) {
             buf_bytes = val_bytes < kChainSmemBytes ? ((kChainSmemBytes - val_bytes) / 2u) & ~15u : 0u;
             if (buf_bytes >= 4096u) pl = plan_chain(counts, lvl, buf_bytes, true, threads);
@@ -867,7 +869,7 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
             threads = (uint32_t)std::min<uint64_t>((uint64_t)kSmallThreadsMax, pow2_ceil((uint32_t)std::min<uint64_t>(want, 4096)));
             threads = small_threads_override(std::max(threads, 256u));
             cudaFuncAttributes fa{};
-            CKP(cudaFuncGetAttributes(&fa, k_anneal_small));
+            CKP(cudaFuncGetAttributes(&fa, k_anneal_small<true, false>));
             const int64_t cap = (int64_t)smem_optin - (int64_t)fa.sharedSizeBytes - (int64_t)val_bytes - 256;
             if (cap >= 8192) {
                 pl = plan_chain(counts, lvl, (uint32_t)cap & ~15u, false, threads);
@@ -905,13 +907,13 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
             if (delta) CKP(cudaMemsetAsync(d_h0, 0, tl * kChainGroups * (size_t)n_t_pad * 16, st));
             k_chain_build<true><<<cb, 256, 0, st>>>(n_t, row_lo, delta ? 1 : 0, p->perm, p->inv, d_row_ptr, d_col, d_w, wtype,
                                                     d_colour, d_cptr, nullptr, reinterpret_cast<uint16_t*>(d_cidx),
-                                                    reinterpret_cast<int8_t*>(d_cw), d_orig);
+                                                    reinterpret_cast<int8_t*>(d_cw), d_orig, premul ? 2u : 0u);
             ChainView& v = p->chain;
             v.chunks = d_chunks; v.segs = d_segs; v.rel16 = d_rel; v.orig = d_orig; v.cidx = d_cidx; v.cw = d_cw;
             v.h0 = d_h0; v.old = d_old;
             v.n_chunks = (uint32_t)pl.chunks.size(); v.n_segs = (uint32_t)pl.segs.size();
             v.n_t = n_t; v.n_t_pad = n_t_pad; v.row_lo = row_lo; v.resident = resident ? 1u : 0u;
-            v.buf_bytes = buf_bytes; v.threads = threads;
+            v.buf_bytes = buf_bytes; v.threads = threads; v.premul = premul ? 1u : 0u;
             v.narrow = (uint64_t)n_t * 2ull * (uint64_t)rep.absw_max < (1ull << 31) ? 1u : 0u;
             if (delta) {
                 p->chain_delta = true;
@@ -919,11 +921,9 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
                 p->chain_small = true;
                 p->small_threads = threads;
                 p->small_dyn = (size_t)val_bytes + (size_t)buf_bytes * (resident ? 1u : 2u);
-                // a throughput-bound small graph (its widest class gives every thread several rows) runs on a cluster of two
-                // CTAs per word: each updates half of every class and mirrors its words into the peer's shared memory
-                uint32_t widest = 0;
-                for (size_t j = 0; j + 1 < lvl.size(); ++j) widest = std::max(widest, lvl[j + 1] - lvl[j]);
-                p->small_csplit = (resident && widest >= 2u * threads && !(flags & ISING_LOAD_NO_CLUSTER)) ? 2u : 1u;
+                // a resident chain may run on clusters of two CTAs per word (levels + flip producer) when an anneal call
+                // leaves enough SMs free: decided per call
+                p->small_csplit = (resident && !(flags & ISING_LOAD_NO_CLUSTER)) ? 2u : 1u;
             }
             CKP(cudaStreamSynchronize(st));   // the plan's host vectors die here
         }
@@ -1076,7 +1076,17 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
         k_finish_energy<<<(unsigned)((tiles * kTile + 255) / 256), 256, 0, st>>>(p->sm.accum_eval, p->W, tiles * kTile,
                                                                               p->sm.E[0], nullptr);
         p->launches++;
-        CK(cudaFuncSetAttribute(k_anneal_small, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->small_dyn));
+        int dev_sms = 0;
+        {
+            int dev = 0;
+            CK(cudaGetDevice(&dev));
+            CK(cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, dev));
+        }
+        const uint32_t csplit = (p->small_csplit > 1u && 2 * (int64_t)tiles * kChainGroups <= (int64_t)dev_sms) ? 2u : 1u;
+        const void* small_fn = p->chain.premul
+            ? (p->timing ? (const void*)k_anneal_small<true, true> : (const void*)k_anneal_small<false, true>)
+            : (p->timing ? (const void*)k_anneal_small<true, false> : (const void*)k_anneal_small<false, false>);
+        CK(cudaFuncSetAttribute(small_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->small_dyn));
         for (int32_t s0 = 0; s0 < n_sweeps; s0 += (int32_t)kThrCap) {
             const int32_t ns = std::min<int32_t>((int32_t)kThrCap, n_sweeps - s0);
             CK(cudaMemcpyAsync(p->sm.thr, p->thr_host.data() + s0, 4 * (size_t)ns, cudaMemcpyHostToDevice, st));
@@ -1104,19 +1114,20 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
             a.timing = s0 == 0 ? p->timing : nullptr;
             a.timing_sweep = p->timing_sweep;
             a.keys = keys;
-            a.csplit = p->small_csplit;
+            a.csplit = csplit;
             {
                 cudaLaunchConfig_t cfg{};
-                cfg.gridDim = dim3((unsigned)(tiles * kChainGroups) * p->small_csplit);
+                cfg.gridDim = dim3((unsigned)(tiles * kChainGroups) * csplit);
                 cfg.blockDim = dim3(p->small_threads);
                 cfg.dynamicSmemBytes = p->small_dyn;
                 cfg.stream = st;
                 cudaLaunchAttribute at[1];
                 at[0].id = cudaLaunchAttributeClusterDimension;
-                at[0].val.clusterDim.x = p->small_csplit; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+                at[0].val.clusterDim.x = csplit; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
                 cfg.attrs = at;
-                cfg.numAttrs = p->small_csplit > 1u ? 1 : 0;
-                CK(cudaLaunchKernelEx(&cfg, k_anneal_small, a));
+                cfg.numAttrs = csplit > 1u ? 1 : 0;
+                void* args[1] = {&a};
+                CK(cudaLaunchKernelExC(&cfg, small_fn, args));
             }
             p->launches++;
         }

@@ -959,7 +959,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 ChainRt rt;
                 rt.thr = thr; rt.T = T; rt.rl0 = p.rep0 + ctile * kTile + 4u * cgrp; rt.tie_rule = p.tie_rule;
                 ChainGlobal cgl;
-                cgl.csplit = 1u; cgl.crank = 0u;
+
                 const size_t o = (size_t)ctile * p.tile_stride + (size_t)v.row_lo * kTile + 4u * cgrp;
                 cgl.state = p.state + o;
                 cgl.best = p.best + o;
@@ -967,7 +967,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 cgl.cap4 = (s_mask[ctile] >> (4u * cgrp)) & 15u;
                 long long cdE[4] = {0, 0, 0, 0};
                 const uint32_t cflip = gbuf_base + chain_align16(4u * v.n_t_pad);
-                chain_pass_streamed<true>(v, s_chunks, s_segs, gbuf_base, cflip, cflip + chain_align16(v.n_t_pad), cta, rt,
+                chain_pass_streamed<true, true>(v, s_chunks, s_segs, gbuf_base, cflip, cflip + chain_align16(v.n_t_pad), cta, rt,
                                           p.keys, cdE, cgl, threadIdx.x, (uint32_t)kSweepThreads, false,
                                           (tsw && cta == 0 && threadIdx.x == 0) ? p.timing : nullptr, n_cta * 8u);
                 chain_reduce_dE(cdE, s_cdE, threadIdx.x, v.narrow != 0u);

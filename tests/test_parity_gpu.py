@@ -410,6 +410,33 @@ def test_power_law_graph_with_and_without_tail_chain(engine, replicas, first):
     np.testing.assert_array_equal(g2["final"], oracle_anneal(wl, first_replica=first, n_threads=16)["final"])
 
 
+@pytest.mark.parametrize("flags", [0, P.ISING_LOAD_NO_CLUSTER])
+def test_small_graph_flip_producer_with_zero_threshold_sweeps(flags):
+    """Small-graph engine as a cluster of two CTAs per word (levels + flip producer) and as one CTA per word: sweeps
+    whose threshold is 0 draw nothing and hand no buffer over (both CTAs must keep the same count), a first replica
+    that is not a multiple of four takes two Philox calls per word, and a call continues where the last one stopped."""
+    wl = er_workload(700, 0.02, 91, "pm4", np.int8, 7, 24, seed=3, p0=0.3)
+    thr = wl.thr.copy()
+    thr[[0, 3, 4, 9, 10, 11, 17, 23]] = 0
+    g = gpu_anneal(wl, thr=thr, first_replica=5, flags=flags)
+    assert g["problem"].engine == P.ENGINE_SMALL and g["problem"].info(18) == (1 if flags else 2)
+    o = oracle_anneal(wl, thr=thr, first_replica=5)
+    assert_same(g, o)
+    g1 = gpu_anneal(wl, thr=thr[:10], first_replica=5, problem=g["problem"])
+    g2 = gpu_anneal(wl, thr=thr[10:], sweep_offset=10, first_replica=5, init_mode=P.ISING_INIT_CONTINUE, problem=g["problem"])
+    np.testing.assert_array_equal(g2["final"], o["final"])
+
+
+def test_small_graph_with_more_than_16k_rows_keeps_local_ids_in_its_cells():
+    """Chains of at most 16 384 rows keep byte offsets (id x 4) in their 16-bit cells; longer ones (the paper's largest
+    benchmark graphs have 20 000 vertices, Table III) keep local ids: the other instance of the kernel."""
+    wl = er_workload(20000, 0.0002, 13, "pm4", np.int8, 6, 10, seed=2, p0=0.2)
+    g = gpu_anneal(wl)
+    assert g["problem"].engine == P.ENGINE_SMALL
+    o = oracle_anneal(wl, n_threads=8)
+    assert_same(g, o)
+
+
 def test_small_graph_streamed_through_shared_memory():
     """A graph whose packed edges do not fit one CTA's shared memory but whose spins do: the chain engine streams the
     edge chunks through two buffers every sweep (several chunks, levels cut across chunks)."""
