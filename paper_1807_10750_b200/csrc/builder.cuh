@@ -12,6 +12,7 @@ struct BuildReport {
     int max_abs_w;             // max |w|
     long long w_sum;           // sum over directed entries (= 2 W)
     long long absw_max;        // max_i sum_j |w_ij|
+    long long kinds;           // entries towards a shorter row minus entries towards a longer row (0 in a symmetric graph)
 };
 
 __device__ __forceinline__ long long load_w(const void* w, int wtype, long long e) {
@@ -32,54 +33,195 @@ __global__ void k_check_rowptr(const long long* row_ptr, int32_t n, long long nn
     if (bad) atomicOr(&rep->err_mask, 1u << 2);
 }
 
-// One warp per row: column range / order / self loops, symmetry (binary search of the
-// mirrored entry), colouring, sum_j |w_ij|.
+// ---------------------------------------------------------------------------------------------
+// Relabelling on the device: internal row order = colour ascending, then degree descending, then caller id ascending
+// (the order the slices are cut from).  A stable LSD radix sort of the caller ids on the key
+//     colour << dbits | (2^dbits - 1 - degree),        dbits = bits of n - 1 (>= any degree),
+// eight bits a pass; the key is recomputed from row_ptr / colour in every pass (three gathers per row: nothing next to
+// the edge traffic of the load), so only the ids move.  Garbage row_ptr / colour values are clamped: the sort never
+// leaves its arrays, and the validation report rejects the graph afterwards.
+// ---------------------------------------------------------------------------------------------
+constexpr int kRadixChunk = 2048;   // rows per warp and pass
+
+struct RelabelKey {
+    const long long* row_ptr;
+    const int32_t* colour;   // or nullptr
+    int32_t n, n_colours;
+    uint32_t dbits;
+    __device__ __forceinline__ uint32_t degree(uint32_t v) const {
+        const long long d = row_ptr[v + 1] - row_ptr[v];
+        const long long cap = (1ll << dbits) - 1;
+        return (uint32_t)(d < 0 ? 0 : (d > cap ? cap : d));
+    }
+    __device__ __forceinline__ uint32_t colour_of(uint32_t v) const {
+        if (!colour) return 0u;
+        const int32_t c = colour[v];
+        return (uint32_t)(c < 0 ? 0 : (c >= n_colours ? n_colours - 1 : c));
+    }
+    __device__ __forceinline__ unsigned long long key(uint32_t v) const {
+        return ((unsigned long long)colour_of(v) << dbits) | (unsigned long long)(((1u << dbits) - 1u) - degree(v));
+    }
+};
+
+// ids == nullptr: the identity (first pass)
+__global__ void k_radix_hist(RelabelKey rk, const uint32_t* ids, uint32_t shift, uint32_t n_chunks, uint32_t* hist) {
+    __shared__ uint32_t s_cnt[4][256];
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
+    const uint32_t chunk = blockIdx.x * 4u + warp;
+    for (uint32_t d = lane; d < 256u; d += 32u) s_cnt[warp][d] = 0u;
+    __syncwarp();
+    if (chunk < n_chunks) {
+        const uint32_t lo = chunk * (uint32_t)kRadixChunk, hi = min((uint32_t)rk.n, lo + (uint32_t)kRadixChunk);
+        for (uint32_t k = lo + lane; k < hi; k += 32u) {
+            const uint32_t v = ids ? ids[k] : k;
+            atomicAdd(&s_cnt[warp][(uint32_t)(rk.key(v) >> shift) & 255u], 1u);
+        }
+        __syncwarp();
+        for (uint32_t d = lane; d < 256u; d += 32u) hist[(size_t)d * n_chunks + chunk] = s_cnt[warp][d];
+    }
+}
+// exclusive scan of hist[256 * n_chunks] in place (digit-major), one CTA
+__global__ void k_radix_scan(uint32_t* hist, uint32_t total) {
+    __shared__ uint32_t s_part[1024];
+    const uint32_t t = threadIdx.x, per = (total + 1023u) / 1024u;
+    const uint32_t lo = min(total, t * per), hi = min(total, lo + per);
+    uint32_t sum = 0;
+    for (uint32_t k = lo; k < hi; ++k) sum += hist[k];
+    s_part[t] = sum;
+    __syncthreads();
+    for (uint32_t o = 1; o < 1024u; o <<= 1) {
+        const uint32_t x = t >= o ? s_part[t - o] : 0u;
+        __syncthreads();
+        s_part[t] += x;
+        __syncthreads();
+    }
+    uint32_t run = s_part[t] - sum;
+    for (uint32_t k = lo; k < hi; ++k) {
+        const uint32_t c = hist[k];
+        hist[k] = run;
+        run += c;
+    }
+}
+// stable scatter: a warp walks its chunk in order, 32 rows a step; rows of one digit keep their order (match_any)
+__global__ void k_radix_scatter(RelabelKey rk, const uint32_t* ids, uint32_t* out, uint32_t shift, uint32_t n_chunks,
+                                const uint32_t* offs) {
+    __shared__ uint32_t s_off[4][256];
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
+    const uint32_t chunk = blockIdx.x * 4u + warp;
+    if (chunk >= n_chunks) return;
+    for (uint32_t d = lane; d < 256u; d += 32u) s_off[warp][d] = offs[(size_t)d * n_chunks + chunk];
+    __syncwarp();
+    const uint32_t lo = chunk * (uint32_t)kRadixChunk, hi = min((uint32_t)rk.n, lo + (uint32_t)kRadixChunk);
+    for (uint32_t k0 = lo; k0 < hi; k0 += 32u) {
+        const uint32_t k = k0 + lane;
+        const bool act = k < hi;
+        const uint32_t v = act ? (ids ? ids[k] : k) : 0u;
+        const uint32_t d = act ? (uint32_t)(rk.key(v) >> shift) & 255u : 256u + lane;   // (idle lanes: a group of their own)
+        const uint32_t m = __match_any_sync(0xffffffffu, d);
+        const uint32_t rank = __popc(m & ((1u << lane) - 1u));
+        if (act) out[s_off[warp][d] + rank] = v;
+        __syncwarp();
+        if (act && rank == 0u) s_off[warp][d] += __popc(m);
+        __syncwarp();
+    }
+}
+// perm -> inv, and the runs of equal (colour, degree) along the internal order: (first row, colour, degree), unordered
+struct RelabelRuns {
+    unsigned int count;
+    unsigned int pad;
+};
+__global__ void k_relabel_finish(RelabelKey rk, const uint32_t* perm, int32_t* inv, RelabelRuns* runs, uint32_t* run_rows,
+                                 uint32_t cap) {
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= (uint32_t)rk.n) return;
+    const uint32_t v = perm[k];
+    inv[v] = (int32_t)k;
+    const unsigned long long key = rk.key(v);
+    if (k == 0u || rk.key(perm[k - 1u]) != key) {
+        const uint32_t at = atomicAdd(&runs->count, 1u);
+        if (at < cap) {
+            run_rows[3u * at] = k;
+            run_rows[3u * at + 1u] = (uint32_t)(key >> rk.dbits);
+            run_rows[3u * at + 2u] = ((1u << rk.dbits) - 1u) - (uint32_t)(key & ((1ull << rk.dbits) - 1ull));
+        }
+    }
+}
+
+// One warp per row: column range / order / self loops, symmetry, colouring, sum_j |w_ij|.
+// Symmetry: entry (i, j) is looked up in row j (binary search) only when row j is not longer than row i; the entries
+// whose row j is longer are counted instead.  Every looked-up entry of the first kind (deg j < deg i) names a distinct
+// entry of the second kind as its mirror, so "all look-ups succeed and both kinds are equally many" means that every
+// entry has its mirror with the same weight -- and the searches run in the SHORT rows (a power-law graph's edges
+// mostly lead to hubs, whose rows cost 14-17 dependent probes each).
 __global__ void k_validate(int32_t n, const long long* row_ptr, const int32_t* col, const void* w, int wtype,
                            const int32_t* colour, int32_t n_colours, BuildReport* rep) {
+    __shared__ unsigned int s_err;
+    __shared__ int s_maxabs;
+    __shared__ long long s_absw, s_wsum, s_kinds;
+    if (threadIdx.x == 0) { s_err = 0u; s_maxabs = 0; s_absw = 0; s_wsum = 0; s_kinds = 0; }
+    __syncthreads();
     const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
-    if (gw >= n) return;
-    const int32_t i = (int32_t)gw;
-    const long long b = row_ptr[i], e = row_ptr[i + 1];
     unsigned int err = 0;
-    long long absw = 0, wsum = 0;
+    long long absw = 0, wsum = 0, kinds = 0;   // kinds: entries towards a shorter row minus entries towards a longer one
     int maxabs = 0;
-    int ci = 0;
-    if (colour) {
-        ci = colour[i];
-        if (ci < 0 || ci >= n_colours) err |= 1u << 6;
-    }
-    for (long long idx = b + lane; idx < e; idx += 32) {
-        const int32_t j = col[idx];
-        if (j < 0 || j >= n) { err |= 1u << 2; continue; }
-        if (j == i) err |= 1u << 4;
-        if (idx > b && col[idx - 1] >= j) err |= 1u << 3;
-        const long long wv = load_w(w, wtype, idx);
-        long long lo = row_ptr[j], hi = row_ptr[j + 1];   // find i in row j
-        while (lo < hi) {
-            const long long mid = (lo + hi) >> 1;
-            if (col[mid] < i) lo = mid + 1; else hi = mid;
+    if (gw < n) {
+        const int32_t i = (int32_t)gw;
+        const long long b = row_ptr[i], e = row_ptr[i + 1];
+        int ci = 0;
+        if (colour) {
+            ci = colour[i];
+            if (ci < 0 || ci >= n_colours) err |= 1u << 6;
         }
-        if (lo >= row_ptr[j + 1] || col[lo] != i || load_w(w, wtype, lo) != wv) err |= 1u << 5;
-        if (colour && colour[j] == ci) err |= 1u << 6;
-        const long long aw = wv < 0 ? -wv : wv;
-        absw += aw;
-        wsum += wv;
-        if (aw > maxabs) maxabs = (int)(aw > 0x7fffffffll ? 0x7fffffffll : aw);
+        for (long long idx = b + lane; idx < e; idx += 32) {
+            const int32_t j = col[idx];
+            if (j < 0 || j >= n) { err |= 1u << 2; continue; }
+            if (j == i) err |= 1u << 4;
+            if (idx > b && col[idx - 1] >= j) err |= 1u << 3;
+            const long long wv = load_w(w, wtype, idx);
+            long long lo = row_ptr[j];
+            const long long end_j = row_ptr[j + 1];
+            if (end_j - lo > e - b) {
+                --kinds;
+            } else {
+                if (end_j - lo < e - b) ++kinds;
+                long long hi = end_j;   // find i in row j
+                while (lo < hi) {
+                    const long long mid = (lo + hi) >> 1;
+                    if (col[mid] < i) lo = mid + 1; else hi = mid;
+                }
+                if (lo >= end_j || col[lo] != i || load_w(w, wtype, lo) != wv) err |= 1u << 5;
+            }
+            if (colour && colour[j] == ci) err |= 1u << 6;
+            const long long aw = wv < 0 ? -wv : wv;
+            absw += aw;
+            wsum += wv;
+            if (aw > maxabs) maxabs = (int)(aw > 0x7fffffffll ? 0x7fffffffll : aw);
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         absw += __shfl_xor_sync(0xffffffffu, absw, o);
         wsum += __shfl_xor_sync(0xffffffffu, wsum, o);
+        kinds += __shfl_xor_sync(0xffffffffu, kinds, o);
         maxabs = max(maxabs, __shfl_xor_sync(0xffffffffu, maxabs, o));
         err |= __shfl_xor_sync(0xffffffffu, err, o);
     }
-    if (lane == 0) {
-        if (err) atomicOr(&rep->err_mask, err);
-        if (absw >= (1ll << 31)) atomicOr(&rep->err_mask, 1u << 7);
-        atomicMax(&rep->absw_max, absw);
-        atomicMax(&rep->max_abs_w, maxabs);
-        if (wsum != 0) atomicAdd(reinterpret_cast<unsigned long long*>(&rep->w_sum), (unsigned long long)wsum);
+    if (lane == 0) {   // the rows of a block meet in shared memory: one set of global atomics per block
+        if (absw >= (1ll << 31)) err |= 1u << 7;
+        if (err) atomicOr(&s_err, err);
+        atomicMax(&s_absw, absw);
+        atomicMax(&s_maxabs, maxabs);
+        if (wsum != 0) atomicAdd(reinterpret_cast<unsigned long long*>(&s_wsum), (unsigned long long)wsum);
+        if (kinds != 0) atomicAdd(reinterpret_cast<unsigned long long*>(&s_kinds), (unsigned long long)kinds);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (s_err) atomicOr(&rep->err_mask, s_err);
+        atomicMax(&rep->absw_max, s_absw);
+        atomicMax(&rep->max_abs_w, s_maxabs);
+        if (s_wsum != 0) atomicAdd(reinterpret_cast<unsigned long long*>(&rep->w_sum), (unsigned long long)s_wsum);
+        if (s_kinds != 0) atomicAdd(reinterpret_cast<unsigned long long*>(&rep->kinds), (unsigned long long)s_kinds);
     }
 }
 

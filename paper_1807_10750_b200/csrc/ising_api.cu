@@ -7,6 +7,8 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <chrono>
+#include <cstdio>
 #include <cstdint>
 #include <cstring>
 #include <new>
@@ -109,6 +111,10 @@ size_t workspace_need(int64_t n, int64_t nnz, int wtype, int64_t max_replicas, i
     }
     add(4 * (size_t)n);                       // perm
     add(4 * (size_t)n);                       // inv
+    add(4 * (size_t)n);                       // relabelling: second id buffer
+    add(4 * 256 * (size_t)((n + kRadixChunk - 1) / kRadixChunk));   // digit histograms
+    add(sizeof(RelabelRuns));
+    add(12 * (size_t)n);                      // runs of equal (colour, degree)
     add(sizeof(SliceDesc) * (size_t)(n_slices + 1));
     add(4 * 16 * (size_t)(n_slices + 1));     // sorig
     add(8 * (size_t)(n_slices + 1));          // slice_aux
@@ -461,12 +467,26 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
     if ((reinterpret_cast<uintptr_t>(workspace) & (kAlign - 1)) != 0 || !is_device_ptr(workspace))
         return ISING_ERR_BAD_SHAPE;   // not 256-byte aligned device memory
     cudaStream_t st = (cudaStream_t)stream;
+#ifdef ISING_TUNING_ENV
+    const bool lt_on = getenv("ISING_LOAD_TIMING") != nullptr;
+    auto lt_t0 = std::chrono::steady_clock::now();
+    auto LT = [&](const char* what) {
+        if (!lt_on) return;
+        if (getenv("ISING_LOAD_TIMING_SYNC")) cudaStreamSynchronize(st);
+        auto t = std::chrono::steady_clock::now();
+        fprintf(stderr, "  [load] %-28s %8.3f ms\n", what, std::chrono::duration<double, std::milli>(t - lt_t0).count());
+        lt_t0 = t;
+    };
+#else
+    auto LT = [](const char*) {};
+#endif
 
     Bump ws{(uint8_t*)workspace, workspace_bytes, 0, false};
     BuildReport* d_rep = (BuildReport*)ws.take(sizeof(BuildReport));
     if (ws.overflow) return ISING_ERR_WORKSPACE_TOO_SMALL;
 
-    // ---- bring the raw CSR to the device (staged in the workspace when it is host memory)
+    // ---- bring the raw CSR to the device (staged in the workspace when it is host memory): row_ptr and colour first,
+    // the relabelling needs nothing else
     const bool rp_dev = is_device_ptr(row_ptr), ci_dev = nnz == 0 || is_device_ptr(col_idx);
     const bool w_dev = nnz == 0 || is_device_ptr(weights), co_dev = colour && is_device_ptr(colour);
     const long long* d_row_ptr = (const long long*)row_ptr;
@@ -479,6 +499,55 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         CK(cudaMemcpyAsync(b, row_ptr, 8 * (size_t)(n + 1), cudaMemcpyHostToDevice, st));
         d_row_ptr = (const long long*)b;
     }
+    if (colour && !co_dev) {
+        void* b = ws.take(4 * (size_t)n);
+        if (!b) return ISING_ERR_WORKSPACE_TOO_SMALL;
+        CK(cudaMemcpyAsync(b, colour, 4 * (size_t)n, cudaMemcpyHostToDevice, st));
+        d_colour = (const int32_t*)b;
+    }
+    CK(cudaMemsetAsync(d_rep, 0, sizeof(BuildReport), st));
+    k_check_rowptr<<<(unsigned)((n + 1 + 255) / 256), 256, 0, st>>>(d_row_ptr, n, nnz, d_rep);
+
+    // ---- relabelling on the device (builder.cuh), on a stream of its own: it overlaps the copies of col_idx / weights
+    const int32_t C = n_colours > 0 ? n_colours : 1;
+    struct Side {   // the side stream and its fork event
+        cudaStream_t s = nullptr;
+        cudaEvent_t e = nullptr;
+        ~Side() { if (s) (void)cudaStreamSynchronize(s); if (e) cudaEventDestroy(e); if (s) cudaStreamDestroy(s); }   // (its work reads the workspace)
+    } side;
+    CK(cudaStreamCreateWithFlags(&side.s, cudaStreamNonBlocking));
+    CK(cudaEventCreateWithFlags(&side.e, cudaEventDisableTiming));
+    CK(cudaEventRecord(side.e, st));
+    CK(cudaStreamWaitEvent(side.s, side.e, 0));
+    auto bits_of = [](uint64_t x) { uint32_t b = 0; while (x) { ++b; x >>= 1; } return b; };
+    RelabelKey rk{};
+    rk.row_ptr = d_row_ptr; rk.colour = d_colour; rk.n = n; rk.n_colours = C;
+    rk.dbits = std::max(1u, bits_of((uint64_t)(n - 1)));
+    const uint32_t key_bits = rk.dbits + bits_of((uint64_t)(C - 1));
+    const uint32_t passes = std::max(1u, (key_bits + 7u) / 8u);
+    const uint32_t n_chunks = (uint32_t)(((int64_t)n + kRadixChunk - 1) / kRadixChunk);
+    int32_t* d_perm = (int32_t*)ws.take(4 * (size_t)n);
+    int32_t* d_inv = (int32_t*)ws.take(4 * (size_t)n);
+    uint32_t* d_ids = (uint32_t*)ws.take(4 * (size_t)n);
+    uint32_t* d_hist = (uint32_t*)ws.take(4 * 256 * (size_t)n_chunks);
+    RelabelRuns* d_runs = (RelabelRuns*)ws.take(sizeof(RelabelRuns));
+    uint32_t* d_run_rows = (uint32_t*)ws.take(12 * (size_t)n);
+    if (ws.overflow) return ISING_ERR_WORKSPACE_TOO_SMALL;
+    {
+        const unsigned cb = (n_chunks + 3u) / 4u;
+        const uint32_t* src = nullptr;
+        for (uint32_t ps = 0; ps < passes; ++ps) {   // (the last pass lands in d_perm)
+            uint32_t* dst = ((passes - ps) & 1u) ? (uint32_t*)d_perm : d_ids;
+            k_radix_hist<<<cb, 128, 0, side.s>>>(rk, src, 8u * ps, n_chunks, d_hist);
+            k_radix_scan<<<1, 1024, 0, side.s>>>(d_hist, 256u * n_chunks);
+            k_radix_scatter<<<cb, 128, 0, side.s>>>(rk, src, dst, 8u * ps, n_chunks, d_hist);
+            src = dst;
+        }
+        CK(cudaMemsetAsync(d_runs, 0, sizeof(RelabelRuns), side.s));
+        k_relabel_finish<<<(unsigned)((n + 255) / 256), 256, 0, side.s>>>(rk, (const uint32_t*)d_perm, d_inv, d_runs, d_run_rows,
+                                                                         (uint32_t)n);
+    }
+    // (meanwhile, on the caller's stream: the edges)
     if (!ci_dev) {
         void* b = ws.take(4 * (size_t)nnz);
         if (!b) return ISING_ERR_WORKSPACE_TOO_SMALL;
@@ -491,34 +560,24 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         CK(cudaMemcpyAsync(b, weights, (size_t)wtype * (size_t)nnz, cudaMemcpyHostToDevice, st));
         d_w = b;
     }
-    if (colour && !co_dev) {
-        void* b = ws.take(4 * (size_t)n);
-        if (!b) return ISING_ERR_WORKSPACE_TOO_SMALL;
-        CK(cudaMemcpyAsync(b, colour, 4 * (size_t)n, cudaMemcpyHostToDevice, st));
-        d_colour = (const int32_t*)b;
-    }
-
-    // ---- validate on the device.  With host inputs the O(n) planning below does not wait for it: the copies and
-    // k_validate run while the host plans (row_ptr and colour are range-checked on the host first, because the
-    // planning indexes with them); the report is read before anything is packed.
-    const bool plan_early = !rp_dev && (!colour || !co_dev);
-    if (plan_early) {
-        const int64_t* rp = row_ptr;
-        bool bad = rp[0] != 0 || rp[n] != nnz;
-        for (int32_t i = 0; i < n && !bad; ++i) bad = rp[i + 1] < rp[i] || rp[i] < 0 || rp[i + 1] > nnz || rp[i + 1] - rp[i] > (int64_t)n - 1;
-        if (bad) return ISING_ERR_BAD_SHAPE;
-        if (colour)
-            for (int32_t i = 0; i < n; ++i)
-                if (colour[i] < 0 || colour[i] >= n_colours) return ISING_ERR_BAD_COLOURING;
-    }
-    CK(cudaMemsetAsync(d_rep, 0, sizeof(BuildReport), st));
-    k_check_rowptr<<<(unsigned)((n + 1 + 255) / 256), 256, 0, st>>>(d_row_ptr, n, nnz, d_rep);
+    LT("copies + relabel enqueued");
+    // the one small read-back of the planning: row_ptr verdict + the runs of equal (colour, degree)
     BuildReport rep{};
-    if (!plan_early) {
-        CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, st));
-        CK(cudaStreamSynchronize(st));
-        if (rep.err_mask) return ISING_ERR_BAD_SHAPE;
+    RelabelRuns runs_hdr{};
+    const size_t runs_first = std::min<size_t>((size_t)n, 32768);
+    std::vector<uint32_t> run_rows(3 * runs_first);
+    CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, side.s));
+    CK(cudaMemcpyAsync(&runs_hdr, d_runs, sizeof(runs_hdr), cudaMemcpyDeviceToHost, side.s));
+    CK(cudaMemcpyAsync(run_rows.data(), d_run_rows, 12 * runs_first, cudaMemcpyDeviceToHost, side.s));
+    CK(cudaStreamSynchronize(side.s));
+    CK(cudaGetLastError());
+    if (rep.err_mask) { (void)cudaStreamSynchronize(st); return ISING_ERR_BAD_SHAPE; }   // (the copies read the caller's arrays)
+    if (runs_hdr.count > runs_first) {
+        run_rows.resize(3 * (size_t)runs_hdr.count);
+        CK(cudaMemcpy(run_rows.data(), d_run_rows, 12 * (size_t)runs_hdr.count, cudaMemcpyDeviceToHost));
     }
+    LT("relabel done (runs on host)");
+    // ---- validate on the device (row_ptr is sound from here on); the report is read before anything is packed
     {
         const long long warps = n;
         const unsigned blocks = (unsigned)((warps * 32 + 255) / 256);
@@ -528,61 +587,34 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
         CK(cudaGetLastError());
+        if (rep.kinds != 0) rep.err_mask |= 1u << ISING_ERR_ASYMMETRIC;   // (k_validate: an entry without a mirror in a longer row)
         for (int code : {ISING_ERR_BAD_SHAPE, ISING_ERR_UNSORTED_OR_DUP, ISING_ERR_SELF_LOOP, ISING_ERR_ASYMMETRIC,
                          ISING_ERR_BAD_COLOURING, ISING_ERR_FIELD_OVERFLOW})
             if (rep.err_mask & (1u << code)) return code;
         return ISING_OK;
     };
-    if (!plan_early)
-        if (ising_status s = read_report()) return s;
 
-    // ---- O(n) planning on the host: relabelling and slices
-    std::vector<int64_t> rp_copy;
-    std::vector<int32_t> co_copy;
-    const int64_t* h_row_ptr = row_ptr;
-    const int32_t* h_colour = colour;
-    if (rp_dev) {
-        rp_copy.resize((size_t)n + 1);
-        CK(cudaMemcpy(rp_copy.data(), row_ptr, 8 * (size_t)(n + 1), cudaMemcpyDeviceToHost));
-        h_row_ptr = rp_copy.data();
-    }
-    if (colour && co_dev) {
-        co_copy.resize((size_t)n);
-        CK(cudaMemcpy(co_copy.data(), colour, 4 * (size_t)n, cudaMemcpyDeviceToHost));
-        h_colour = co_copy.data();
-    }
-    const int32_t C = n_colours > 0 ? n_colours : 1;
-    std::vector<int32_t> perm(n), inv(n);
-    std::vector<int32_t> dsort(n);                       // degree of internal row k
+    // ---- O(slices) planning on the host, from the runs: internal rows [run_start[q], run_start[q + 1]) have degree
+    // run_deg[q]; a run never crosses a colour boundary
+    const size_t n_runs = runs_hdr.count;
+    std::vector<int64_t> run_start(n_runs + 1), run_deg(n_runs + 1, 0);
     std::vector<int64_t> cstart((size_t)C + 1, 0);       // internal rows of colour c: [cstart[c], cstart[c+1])
     {
-        // stable counting sorts: by degree descending, then by colour ascending
-        std::vector<int32_t> deg(n);
-        int64_t dmax = 0;
-        for (int32_t i = 0; i < n; ++i) {
-            const int64_t d = h_row_ptr[i + 1] - h_row_ptr[i];
-            deg[i] = (int32_t)d;
-            dmax = std::max(dmax, d);
+        std::vector<uint64_t> order(n_runs);             // (first row << 32 | run index), sorted by first row
+        for (size_t q = 0; q < n_runs; ++q) order[q] = ((uint64_t)run_rows[3 * q] << 32) | q;
+        std::sort(order.begin(), order.end());
+        for (size_t q = 0; q < n_runs; ++q) {
+            const size_t r = (size_t)(order[q] & 0xffffffffu);
+            const int64_t k0 = run_rows[3 * r], k1 = q + 1 < n_runs ? (int64_t)(order[q + 1] >> 32) : (int64_t)n;
+            const uint32_t c = std::min<uint32_t>(run_rows[3 * r + 1], (uint32_t)C - 1u);
+            run_start[q] = k0;
+            run_deg[q] = run_rows[3 * r + 2];
+            cstart[(size_t)c + 1] += k1 - k0;
         }
-        std::vector<int32_t> cnt((size_t)dmax + 2, 0);
-        for (int32_t i = 0; i < n; ++i) cnt[(size_t)(dmax - deg[i]) + 1]++;
-        for (size_t k = 1; k < cnt.size(); ++k) cnt[k] += cnt[k - 1];
-        std::vector<int32_t> by_deg(n);
-        for (int32_t i = 0; i < n; ++i) by_deg[(size_t)cnt[(size_t)(dmax - deg[i])]++] = i;
-        if (h_colour)
-            for (int32_t i = 0; i < n; ++i) cstart[(size_t)h_colour[i] + 1]++;
-        else
-            cstart[1] = n;
+        run_start[n_runs] = n;
         for (size_t k = 1; k < cstart.size(); ++k) cstart[k] += cstart[k - 1];
-        std::vector<int64_t> cc(cstart.begin(), cstart.end() - 1);
-        for (int32_t k = 0; k < n; ++k) {
-            const int32_t i = by_deg[k];
-            const int64_t at = cc[h_colour ? (size_t)h_colour[i] : 0]++;
-            perm[(size_t)at] = i;
-            dsort[(size_t)at] = deg[i];
-            inv[i] = (int32_t)at;
-        }
     }
+    LT("runs sorted");
     // ---- work units: hubs (rows above kHubDegree, one CTA each) and slices (one warp each)
     int sm_count = 148, coop = 0;
     {
@@ -593,11 +625,12 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
     }
     std::vector<SliceDesc> slices;
     std::vector<uint32_t> slice_aux;                            // per slice: (hub id, part index) of hub-part slices
+    slices.reserve((size_t)n / 3 + 1024);
+    slice_aux.reserve(2 * ((size_t)n / 3 + 1024));
     std::vector<uint32_t> slice_begin((size_t)C + 1, 0);
     uint64_t tail_cells = 0;
     uint32_t n_hub_rows = 0;
     bool too_many_parts = false;
-    auto degree_of = [&](int32_t k) { return (int64_t)dsort[k]; };
     // Edges per sub-row before a row is split over more sub-rows: 16 keeps the instruction count per edge low
     // (throughput-bound colour phases); 8 keeps every row inside the prefetched head cells, i.e. one gather round
     // trip per phase (latency-bound phases: fewer units than HALF the warps on the GPU; measured on config 5 in ms
@@ -608,8 +641,11 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
     auto emit_colour = [&](int32_t c, int32_t k, int sub_row_edges) {   // rows k.. of colour c -> slices; returns the next row
         const int64_t part_cells_max = (int64_t)kSubRows * (sub_row_edges / 4);
         const int32_t k_end = (int32_t)cstart[(size_t)c + 1];
+        size_t ri = (size_t)(std::upper_bound(run_start.begin(), run_start.end(), (int64_t)k) - run_start.begin()) - 1;   // run of row k
+        int64_t same_l_end = k;   // rows [k, same_l_end) share this row's sub-row split
         while (k < k_end) {
-            const int64_t deg = degree_of(k);
+            while (run_start[ri + 1] <= k) ++ri;
+            const int64_t deg = run_deg[ri];
             const int64_t groups = (deg + 3) / 4;
             if (groups > part_cells_max) {
                 // parts of at most 128 edges in every phase: a part lives in the prefetched head cells alone (measured
@@ -635,9 +671,12 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
             }
             const int l = spr_log2_for_degree(deg, sub_row_edges);
             const int rps = kSubRows >> l;
-            int nr = 1;
-            while (nr < rps && k + nr < k_end && spr_log2_for_degree(degree_of(k + nr), sub_row_edges) == l)
-                ++nr;
+            if (same_l_end <= k) {   // (degrees descend inside a colour: the rows of one split are a stretch of runs)
+                size_t rj = ri + 1;
+                while (run_start[rj] < k_end && spr_log2_for_degree(run_deg[rj], sub_row_edges) == l) ++rj;
+                same_l_end = std::min<int64_t>(run_start[rj], k_end);
+            }
+            const int nr = (int)std::min<int64_t>(rps, same_l_end - k);
             const int64_t G = std::max<int64_t>(1, (groups + (1ll << l) - 1) >> l);
             SliceDesc d;
             d.off = 0;
@@ -682,6 +721,7 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         slice_begin[C] = (uint32_t)slices.size();
         for (const SliceDesc& d : slices) tail_cells += (uint64_t)(d.G > (uint32_t)kHeadGroups ? d.G - kHeadGroups : 0u) * kSubRows;
     }
+    LT("slices");
     if (too_many_parts) { (void)cudaStreamSynchronize(st); return ISING_ERR_BAD_SHAPE; }   // the copies read the caller's arrays
     const uint64_t head_cells = (uint64_t)slices.size() * kSubRows * kHeadGroups;
     const uint64_t cells = head_cells + tail_cells;
@@ -741,8 +781,9 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         }
     }
 
-    if (plan_early)
-        if (ising_status s = read_report()) return s;
+    LT("ranges");
+    if (ising_status s = read_report()) return s;
+    LT("wait for validation report");
     const bool wide = rep.max_abs_w > 127 || (uint64_t)rep.absw_max * 2ull >= (1ull << 31);
     const bool complete = n >= 2 && nnz == (int64_t)n * (n - 1);
     const bool want_dense = kDenseEnabled && complete && !(flags & ISING_LOAD_NO_DENSE) && rep.max_abs_w <= 127;
@@ -761,8 +802,8 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
                          : (uint32_t)std::max<int64_t>(1, ((1ll << 31) - 1) / std::max<int64_t>(1, 2 * rep.absw_max));
 
     const size_t tiles = (size_t)p->tiles_max;
-    p->perm = (int32_t*)ws.take(4 * (size_t)n);
-    p->inv = (int32_t*)ws.take(4 * (size_t)n);
+    p->perm = d_perm;
+    p->inv = d_inv;
     p->slices = (SliceDesc*)ws.take(sizeof(SliceDesc) * (slices.size() + 1));
     p->sorig = (uint32_t*)ws.take(4 * kSubRows * (slices.size() + 1));
     p->slice_aux = (uint32_t*)ws.take(8 * (slices.size() + 1));
@@ -800,8 +841,6 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
 
     auto fail = [&](ising_status s) { delete p; return s; };
 #define CKP(call) do { if ((call) != cudaSuccess) { (void)cudaGetLastError(); return fail(ISING_ERR_CUDA); } } while (0)
-    CKP(cudaMemcpyAsync(p->perm, perm.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
-    CKP(cudaMemcpyAsync(p->inv, inv.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
     CKP(cudaMemcpyAsync(p->ranges, ranges.data(), sizeof(PhaseRange) * ranges.size(), cudaMemcpyHostToDevice, st));
     CKP(cudaMemcpyAsync(p->phase_slices, slice_begin.data(), 4 * ((size_t)C + 1), cudaMemcpyHostToDevice, st));
     if (!slices.empty()) {
@@ -818,6 +857,7 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         if (!p->dense) return fail(ISING_ERR_CUDA);
     }
 
+    LT("uploads + pack enqueued");
     // ---- chain engine (chain.cuh): the whole graph (k_anneal_small) or the tail classes of the persistent kernel
     p->vphase_slices = (uint32_t*)ws.take(4 * ((size_t)C + 2));
     if (ws.overflow) return fail(ISING_ERR_WORKSPACE_TOO_SMALL);
@@ -928,6 +968,7 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
             CKP(cudaStreamSynchronize(st));   // the plan's host vectors die here
         }
     }
+    LT("chain plan + build");
     {
         // virtual phases of the persistent kernel: the colour phases, or (tail chain) the phases before the tail plus
         // ONE bulk pseudo-phase holding every slice of the tail classes
@@ -944,6 +985,7 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
     CKP(cudaFuncSetAttribute(k_anneal_gs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
     CKP(cudaStreamSynchronize(st));   // the host vectors die at return
     CKP(cudaGetLastError());
+    LT("final sync");
 #undef CKP
     *out = p;
     return ISING_OK;

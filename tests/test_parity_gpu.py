@@ -232,6 +232,22 @@ def test_isolated_vertices_and_empty_graph():
     assert np.all(g["trace"] == 0)
 
 
+def test_device_relabelling_with_more_degree_runs_than_the_first_read_back():
+    """a1 relabels on the device (radix sort of the rows by colour, degree) and reads back only the runs of equal
+    (colour, degree); more than 32 768 runs take a second copy.  A ring in which every vertex has a colour of its own
+    (a proper colouring) has one run per vertex; also a load from device-resident inputs."""
+    n = 40000
+    u = np.arange(n, dtype=np.int64)
+    v = (u + 1) % n
+    wt = W.weights_from_hash(W.hash_pairs(5, np.minimum(u, v), np.maximum(u, v)), "pm4")
+    csr = W.csr_from_edges(n, u, v, wt, np.int8)
+    colour = np.random.default_rng(1).permutation(n).astype(np.int32)
+    wl = wl_from_csr(n, csr, colour, n, 2, W.linear_schedule(0.2, 0.0, 2), seed=8)
+    o = oracle_anneal(wl)
+    assert_same(gpu_anneal(wl), o)
+    assert_same(gpu_anneal(wl, device_inputs=True), o)
+
+
 def test_n_sweeps_zero_only_initialises():
     wl = er_workload(300, 0.05, 71, "pm1", np.int8, 4, 0)
     g = gpu_anneal(wl, thr=np.zeros(0, dtype=np.uint32))
@@ -285,6 +301,34 @@ def test_load_errors():
     with pytest.raises(P.IsingError) as e:
         P.ising_best_state(p, 0)
     assert e.value.status == 14
+
+
+def _drop_entry(rp, col, w, i, j):
+    """CSR without the directed entry (i, j)."""
+    at = int(rp[i]) + int(np.searchsorted(col[rp[i]:rp[i + 1]], j))
+    assert col[at] == j
+    rp2 = rp.copy(); rp2[i + 1:] -= 1
+    return rp2, np.delete(col, at), np.delete(w, at)
+
+
+def test_asymmetry_is_found_whichever_row_is_longer():
+    """k_validate looks an entry (i, j) up only in rows j that are not longer than row i and counts the entries of the two
+    other kinds against each other (builder.cuh): a missing mirror must be reported from either side, also between rows
+    of equal length, and so must a mirror with another weight."""
+    n = 40
+    u = np.concatenate([np.zeros(30, dtype=np.int64), np.array([31, 32, 33, 34])])      # a hub (0 - 1..30), a path 31-32-33-34-35
+    v = np.concatenate([np.arange(1, 31, dtype=np.int64), np.array([32, 33, 34, 35])])
+    wt = np.arange(1, 35) % 7 + 1
+    rp, col, w = W.csr_from_edges(n, u, v, wt, np.int8)
+    assert _load_status(rp, col, w) == 0
+    assert _load_status(*_drop_entry(rp, col, w, 0, 7)) == 5       # the entry in the LONG row is missing
+    assert _load_status(*_drop_entry(rp, col, w, 7, 0)) == 5       # the entry in the SHORT row is missing
+    assert _load_status(*_drop_entry(rp, col, w, 32, 33)) == 5     # rows of equal length (the path's inner vertices)
+    assert _load_status(*_drop_entry(rp, col, w, 33, 32)) == 5
+    for (i, j) in [(0, 7), (7, 0), (32, 33)]:
+        a = w.copy()
+        a[int(rp[i]) + int(np.searchsorted(col[rp[i]:rp[i + 1]], j))] += 1
+        assert _load_status(rp, col, a) == 5
 
 
 def test_run_twice_is_bit_identical():
