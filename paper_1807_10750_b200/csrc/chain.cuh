@@ -187,7 +187,9 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
 // One segment: every row takes its energy-minimising value (L47-49, Q1/Q3), the scheduled flip (L177), and its
 // energy increment dE = (a - s) h is added to dE[] (a7; exact because a colour class is an independent set).
 // PREMUL: the cells hold BYTE offsets into val[] (local id x 4: chains of at most 16 384 rows), not local ids.
-template <bool DELTA, bool PREMUL>
+// N32: the energy increments of a thread's rows are added up in 32 bits inside the segment (the chain is `narrow`: all
+// its sums fit) and widened once at the end: one IMAD per value (segments of several rows per thread).
+template <bool DELTA, bool PREMUL, bool N32 = false>
 __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChunk& ck, uint32_t buf, uint32_t val,
                                               uint32_t flip, const ChainRt& rt, const PhiloxKeys& keys, long long (&dE)[4],
                                               const ChainGlobal& cg, uint32_t tid, uint32_t nthr) {
@@ -196,6 +198,7 @@ __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChun
     const ChunkLayout l = chunk_layout(ck.r1 - ck.r0, ck.c1 - ck.c0, DELTA);
     const uint32_t s_lo = sg.r0, s_hi = sg.r1;
     const uint32_t fmask = rt.thr != 0u ? 15u : 0u;
+    int e0s = 0, e1s = 0, e2s = 0, e3s = 0;
     uint32_t r = s_lo + (tid >> logL);
     for (uint32_t rw = s_lo + ((tid & ~31u) >> logL); rw < s_hi; rw += rpi, r += rpi) {   // warp-uniform trip count
         // every lane runs the whole update on a valid row (no divergence); the first lane of a live row stores it
@@ -252,10 +255,14 @@ __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChun
         }
         a ^= ((f4 * 0x00204081u) & 0x01010101u) * 0xfeu;
         const uint32_t d2 = storer ? (a << 1) & (a ^ oldw) : 0u;  // a - s per byte: 0, +2, -2
-        asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[0]) : "r"(sbyte(d2, 0)), "r"(h0));
-        asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[1]) : "r"(sbyte(d2, 1)), "r"(h1));
-        asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[2]) : "r"(sbyte(d2, 2)), "r"(h2));
-        asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[3]) : "r"(sbyte(d2, 3)), "r"(h3));
+        if (N32) {
+            e0s += sbyte(d2, 0) * h0; e1s += sbyte(d2, 1) * h1; e2s += sbyte(d2, 2) * h2; e3s += sbyte(d2, 3) * h3;
+        } else {
+            asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[0]) : "r"(sbyte(d2, 0)), "r"(h0));
+            asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[1]) : "r"(sbyte(d2, 1)), "r"(h1));
+            asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[2]) : "r"(sbyte(d2, 2)), "r"(h2));
+            asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(dE[3]) : "r"(sbyte(d2, 3)), "r"(h3));
+        }
         if (storer) {
             if (DELTA) {
                 sts32(val + 4u * rowc, d2);
@@ -278,6 +285,7 @@ __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChun
             }
         }
     }
+    if (N32) { dE[0] += e0s; dE[1] += e1s; dE[2] += e2s; dE[3] += e3s; }
 }
 
 // One pass over all chain levels (one sweep of the chain rows), chunks streamed through two buffers.
@@ -482,7 +490,10 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
             const ChainChunk ck = s_chunks[0];
             for (uint32_t s = 0; s < v.n_segs; ++s) {
                 const ChainSeg sg = s_segs[s];
-                chain_segment<false, PREMUL>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
+                if (v.narrow != 0u && sg.r1 - sg.r0 > (nthr >> (sg.info & 0xffu)))   // several rows per thread
+                    chain_segment<false, PREMUL, true>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
+                else
+                    chain_segment<false, PREMUL, false>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
                 if (sg.info & 0x100u) __syncthreads();
                 if (TIMING && ts) *ts++ = (unsigned long long)clock64();
             }
