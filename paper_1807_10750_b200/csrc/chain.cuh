@@ -30,7 +30,7 @@ constexpr int kChainGroups = 8;                 // chain CTAs per replica tile: 
 constexpr uint32_t kChainMaxLocal = 65535;      // local row ids are 16 bit
 constexpr int kChainMaxChunks = 96;
 constexpr int kChainMaxSegs = 192;
-constexpr int kSmallThreadsMax = 1024;
+constexpr int kSmallThreadsMax = 512;           // (measured on configs 1-3: 512 threads are as fast as or faster than 1024)
 
 struct ChainSeg {
     uint32_t r0, r1;   // local rows [r0, r1) of one level, inside one chunk

@@ -302,6 +302,10 @@ inline uint32_t small_threads_override(uint32_t t) {
 #endif
     return t;
 }
+inline const void* small_kernel(bool timing, bool premul) {
+    if (timing) return premul ? (const void*)k_anneal_small<true, true> : (const void*)k_anneal_small<true, false>;
+    return premul ? (const void*)k_anneal_small<false, true> : (const void*)k_anneal_small<false, false>;
+}
 inline uint32_t align4u(uint32_t x) { return (x + 3u) & ~3u; }
 inline uint32_t pow2_floor(uint32_t x) { uint32_t r = 1; while (2u * r <= x) r *= 2u; return r; }
 inline uint32_t pow2_ceil(uint32_t x) { uint32_t r = 1; while (r < x) r *= 2u; return r; }
@@ -1125,9 +1129,7 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
             CK(cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, dev));
         }
         const uint32_t csplit = (p->small_csplit > 1u && 2 * (int64_t)tiles * kChainGroups <= (int64_t)dev_sms) ? 2u : 1u;
-        const void* small_fn = p->chain.premul
-            ? (p->timing ? (const void*)k_anneal_small<true, true> : (const void*)k_anneal_small<false, true>)
-            : (p->timing ? (const void*)k_anneal_small<true, false> : (const void*)k_anneal_small<false, false>);
+        const void* small_fn = small_kernel(p->timing != nullptr, p->chain.premul != 0u);
         CK(cudaFuncSetAttribute(small_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->small_dyn));
         for (int32_t s0 = 0; s0 < n_sweeps; s0 += (int32_t)kThrCap) {
             const int32_t ns = std::min<int32_t>((int32_t)kThrCap, n_sweeps - s0);
