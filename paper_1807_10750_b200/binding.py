@@ -83,6 +83,8 @@ def lib():
                                        ctypes.POINTER(ctypes.c_double), _vp]
     L.ising_free.restype = _i32
     L.ising_free.argtypes = [_vp]
+    L.ising_energy_cut_noalloc.restype = _i32
+    L.ising_energy_cut_noalloc.argtypes = [_i32, _i64, _vp, _vp, _vp, _i32, _vp, _i32, _vp, _vp, _vp]
     _lib = L
     return L
 
@@ -259,6 +261,28 @@ def ising_energy_cut(p: Problem, spins=None, n_replicas: Optional[int] = None, s
     _check(lib().ising_energy_cut(p.handle, _ptr(spins), n_replicas, _ptr(e), _ptr(c), _stream(stream)),
            "ising_energy_cut")
     return e, c
+
+
+NOALLOC_MAX_REPLICAS = 1024
+
+
+def ising_energy_cut_noalloc(row_ptr, col_idx, weights, spins, energy_out, cut_out, stream=None):
+    """include/ising_noalloc.h: energy / cut straight from a DEVICE CSR, nothing allocated (the library's static
+    scratch; at most NOALLOC_MAX_REPLICAS replicas; calls that overlap on the GPU race).  Every argument is a CUDA
+    tensor the caller owns: row_ptr int64 [n+1], col_idx int32 [nnz], weights int8 | int32 [nnz], spins int8 [R][n],
+    energy_out / cut_out int64 [R] (either may be None).  Marshals only: no tensor is created here."""
+    torch = _torch()
+    for t in (row_ptr, col_idx, weights, spins, energy_out, cut_out):
+        if t is not None and not (t.is_cuda and t.is_contiguous()):
+            raise ValueError("ising_energy_cut_noalloc takes contiguous CUDA tensors")
+    if row_ptr.dtype != torch.int64 or col_idx.dtype != torch.int32 or spins.dtype != torch.int8:
+        raise ValueError("row_ptr int64, col_idx int32, spins int8")
+    wtype = {torch.int8: ISING_W_INT8, torch.int32: ISING_W_INT32}[weights.dtype]
+    n = int(row_ptr.numel()) - 1
+    n_replicas = int(spins.shape[0]) if spins.ndim == 2 else 1
+    _check(lib().ising_energy_cut_noalloc(n, int(col_idx.numel()), _ptr(row_ptr), _ptr(col_idx), _ptr(weights), wtype,
+                                          _ptr(spins), n_replicas, _ptr(energy_out), _ptr(cut_out), _stream(stream)),
+           "ising_energy_cut_noalloc")
 
 
 def ising_best_state(p: Problem, replica: int = -1, want_spins: bool = True, stream=None):

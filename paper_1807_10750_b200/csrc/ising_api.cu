@@ -20,6 +20,7 @@
 #include "builder.cuh"
 #include "common.cuh"
 #include "dense_tcgen05.cuh"
+#include "noalloc.cuh"
 #include "probe.cuh"
 #include "sparse_sweep.cuh"
 
@@ -1528,6 +1529,28 @@ ising_status ising_debug_probe_l2(void* scratch, size_t bytes, double* gather_gb
     const double g4 = (double)blocks * 64.0 * per_pair * 32.0 / (ms_g4 * 1e-3) / 1e9;      // 4-byte lanes: 64 groups per CTA
     *gather_gbs = std::max(*gather16_gbs, g4);
     *stream_gbs = (double)use * passes / (ms_s * 1e-3) / 1e9;
+    return ISING_OK;
+}
+
+// include/ising_noalloc.h: no handle, no workspace, no allocation; scratch = g_noalloc_scratch (noalloc.cuh, this
+// translation unit), its device address taken with cudaGetSymbolAddress once per device.
+ising_status ising_energy_cut_noalloc(int32_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
+                                      const void* weights, int32_t wtype, const int8_t* spins, int32_t n_replicas,
+                                      int64_t* energy_out, int64_t* cut_out, void* stream) {
+    if (!row_ptr || !spins || (nnz > 0 && (!col_idx || !weights))) return ISING_ERR_NULL_ARG;
+    if (n <= 0 || nnz < 0 || (wtype != ISING_W_INT8 && wtype != ISING_W_INT32)) return ISING_ERR_BAD_SHAPE;
+    if (n_replicas < 1 || n_replicas > kNoAllocMaxReplicas) return ISING_ERR_TOO_MANY_REPLICAS;   // the scratch holds no more
+    if (ising_status s = check_device()) return s;
+    long long* scratch = noalloc_scratch_ptr();
+    if (!scratch) return ISING_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    k_noalloc_clear<<<(unsigned)((n_replicas + 255) / 256), 256, 0, st>>>(scratch, n_replicas);
+    const unsigned row_blocks = (unsigned)std::min<long long>(((long long)n + 7) / 8, 2048);
+    k_noalloc_accumulate<<<dim3(row_blocks, (unsigned)n_replicas), 256, 0, st>>>(
+        n, reinterpret_cast<const long long*>(row_ptr), col_idx, weights, wtype, spins, scratch);
+    k_noalloc_finish<<<(unsigned)((n_replicas + 255) / 256), 256, 0, st>>>(
+        scratch, n_replicas, reinterpret_cast<long long*>(energy_out), reinterpret_cast<long long*>(cut_out));
+    CK(cudaGetLastError());
     return ISING_OK;
 }
 
