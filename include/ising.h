@@ -92,7 +92,9 @@ enum {
     ISING_LOAD_NO_SMALL = 2,      /* do not run a small graph wholly inside one CTA per four replicas (shared memory)   */
     ISING_LOAD_NO_CLUSTER = 4,    /* no thread-block clusters: neither one per replica tile, nor pairs of CTAs sharing   */
                                   /* the rows of a small graph in the shared-memory engine                               */
-    ISING_LOAD_NO_TAIL_CHAIN = 8  /* big graph: every colour class is a grid-wide phase (no shared-memory tail chain)    */
+    ISING_LOAD_NO_TAIL_CHAIN = 8, /* big graph: every colour class is a grid-wide phase (no shared-memory tail chain)    */
+    ISING_LOAD_NO_OVERLAP = 16    /* tail chain: do not update the chain-free rows of colour class 0 for sweep t + 1 while */
+                                  /* the chain finishes sweep t (the chain runs alone, as in the build before)            */
 };
 
 /*
@@ -205,7 +207,8 @@ ising_status ising_current_state(ising_problem* p, int8_t* spins_out, int32_t n_
  *         clusters, 3 persistent grid + shared-memory tail chain, 4 shared-memory chain for the whole graph),
  *         14 rows of the shared-memory chain, 15 virtual phases of the persistent kernel,
  *         16 chunks of the chain, 17 1 if the chain is resident in shared memory,
- *         18 CTAs per word of four replicas of the small-graph engine (cluster size)
+ *         18 CTAs per word of four replicas of the small-graph engine (cluster size),
+ *         19 rows of colour class 0 updated beside the tail chain (chain overlap; 0 = off)
  */
 ising_status ising_problem_info(const ising_problem* p, int32_t what, int64_t* value_out);
 

@@ -21,7 +21,7 @@ ISING_TIE_MINUS, ISING_TIE_KEEP = 0, 1
 ISING_INIT_PHILOX, ISING_INIT_GIVEN, ISING_INIT_CONTINUE = 0, 1, 2
 ISING_W_INT8, ISING_W_INT32 = 1, 4
 ISING_LOAD_DEFAULT, ISING_LOAD_NO_DENSE = 0, 1
-ISING_LOAD_NO_SMALL, ISING_LOAD_NO_CLUSTER, ISING_LOAD_NO_TAIL_CHAIN = 2, 4, 8
+ISING_LOAD_NO_SMALL, ISING_LOAD_NO_CLUSTER, ISING_LOAD_NO_TAIL_CHAIN, ISING_LOAD_NO_OVERLAP = 2, 4, 8, 16
 # ising_problem_info(13): the Gauss-Seidel engine of a loaded problem
 ENGINE_PER_PHASE, ENGINE_GRID, ENGINE_CLUSTER, ENGINE_GRID_TAIL_CHAIN, ENGINE_SMALL = 0, 1, 2, 3, 4
 

@@ -147,6 +147,33 @@ __global__ void k_relabel_finish(RelabelKey rk, const uint32_t* perm, int32_t* i
     }
 }
 
+// Overlap split (ising_api.cu, "chain overlap"): colour class 0 is cut into the rows WITHOUT a neighbour among the tail
+// chain's classes (colour >= c_tail; new colour 0) and the rest (new colour 1); every other class moves up by one.  Both
+// halves of class 0 are independent sets, so this is a valid colouring with the same Gauss-Seidel result (the order
+// inside a class is irrelevant), and the first half can be updated for sweep t + 1 while the chain still finishes
+// sweep t: none of its rows reads or is read by a chain row.  One warp per row; only class-0 rows look at their edges.
+__global__ void k_split_class0(int32_t n, const long long* row_ptr, const int32_t* col, const int32_t* colour,
+                               int32_t n_colours, int32_t c_tail, int32_t* colour2) {
+    const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (gw >= n) return;
+    const int32_t i = (int32_t)gw;
+    const int32_t c = colour[i];
+    if (c != 0) {
+        if (lane == 0) colour2[i] = (c < 0 ? 0 : (c >= n_colours ? n_colours - 1 : c)) + 1;   // (garbage is rejected by k_validate)
+        return;
+    }
+    bool adj = false;
+    long long b = row_ptr[i], e = row_ptr[i + 1];
+    if (b < 0 || e < b) { b = 0; e = 0; }
+    for (long long k = b + lane; k < e && !adj; k += 32) {
+        const int32_t j = col[k];
+        if (j >= 0 && j < n) adj = colour[j] >= c_tail;
+    }
+    adj = __any_sync(0xffffffffu, adj);
+    if (lane == 0) colour2[i] = adj ? 1 : 0;
+}
+
 // One warp per row: column range / order / self loops, symmetry, colouring, sum_j |w_ij|.
 // Symmetry: entry (i, j) is looked up in row j (binary search) only when row j is not longer than row i; the entries
 // whose row j is longer are counted instead.  Every looked-up entry of the first kind (deg j < deg i) names a distinct

@@ -100,7 +100,7 @@ size_t chain_ws_bound(int64_t n, int64_t nnz, int64_t tiles);
 size_t workspace_need(int64_t n, int64_t nnz, int wtype, int64_t max_replicas, int64_t C, bool wide,
                       uint64_t n_slices, uint64_t n_hubs, uint64_t cells, bool with_raw, bool dense) {
     const uint64_t tiles = (uint64_t)(max_replicas + kTile - 1) / kTile;
-    const uint64_t phases = (uint64_t)std::max<int64_t>(1, C);
+    const uint64_t phases = (uint64_t)std::max<int64_t>(1, C) + 1;   // (+ 1: the overlap split of class 0)
     size_t s = 0;
     auto add = [&](size_t b) { s = align_up(s) + b; };
     add(sizeof(BuildReport));
@@ -116,6 +116,7 @@ size_t workspace_need(int64_t n, int64_t nnz, int wtype, int64_t max_replicas, i
     add(4 * 256 * (size_t)((n + kRadixChunk - 1) / kRadixChunk));   // digit histograms
     add(sizeof(RelabelRuns));
     add(12 * (size_t)n);                      // runs of equal (colour, degree)
+    add(4 * (size_t)n);                       // colours after the overlap split of class 0
     add(sizeof(SliceDesc) * (size_t)(n_slices + 1));
     add(4 * 16 * (size_t)(n_slices + 1));     // sorig
     add(8 * (size_t)(n_slices + 1));          // slice_aux
@@ -158,6 +159,8 @@ struct ising_problem {
     SliceDesc* slices = nullptr;
     uint32_t* sorig = nullptr;
     uint32_t* slice_aux = nullptr;       // [n_slices][2] (hub id, part index) of hub-part slices
+    bool overlap0 = false;               // chain overlap: virtual phase 0 (the rows of colour class 0 without a chain neighbour) runs
+    uint32_t ov_rows = 0;                // for sweep t + 1 beside the chain of sweep t; these are the internal rows [0, ov_rows)
     int cluster_ctas = 0;                // small graph: the persistent kernel runs as one cluster of this many CTAs per replica tile (0: grid)
     unsigned long long* hub_acc = nullptr;   // [n_hubs][tiles_max][32] partial local fields of hub rows
     unsigned int* hub_cnt = nullptr;     // [n_hubs][tiles_max] parts arrived (monotone)
@@ -451,7 +454,7 @@ ising_status ising_workspace_bytes(int32_t n, int64_t nnz, int32_t wtype, int32_
     if (max_replicas < 1 || max_replicas > 65536) return ISING_ERR_TOO_MANY_REPLICAS;
     const bool dense = kDenseEnabled && nnz == (int64_t)n * (n - 1) && n >= 2;
     *bytes_out = workspace_need(n, nnz, wtype, max_replicas, n_colours, wtype == ISING_W_INT32,
-                                bound_slices(n, nnz, n_colours), bound_hubs(n, nnz), bound_cells(n, nnz, n_colours), true,
+                                bound_slices(n, nnz, n_colours + 1), bound_hubs(n, nnz), bound_cells(n, nnz, n_colours + 1), true,
                                 dense);
     return ISING_OK;
 }
@@ -514,7 +517,7 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
     k_check_rowptr<<<(unsigned)((n + 1 + 255) / 256), 256, 0, st>>>(d_row_ptr, n, nnz, d_rep);
 
     // ---- relabelling on the device (builder.cuh), on a stream of its own: it overlaps the copies of col_idx / weights
-    const int32_t C = n_colours > 0 ? n_colours : 1;
+    int32_t C = n_colours > 0 ? n_colours : 1;   // (+ 1 after the overlap split of class 0, below)
     struct Side {   // the side stream and its fork event
         cudaStream_t s = nullptr;
         cudaEvent_t e = nullptr;
@@ -538,20 +541,22 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
     RelabelRuns* d_runs = (RelabelRuns*)ws.take(sizeof(RelabelRuns));
     uint32_t* d_run_rows = (uint32_t*)ws.take(12 * (size_t)n);
     if (ws.overflow) return ISING_ERR_WORKSPACE_TOO_SMALL;
-    {
+    auto enqueue_relabel = [&](const RelabelKey& key, uint32_t n_passes, cudaStream_t s) -> ising_status {
         const unsigned cb = (n_chunks + 3u) / 4u;
         const uint32_t* src = nullptr;
-        for (uint32_t ps = 0; ps < passes; ++ps) {   // (the last pass lands in d_perm)
-            uint32_t* dst = ((passes - ps) & 1u) ? (uint32_t*)d_perm : d_ids;
-            k_radix_hist<<<cb, 128, 0, side.s>>>(rk, src, 8u * ps, n_chunks, d_hist);
-            k_radix_scan<<<1, 1024, 0, side.s>>>(d_hist, 256u * n_chunks);
-            k_radix_scatter<<<cb, 128, 0, side.s>>>(rk, src, dst, 8u * ps, n_chunks, d_hist);
+        for (uint32_t ps = 0; ps < n_passes; ++ps) {   // (the last pass lands in d_perm)
+            uint32_t* dst = ((n_passes - ps) & 1u) ? (uint32_t*)d_perm : d_ids;
+            k_radix_hist<<<cb, 128, 0, s>>>(key, src, 8u * ps, n_chunks, d_hist);
+            k_radix_scan<<<1, 1024, 0, s>>>(d_hist, 256u * n_chunks);
+            k_radix_scatter<<<cb, 128, 0, s>>>(key, src, dst, 8u * ps, n_chunks, d_hist);
             src = dst;
         }
-        CK(cudaMemsetAsync(d_runs, 0, sizeof(RelabelRuns), side.s));
-        k_relabel_finish<<<(unsigned)((n + 255) / 256), 256, 0, side.s>>>(rk, (const uint32_t*)d_perm, d_inv, d_runs, d_run_rows,
-                                                                         (uint32_t)n);
-    }
+        CK(cudaMemsetAsync(d_runs, 0, sizeof(RelabelRuns), s));
+        k_relabel_finish<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(key, (const uint32_t*)d_perm, d_inv, d_runs, d_run_rows,
+                                                                    (uint32_t)n);
+        return ISING_OK;
+    };
+    if (ising_status s = enqueue_relabel(rk, passes, side.s)) return s;
     // (meanwhile, on the caller's stream: the edges)
     if (!ci_dev) {
         void* b = ws.take(4 * (size_t)nnz);
@@ -571,16 +576,20 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
     RelabelRuns runs_hdr{};
     const size_t runs_first = std::min<size_t>((size_t)n, 32768);
     std::vector<uint32_t> run_rows(3 * runs_first);
-    CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, side.s));
-    CK(cudaMemcpyAsync(&runs_hdr, d_runs, sizeof(runs_hdr), cudaMemcpyDeviceToHost, side.s));
-    CK(cudaMemcpyAsync(run_rows.data(), d_run_rows, 12 * runs_first, cudaMemcpyDeviceToHost, side.s));
-    CK(cudaStreamSynchronize(side.s));
-    CK(cudaGetLastError());
+    auto fetch_runs = [&](cudaStream_t s) -> ising_status {
+        CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, s));
+        CK(cudaMemcpyAsync(&runs_hdr, d_runs, sizeof(runs_hdr), cudaMemcpyDeviceToHost, s));
+        CK(cudaMemcpyAsync(run_rows.data(), d_run_rows, 12 * runs_first, cudaMemcpyDeviceToHost, s));
+        CK(cudaStreamSynchronize(s));
+        CK(cudaGetLastError());
+        if (runs_hdr.count > runs_first) {
+            run_rows.resize(3 * (size_t)runs_hdr.count);
+            CK(cudaMemcpy(run_rows.data(), d_run_rows, 12 * (size_t)runs_hdr.count, cudaMemcpyDeviceToHost));
+        }
+        return ISING_OK;
+    };
+    if (ising_status s = fetch_runs(side.s)) return s;
     if (rep.err_mask) { (void)cudaStreamSynchronize(st); return ISING_ERR_BAD_SHAPE; }   // (the copies read the caller's arrays)
-    if (runs_hdr.count > runs_first) {
-        run_rows.resize(3 * (size_t)runs_hdr.count);
-        CK(cudaMemcpy(run_rows.data(), d_run_rows, 12 * (size_t)runs_hdr.count, cudaMemcpyDeviceToHost));
-    }
     LT("relabel done (runs on host)");
     // ---- validate on the device (row_ptr is sound from here on); the report is read before anything is packed
     {
@@ -601,10 +610,14 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
 
     // ---- O(slices) planning on the host, from the runs: internal rows [run_start[q], run_start[q + 1]) have degree
     // run_deg[q]; a run never crosses a colour boundary
-    const size_t n_runs = runs_hdr.count;
-    std::vector<int64_t> run_start(n_runs + 1), run_deg(n_runs + 1, 0);
-    std::vector<int64_t> cstart((size_t)C + 1, 0);       // internal rows of colour c: [cstart[c], cstart[c+1])
-    {
+    size_t n_runs = 0;
+    std::vector<int64_t> run_start, run_deg;
+    std::vector<int64_t> cstart;                         // internal rows of colour c: [cstart[c], cstart[c+1])
+    auto sort_runs = [&]() {
+        n_runs = runs_hdr.count;
+        run_start.assign(n_runs + 1, 0);
+        run_deg.assign(n_runs + 1, 0);
+        cstart.assign((size_t)C + 1, 0);
         std::vector<uint64_t> order(n_runs);             // (first row << 32 | run index), sorted by first row
         for (size_t q = 0; q < n_runs; ++q) order[q] = ((uint64_t)run_rows[3 * q] << 32) | q;
         std::sort(order.begin(), order.end());
@@ -618,8 +631,47 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         }
         run_start[n_runs] = n;
         for (size_t k = 1; k < cstart.size(); ++k) cstart[k] += cstart[k - 1];
-    }
+    };
+    sort_runs();
     LT("runs sorted");
+    // Tail chain (chain.cuh, DELTA): the last colour classes of a big graph hold few, hub-like rows and cost a grid
+    // barrier plus a dependent unit each (config 5: 14 of 22 phases, 8 % of the edges, 29 % of the sweep).  If the
+    // classes c_tail .. C-1 hold at most kTailRows rows in all, the persistent kernel computes their fields in ONE
+    // bulk pseudo-phase and walks the classes inside one CTA per four replicas.  Graphs small enough for
+    // k_anneal_small are wholly a chain and need no tail.
+    auto tail_start = [&]() {
+        int32_t ct = C;
+        if (colour && C >= 3 && !(flags & ISING_LOAD_NO_TAIL_CHAIN)) {
+            const int64_t tail_rows = tail_rows_limit();
+            int32_t c = C;
+            while (c > 1 && (int64_t)n - cstart[(size_t)c - 1] <= tail_rows) --c;
+            if (C - c >= 2) ct = c;
+        }
+        return ct;
+    };
+    int32_t c_tail = tail_start();
+    // Chain overlap: while the chain (8 CTAs per tile) finishes sweep t, the other CTAs already update, for sweep
+    // t + 1, the rows of colour class 0 that have no neighbour among the chain's rows (builder.cuh k_split_class0: they
+    // become a colour class of their own in front of the rest of class 0; same Gauss-Seidel result).  Needs the edges on
+    // the device, so the relabelling is repeated on the caller's stream behind the copies.
+    const int32_t* d_colour_eff = d_colour;   // the colouring the internal row order follows
+    bool split0 = false;
+    if (c_tail < C && (int64_t)n > (int64_t)kChainMaxLocal && !(flags & ISING_LOAD_NO_OVERLAP)) {
+        int32_t* d_colour2 = (int32_t*)ws.take(4 * (size_t)n);
+        if (ws.overflow) { (void)cudaStreamSynchronize(st); return ISING_ERR_WORKSPACE_TOO_SMALL; }
+        k_split_class0<<<(unsigned)(((long long)n * 32 + 255) / 256), 256, 0, st>>>(n, d_row_ptr, d_col, d_colour, C, c_tail, d_colour2);
+        C += 1;
+        RelabelKey rk2 = rk;
+        rk2.colour = d_colour2; rk2.n_colours = C;
+        const uint32_t passes2 = std::max(1u, (rk.dbits + bits_of((uint64_t)(C - 1)) + 7u) / 8u);
+        if (ising_status s = enqueue_relabel(rk2, passes2, st)) { (void)cudaStreamSynchronize(st); return s; }
+        if (ising_status s = fetch_runs(st)) { (void)cudaStreamSynchronize(st); return s; }
+        sort_runs();
+        c_tail = tail_start();
+        d_colour_eff = d_colour2;
+        split0 = true;
+        LT("overlap split + second relabel");
+    }
     // ---- work units: hubs (rows above kHubDegree, one CTA each) and slices (one warp each)
     int sm_count = 148, coop = 0;
     {
@@ -695,18 +747,6 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         }
         return k;
     };
-    // Tail chain (chain.cuh, DELTA): the last colour classes of a big graph hold few, hub-like rows and cost a grid
-    // barrier plus a dependent unit each (config 5: 14 of 22 phases, 8 % of the edges, 29 % of the sweep).  If the
-    // classes c_tail .. C-1 hold at most kTailRows rows in all, the persistent kernel computes their fields in ONE
-    // bulk pseudo-phase and walks the classes inside one CTA per four replicas.  Graphs small enough for
-    // k_anneal_small are wholly a chain and need no tail.
-    int32_t c_tail = C;
-    if (colour && C >= 3 && !(flags & ISING_LOAD_NO_TAIL_CHAIN)) {
-        const int64_t tail_rows = tail_rows_limit();
-        int32_t c = C;
-        while (c > 1 && (int64_t)n - cstart[(size_t)c - 1] <= tail_rows) --c;
-        if (C - c >= 2) c_tail = c;
-    }
     {
         int32_t k = 0;
         for (int32_t c = 0; c < C; ++c) {
@@ -962,6 +1002,8 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
             v.narrow = (uint64_t)n_t * 2ull * (uint64_t)rep.absw_max < (1ull << 31) ? 1u : 0u;
             if (delta) {
                 p->chain_delta = true;
+                p->overlap0 = split0;
+                p->ov_rows = split0 ? (uint32_t)cstart[1] : 0u;
             } else {
                 p->chain_small = true;
                 p->small_threads = threads;
@@ -986,8 +1028,9 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         CKP(cudaStreamSynchronize(st));
     }
     p->ws_used = ws.used;
-    CKP(cudaFuncSetAttribute(k_anneal_gs<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
-    CKP(cudaFuncSetAttribute(k_anneal_gs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
+    CKP(cudaFuncSetAttribute(k_anneal_gs<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
+    CKP(cudaFuncSetAttribute(k_anneal_gs<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
+    CKP(cudaFuncSetAttribute(k_anneal_gs<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnnealDynSmem));
     CKP(cudaStreamSynchronize(st));   // the host vectors die at return
     CKP(cudaGetLastError());
     LT("final sync");
@@ -1222,6 +1265,9 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
                 a.n_vphases = p->n_vphases;
                 a.chain_on = p->chain_delta ? 1u : 0u;
                 a.chain = p->chain;
+                const bool overlap = p->overlap0 && 2 * kChainGroups * bt <= (int)p->n_cta;   // (the phase runs on the CTAs that are not chain CTAs)
+                a.ov_rows = p->ov_rows;
+                a.alt = p->state[p->cur ^ 1] + (size_t)t0 * tile_stride;
                 a.resume = s0 > 0 ? 1 : 0;
                 a.timing = (t0 == 0 && s0 == 0) ? p->timing : nullptr;
                 a.timing_sweep = p->timing_sweep;
@@ -1239,11 +1285,11 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
                     at[0].val.clusterDim.x = (unsigned)p->cluster_ctas; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
                     cfg.attrs = at;
                     cfg.numAttrs = 1;
-                    CK(cudaLaunchKernelEx(&cfg, k_anneal_gs<true>, a));
+                    CK(cudaLaunchKernelEx(&cfg, k_anneal_gs<true, false>, a));
                 } else {
                     void* args[] = {&a};
-                    CK(cudaLaunchCooperativeKernel((const void*)k_anneal_gs<false>, dim3(p->n_cta), dim3(kSweepThreads), args,
-                                                   kAnnealDynSmem, st));
+                    CK(cudaLaunchCooperativeKernel(overlap ? (const void*)k_anneal_gs<false, true> : (const void*)k_anneal_gs<false, false>,
+                                                   dim3(p->n_cta), dim3(kSweepThreads), args, kAnnealDynSmem, st));
                 }
                 p->launches++;
             }
@@ -1260,7 +1306,7 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
             q.src = p->state[p->cur]; q.dst = p->state[p->cur];
             q.accum = p->sm.accum[p->parity];
             q.thr = thresholds[t]; q.T = (uint32_t)(sweep_offset + t);
-            for (int32_t c = 0; c < p->n_colours; ++c) {
+            for (int32_t c = 0; c < (int32_t)p->n_phases; ++c) {
                 q.phase_begin = (uint32_t)c; q.phase_end = (uint32_t)c + 1;
                 launch_sweep(p, kKindGS, q, tiles, st);
             }
@@ -1293,7 +1339,7 @@ ising_status ising_anneal(ising_problem* p, int32_t mode, int32_t tie_rule, int3
             q.src = p->state[p->cur]; q.dst = p->state[p->cur];
             q.accum = p->sm.accum_eval;   // increments of the minimisation sweep: not used, the cut is evaluated below
             q.thr = 0u; q.T = (uint32_t)(sweep_offset + t);
-            for (int32_t c = 0; c < p->n_colours; ++c) {
+            for (int32_t c = 0; c < (int32_t)p->n_phases; ++c) {
                 q.phase_begin = (uint32_t)c; q.phase_end = (uint32_t)c + 1;
                 launch_sweep(p, kKindGS, q, tiles, st);
             }
@@ -1470,6 +1516,7 @@ ising_status ising_problem_info(const ising_problem* p, int32_t what, int64_t* v
         case 16: *value_out = (p->chain_small || p->chain_delta) ? p->chain.n_chunks : 0; break;
         case 17: *value_out = (p->chain_small || p->chain_delta) ? p->chain.resident : 0; break;
         case 18: *value_out = p->chain_small ? p->small_csplit : 0; break;
+        case 19: *value_out = p->overlap0 ? (int64_t)p->ov_rows : 0; break;
         default: return ISING_ERR_BAD_SHAPE;
     }
     return ISING_OK;

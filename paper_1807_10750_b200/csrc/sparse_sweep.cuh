@@ -695,6 +695,12 @@ struct AnnealParams {
     uint32_t n_vphases;
     uint32_t chain_on;
     ChainView chain;
+    // Chain overlap (k_anneal_gs<false, true>, chain_on): virtual phase 0 holds the rows [0, ov_rows) of colour class 0
+    // that have no neighbour among the chain's rows.  It runs on the CTAs that are not chain CTAs: for sweep 0 on its
+    // own, for sweep t + 1 while the chain finishes sweep t.  The improved mask of sweep t is not known then, so these
+    // rows park the value they held in `alt` (same layout as state); the capture into `best` follows once the mask is known.
+    uint32_t ov_rows;
+    uint8_t* alt;
     unsigned long long* timing;     // diagnostics: [n_vphases + 1][n_cta][8] SM-clock stamps of sweep timing_sweep (0 / 1: arrival at
                                     // / departure from the barrier that ends the virtual phase; row n_vphases: the chain), or nullptr
     uint32_t timing_sweep;
@@ -730,8 +736,9 @@ __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int
     if (stamp && threadIdx.x == 0) stamp[1] = (unsigned long long)clock64();
 }
 
-template <bool CLUSTER>
+template <bool CLUSTER, bool OV>
 __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealParams p) {
+    static_assert(!(CLUSTER && OV), "the chain overlap belongs to the grid variant");
     __shared__ long long s_acc[kMaxPersistReplicas];
     __shared__ long long s_wacc[kWarpsPerCta][kTile];
     __shared__ uint32_t s_wtile[kWarpsPerCta];
@@ -818,25 +825,91 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
     // its first unit can be requested across the barrier that precedes the phase.
     const uint32_t n_static = n_cta * (uint32_t)kWarpsPerCta;
     const uint32_t u_static = (uint32_t)warp * n_cta + cta;
+    // (OV: virtual phase 0 is dealt out over the CTAs that are not chain CTAs, like this)
+    const uint32_t n_chain = OV ? (uint32_t)kChainGroups * tiles : 0u;
+    const uint32_t n_static0 = OV ? (n_cta - n_chain) * (uint32_t)kWarpsPerCta : n_static;
+    const uint32_t u_static0 = OV ? (chain_cta ? 0xffffffffu : (uint32_t)warp * (n_cta - n_chain) + (cta - n_chain)) : u_static;
     uint32_t ps0 = ps_of(0u);
     uint32_t nu = (ps_of(1u) - ps0) * tiles;
     // one-unit lookahead of the static data, kept across the barrier
-    bool have = u_static < nu;
+    bool have = u_static0 < nu;
     HeadIdx nxt{};
     uint32_t mslot = 0;   // meta slot of the unit whose head is in flight (`nxt`)
-    if (have) nxt = tiles == 1u ? request_head(p.g, pa, mslot, ps0 + u_static, 0u, sr, lane)
-                              : request_head(p.g, pa, mslot, ps0 + u_static / tiles, u_static % tiles, sr, lane);
+    if (have) nxt = tiles == 1u ? request_head(p.g, pa, mslot, ps0 + u_static0, 0u, sr, lane)
+                              : request_head(p.g, pa, mslot, ps0 + u_static0 / tiles, u_static0 % tiles, sr, lane);
 
     for (uint32_t t = 0; t < p.n_sweeps; ++t) {
         const uint32_t thr = __ldg(p.thr + t);
         const uint32_t T = p.sweep_offset + t;
         unsigned long long* const tsw = (!CLUSTER && p.timing && t == p.timing_sweep) ? p.timing + (size_t)cta * 8 : nullptr;
-        for (uint32_t vp = 0; vp < VP; ++vp) {
+        const bool more_sweeps = t + 1 < p.n_sweeps;
+        // OV: one (slice, tile) unit loop more, used beside the chain for virtual phase 0 of sweep t + 1 (same pipeline as
+        // the loop of the ordinary phases below; the rows park their previous values in `alt`, see AnnealParams)
+        auto run_phase0_parked = [&]() {
+            if (!have) return;
+            const uint32_t thr_u = __ldg(p.thr + t + 1), T_u = T + 1u;
+            SliceDesc pend_d{};
+            uint32_t pend_tile = 0;
+            uint32_t u_pos = u_static0;
+            auto stage_next = [&](uint32_t gb_) {
+                pend_d = lds_desc(pa.desc(mslot));
+                pend_tile = lds32(pa.desc(mslot) + 16);
+                issue_slice_gathers(state() + (size_t)pend_tile * p.tile_stride + (size_t)half * 16, nxt, pend_d, sr, gb_, true);
+                if (pend_d.G > (uint32_t)kHeadGroups) {
+                    const size_t tail_at = (size_t)pend_d.off + sr;
+                    if (half == 0) prefetch_l2(p.g.col4 + tail_at);
+                    else if (pend_d.G > (uint32_t)kHeadGroups + 1u) prefetch_l2(p.g.col4 + tail_at + kSubRows);
+                    if (lane == 0) prefetch_l2(p.g.w4 + tail_at);
+                }
+                u_pos += n_static0;
+                have = u_pos < nu;
+                if (have) {
+                    mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
+                    nxt = tiles == 1u ? request_head(p.g, pa, mslot, ps0 + u_pos, 0u, sr, lane)
+                                      : request_head(p.g, pa, mslot, ps0 + u_pos / tiles, u_pos % tiles, sr, lane);
+                }
+            };
+            uint32_t gb = gbuf0;
+            cp_async_wait<0>();
+            __syncwarp();
+            uint32_t cur_m = mslot;
+            stage_next(gb);
+            while (true) {
+                const SliceDesc cur_d = pend_d;
+                const uint32_t tile = pend_tile;
+                const bool more = have;
+                const uint32_t nxt_m = mslot;
+                cp_async_wait<0>();
+                if (more) {
+                    __syncwarp();
+                    stage_next(gb ^ gbuf_flip);
+                }
+                if (tile != acc_tile) {
+                    flush_warp(acc, s_wacc[warp], lane);
+                    fold_warp(s_wacc[warp], s_acc + acc_tile * kTile, lane);
+                    rows_acc = 0;
+                    acc_tile = tile;
+                }
+                const PassCtx x = make_ctx(state(), state(), p.alt, 0xffffffffu, p.tile_stride, tile, half, rep0(), thr_u, T_u, p.tie_rule);
+                slice_compute(p.g, x, cur_d, pa.meta(cur_m, 0), sr, acc, p.keys, gb, false, bd);
+                if (++rows_acc >= p.flush_rows) {
+                    flush_warp(acc, s_wacc[warp], lane);
+                    rows_acc = 0;
+                }
+                if (!more) break;
+                gb ^= gbuf_flip;
+                cur_m = nxt_m;
+            }
+        };
+        for (uint32_t vp = (OV && t > 0u) ? 1u : 0u; vp < VP; ++vp) {
             const bool last_phase = vp + 1 == VP;
             const bool very_last = last_phase && t + 1 == p.n_sweeps;
             const bool bulk = chain_on && last_phase;
             const uint32_t vpn = last_phase ? 0u : vp + 1u;
             const uint32_t psn0 = ps_of(vpn), psn1 = ps_of(vpn + 1u);
+            // (OV: virtual phase 0 has its own unit mapping)
+            const uint32_t us = (OV && vp == 0u) ? u_static0 : u_static, ns = (OV && vp == 0u) ? n_static0 : n_static;
+            const uint32_t usn = (OV && vpn == 0u) ? u_static0 : u_static, nsn = (OV && vpn == 0u) ? n_static0 : n_static;
 
             if (have) {
                 // software pipeline: unit k is computed from gather buffer gb while the gathers of unit k+1 fly
@@ -844,7 +917,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 // meta slot)
                 SliceDesc pend_d{};
                 uint32_t pend_tile = 0;
-                uint32_t u_pos = u_static;
+                uint32_t u_pos = us;
                 auto stage_next = [&](uint32_t gb_) {   // needs: head of `nxt` landed (cp.async.wait_group 0 + __syncwarp)
                     pend_d = lds_desc(pa.desc(mslot));
                     pend_tile = lds32(pa.desc(mslot) + 16);
@@ -855,7 +928,7 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                         else if (pend_d.G > (uint32_t)kHeadGroups + 1u) prefetch_l2(p.g.col4 + tail_at + kSubRows);
                         if (lane == 0) prefetch_l2(p.g.w4 + tail_at);
                     }
-                    u_pos += n_static;
+                    u_pos += ns;
                     have = u_pos < nu;
                     if (have) {
                         mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
@@ -902,9 +975,9 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             // static data of this warp's first slice of the next phase: issued before the barrier
             ps0 = psn0;
             nu = (psn1 - psn0) * tiles;
-            have = !very_last && u_static < nu;
-            if (have && u_static + n_static < nu) {   // this warp's second unit: head towards L2
-                const uint32_t u2 = u_static + n_static;
+            have = !very_last && usn < nu;
+            if (have && usn + nsn < nu) {   // this warp's second unit: head towards L2
+                const uint32_t u2 = usn + nsn;
                 const uint32_t s2 = ps0 + (tiles == 1u ? u2 : u2 / tiles);
                 const size_t at2 = (size_t)s2 * (kHeadGroups * kSubRows) + sr;
                 prefetch_l2(half == 0 ? p.g.col4 + at2 : p.g.col4 + at2 + kSubRows);
@@ -912,8 +985,8 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
             }
             if (have) {
                 mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
-                nxt = tiles == 1u ? request_head(p.g, pa, mslot, ps0 + u_static, 0u, sr, lane)
-                              : request_head(p.g, pa, mslot, ps0 + u_static / tiles, u_static % tiles, sr, lane);
+                nxt = tiles == 1u ? request_head(p.g, pa, mslot, ps0 + usn, 0u, sr, lane)
+                              : request_head(p.g, pa, mslot, ps0 + usn / tiles, usn % tiles, sr, lane);
             }
 
             if (last_phase) {   // a7: this sweep's energy increments -> accum slot t % 3
@@ -953,6 +1026,17 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
         }
 
         if constexpr (!CLUSTER) if (chain_on) {
+            if constexpr (OV) {   // beside the chain: virtual phase 0 of sweep t + 1, then the head of this warp's first unit of phase 1
+                if (more_sweeps) run_phase0_parked();
+                ps0 = ps_of(1u);
+                nu = (ps_of(2u) - ps0) * tiles;
+                have = more_sweeps && u_static < nu;
+                if (have) {
+                    mslot = mslot == kMetaSlots - 1u ? 0u : mslot + 1u;
+                    nxt = tiles == 1u ? request_head(p.g, pa, mslot, ps0 + u_static, 0u, sr, lane)
+                                      : request_head(p.g, pa, mslot, ps0 + u_static / tiles, u_static % tiles, sr, lane);
+                }
+            }
             // the chain: the last colour classes level by level inside one CTA per word of four replicas
             if (chain_cta) {
                 const ChainView& v = p.chain;
@@ -1001,6 +1085,32 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                 }
             }
             __syncthreads();
+        }
+        // chain overlap: the rows of virtual phase 0 were updated for sweep t + 1 before this sweep's improved mask
+        // was known; the values they held (parked in `alt`) are captured now
+        if constexpr (OV) if (more_sweeps) {
+            for (uint32_t tile = 0; tile < tiles; ++tile) {
+                const uint32_t mask = s_mask[tile];
+                if (mask == 0u) continue;
+                const uint4* alt = reinterpret_cast<const uint4*>(p.alt + (size_t)tile * p.tile_stride);
+                uint4* best = reinterpret_cast<uint4*>(bestp() + (size_t)tile * p.tile_stride);
+                const uint32_t m_lo = mask & 0xffffu, m_hi = mask >> 16;
+                const uint32_t units = p.ov_rows * 2u;
+                for (uint32_t uu = cta * blockDim.x + threadIdx.x; uu < units; uu += n_cta * blockDim.x) {
+                    const uint32_t m = (uu & 1u) ? m_hi : m_lo;
+                    if (m == 0u) continue;
+                    const uint4 v = __ldcg(alt + uu);
+                    if (m == 0xffffu) { best[uu] = v; continue; }
+                    uint4 b = __ldcg(best + uu);
+                    const uint32_t k0 = nibble_to_bytemask(m & 15u), k1 = nibble_to_bytemask((m >> 4) & 15u);
+                    const uint32_t k2 = nibble_to_bytemask((m >> 8) & 15u), k3 = nibble_to_bytemask((m >> 12) & 15u);
+                    b.x = (v.x & k0) | (b.x & ~k0);
+                    b.y = (v.y & k1) | (b.y & ~k1);
+                    b.z = (v.z & k2) | (b.z & ~k2);
+                    b.w = (v.w & k3) | (b.w & ~k3);
+                    best[uu] = b;
+                }
+            }
         }
     }
 
