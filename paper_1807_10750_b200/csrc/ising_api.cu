@@ -754,8 +754,12 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
             const size_t mark = slices.size();
             const uint32_t hub_mark = n_hub_rows;
             const int32_t k_end = emit_colour(c, k, kSubRowEdges);
+            uint64_t sub8_units = (uint64_t)sm_count * kWarpsPerCta / 2;   // latency-bound phase: less than half a round of the grid's warps
+#ifdef ISING_TUNING_ENV
+            if (const char* e = getenv("ISING_SUB8_UNITS")) sub8_units = (uint64_t)atoll(e);
+#endif
             if (c < c_tail &&   // (the tail classes are throughput work of the bulk pseudo-phase)
-                (uint64_t)(slices.size() - mark) * tiles_all * 2ull < (uint64_t)sm_count * kWarpsPerCta) {   // latency-bound phase: less than half a round of the grid's warps
+                (uint64_t)(slices.size() - mark) * tiles_all < sub8_units) {
                 slices.resize(mark);
                 slice_aux.resize(2 * mark);
                 n_hub_rows = hub_mark;

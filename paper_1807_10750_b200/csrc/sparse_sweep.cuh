@@ -1063,7 +1063,9 @@ __global__ void __launch_bounds__(kSweepThreads, 1) k_anneal_gs(const AnnealPara
                                                                          4u * cgrp + threadIdx.x), (unsigned long long)v4);
                 }
             }
-            grid_barrier<CLUSTER>(p.barrier, epoch, n_cta, tsw ? tsw + (size_t)VP * n_cta * 8 : nullptr);
+            // (diagnostics, OV: the chain step of the sweep before the recorded one is that sweep's virtual phase 0: row 0)
+            grid_barrier<CLUSTER>(p.barrier, epoch, n_cta, tsw ? tsw + (size_t)VP * n_cta * 8
+                                  : (OV && p.timing && t + 1u == p.timing_sweep) ? p.timing + (size_t)cta * 8 : nullptr);
         }
 
         // sweep end (every CTA redundantly): E, cut = (W - E)/2 (eq. 4), improved mask

@@ -50,6 +50,9 @@ def report(wl, sweep: int, flags: int = 0, out=sys.stdout):
     else:
         rows = p.info(15) + (1 if eng == B.ENGINE_GRID_TAIL_CHAIN else 0)
         total = 0
+        if p.info(19) > 0:
+            print("  chain overlap: virtual phase 0 = %d rows of colour class 0 without a chain neighbour, updated beside the "
+                  "chain of the sweep before (row 0 below = that chain step's barrier)" % p.info(19), file=out)
         for ph in range(rows):
             arrive, leave = b[ph, :, 0], b[ph, :, 1]
             wait = leave - arrive
