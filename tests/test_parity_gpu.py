@@ -416,8 +416,11 @@ ENGINE_FLAGS = {
     "cluster": P.ISING_LOAD_NO_SMALL,                                # one thread-block cluster per replica tile
     "grid": P.ISING_LOAD_NO_SMALL | P.ISING_LOAD_NO_CLUSTER | P.ISING_LOAD_NO_TAIL_CHAIN,   # cooperative grid, every class a phase
     "grid+tail": P.ISING_LOAD_NO_SMALL | P.ISING_LOAD_NO_CLUSTER,    # cooperative grid, last classes as a shared-memory chain
+    # ... and without the chain overlap (class 0 in one piece, the chain step on its own)
+    "grid+tail-overlap": P.ISING_LOAD_NO_SMALL | P.ISING_LOAD_NO_CLUSTER | P.ISING_LOAD_NO_OVERLAP,
 }
-ENGINE_CODE = {"small": P.ENGINE_SMALL, "cluster": P.ENGINE_CLUSTER, "grid": P.ENGINE_GRID, "grid+tail": P.ENGINE_GRID_TAIL_CHAIN}
+ENGINE_CODE = {"small": P.ENGINE_SMALL, "cluster": P.ENGINE_CLUSTER, "grid": P.ENGINE_GRID, "grid+tail": P.ENGINE_GRID_TAIL_CHAIN,
+               "grid+tail-overlap": P.ENGINE_GRID_TAIL_CHAIN}
 
 
 @pytest.mark.parametrize("engine", ["small", "cluster", "grid"])
@@ -435,17 +438,19 @@ def test_small_graph_through_every_gauss_seidel_engine(engine):
     np.testing.assert_array_equal(g2["final"], oracle_anneal(wl)["final"])
 
 
-@pytest.mark.parametrize("engine", ["grid", "grid+tail"])
+@pytest.mark.parametrize("engine", ["grid", "grid+tail", "grid+tail-overlap"])
 @pytest.mark.parametrize("replicas,first", [(32, 0), (70, 5)])
 def test_power_law_graph_with_and_without_tail_chain(engine, replicas, first):
     """Config-5-shaped graph: the last colour classes (few hub rows each) run as a shared-memory chain after one bulk
-    pseudo-phase, or as grid-wide phases.  Ragged replica count over several tiles, a first replica that is not a
+    pseudo-phase (with the chain-free rows of class 0 of the next sweep updated beside the chain, or without that
+    overlap), or as grid-wide phases.  Ragged replica count over several tiles, a first replica that is not a
     multiple of four (two Philox calls per word), KEEP ties, trace / best state, and a continued run."""
     wl = W.config5(n=120000, sweeps=9, replicas=replicas)
     g = gpu_anneal(wl, first_replica=first, tie_rule=1, flags=ENGINE_FLAGS[engine])
     assert g["problem"].engine == ENGINE_CODE[engine]
-    if engine == "grid+tail":
+    if engine.startswith("grid+tail"):
         assert 0 < g["problem"].info(14) <= 12288 and g["problem"].info(15) < wl.n_colours
+        assert (g["problem"].info(19) > 0) == (engine == "grid+tail")   # rows of the overlapped part of class 0
     o = oracle_anneal(wl, first_replica=first, tie_rule=1, n_threads=16)
     assert_same(g, o)
     g1 = gpu_anneal(wl, thr=wl.thr[:4], first_replica=first, problem=g["problem"], want_best_spins=False)
