@@ -591,12 +591,13 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
     if (ising_status s = fetch_runs(side.s)) return s;
     if (rep.err_mask) { (void)cudaStreamSynchronize(st); return ISING_ERR_BAD_SHAPE; }   // (the copies read the caller's arrays)
     LT("relabel done (runs on host)");
-    // ---- validate on the device (row_ptr is sound from here on); the report is read before anything is packed
-    {
+    // ---- validate on the device (row_ptr is sound from here on); the report is read before anything is packed.
+    // (Launched below, behind the overlap split and its relabelling: the host waits for those, not for the validation.)
+    auto enqueue_validate = [&]() {
         const long long warps = n;
         const unsigned blocks = (unsigned)((warps * 32 + 255) / 256);
         k_validate<<<blocks, 256, 0, st>>>(n, d_row_ptr, d_col, d_w, wtype, d_colour, n_colours, d_rep);
-    }
+    };
     auto read_report = [&]() -> ising_status {
         CK(cudaMemcpyAsync(&rep, d_rep, sizeof(rep), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
@@ -672,6 +673,7 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         split0 = true;
         LT("overlap split + second relabel");
     }
+    enqueue_validate();
     // ---- work units: hubs (rows above kHubDegree, one CTA each) and slices (one warp each)
     int sm_count = 148, coop = 0;
     {
