@@ -34,7 +34,8 @@ constexpr int kSmallThreadsMax = 512;           // (measured on configs 1-3: 512
 
 struct ChainSeg {
     uint32_t r0, r1;   // local rows [r0, r1) of one level, inside one chunk
-    uint32_t info;     // bits 0-7: log2(lanes per row); bit 8: the level ends with this segment (CTA barrier follows)
+    uint32_t info;     // bits 0-7: log2(lanes per row); bit 8: the level ends with this segment (CTA barrier follows);
+                       // bit 9: more rows than the planned CTA has lane groups (a thread walks several rows)
     uint32_t pad;
 };
 struct ChainChunk {
@@ -236,17 +237,18 @@ __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChun
             h3 = __dp4a((int)t3, (int)w, h3);
         }
         // (a REDUX per group member mask was measured 3x slower than the butterfly: the groups of a warp are serialised)
-        if (L > 1u) {
-#pragma unroll
-            for (uint32_t o = 1; o < 32u; o <<= 1) {
-                if (o < L) {
-                    h0 += __shfl_xor_sync(0xffffffffu, h0, o);
-                    h1 += __shfl_xor_sync(0xffffffffu, h1, o);
-                    h2 += __shfl_xor_sync(0xffffffffu, h2, o);
-                    h3 += __shfl_xor_sync(0xffffffffu, h3, o);
-                }
-            }
+        // exactly log2(L) butterfly levels, entered by one jump (the order of the levels does not matter for a sum)
+#define ISING_BFLY(o) h0 += __shfl_xor_sync(0xffffffffu, h0, o); h1 += __shfl_xor_sync(0xffffffffu, h1, o); \
+                      h2 += __shfl_xor_sync(0xffffffffu, h2, o); h3 += __shfl_xor_sync(0xffffffffu, h3, o);
+        if (L > 1u) switch (logL) {
+            case 5: ISING_BFLY(16)   // fall through
+            case 4: ISING_BFLY(8)    // fall through
+            case 3: ISING_BFLY(4)    // fall through
+            case 2: ISING_BFLY(2)    // fall through
+            case 1: ISING_BFLY(1)    // fall through
+            default: break;
         }
+#undef ISING_BFLY
         uint32_t a = ~sign_bytes(h0, h1, h2, h3) | 0x01010101u;   // +1 where h < 0, else -1
         if (rt.tie_rule == 1) {                                   // KEEP: h == 0 leaves the spin
             const uint32_t z = (h0 == 0 ? 0xffu : 0u) | (h1 == 0 ? 0xff00u : 0u) | (h2 == 0 ? 0xff0000u : 0u) |
@@ -473,6 +475,8 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
     }
     ChainGlobal cg{};
     long long dE[4] = {0, 0, 0, 0};
+    const uint32_t n_segs = v.n_segs;
+    const uint32_t n32_bit = (v.narrow != 0u && nthr == v.threads) ? 0x200u : 0u;   // (bit 9 of a segment was planned for v.threads)
     for (uint32_t t = 0; t < p.n_sweeps; ++t) {
         rt.thr = __ldg(p.thr + t);
         rt.T = p.sweep_offset + t;
@@ -488,9 +492,9 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
             }
             if (TIMING && ts) *ts++ = (unsigned long long)clock64();
             const ChainChunk ck = s_chunks[0];
-            for (uint32_t s = 0; s < v.n_segs; ++s) {
+            for (uint32_t s = 0; s < n_segs; ++s) {
                 const ChainSeg sg = s_segs[s];
-                if (v.narrow != 0u && sg.r1 - sg.r0 > (nthr >> (sg.info & 0xffu)))   // several rows per thread
+                if (sg.info & n32_bit)   // several rows per thread and all sums fit 32 bits
                     chain_segment<false, PREMUL, true>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
                 else
                     chain_segment<false, PREMUL, false>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);

@@ -380,7 +380,7 @@ ChainPlan plan_chain(const std::vector<uint32_t>& counts, const std::vector<uint
             while ((1u << logL) < L) ++logL;
             ChainSeg sg{};
             sg.r0 = s0; sg.r1 = s1;
-            sg.info = logL | (b <= ck.r1 ? 0x100u : 0u);
+            sg.info = logL | (b <= ck.r1 ? 0x100u : 0u) | ((s1 - s0) > (threads >> logL) ? 0x200u : 0u);
             pl.segs.push_back(sg);
         }
         ck.seg1 = (uint32_t)pl.segs.size();
