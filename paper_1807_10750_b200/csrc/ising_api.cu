@@ -655,7 +655,6 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
     // t + 1, the rows of colour class 0 that have no neighbour among the chain's rows (builder.cuh k_split_class0: they
     // become a colour class of their own in front of the rest of class 0; same Gauss-Seidel result).  Needs the edges on
     // the device, so the relabelling is repeated on the caller's stream behind the copies.
-    const int32_t* d_colour_eff = d_colour;   // the colouring the internal row order follows
     bool split0 = false;
     if (c_tail < C && (int64_t)n > (int64_t)kChainMaxLocal && !(flags & ISING_LOAD_NO_OVERLAP)) {
         int32_t* d_colour2 = (int32_t*)ws.take(4 * (size_t)n);
@@ -669,7 +668,6 @@ ising_status load_csr_impl(int32_t n, int64_t nnz, const int64_t* row_ptr, const
         if (ising_status s = fetch_runs(st)) { (void)cudaStreamSynchronize(st); return s; }
         sort_runs();
         c_tail = tail_start();
-        d_colour_eff = d_colour2;
         split0 = true;
         LT("overlap split + second relabel");
     }
