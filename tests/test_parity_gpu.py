@@ -459,6 +459,20 @@ def test_power_law_graph_with_and_without_tail_chain(engine, replicas, first):
     np.testing.assert_array_equal(g2["final"], oracle_anneal(wl, first_replica=first, n_threads=16)["final"])
 
 
+def test_chain_overlap_layout_with_more_tiles_than_the_overlap_takes():
+    """The overlap split of class 0 is part of the loaded layout, but a launch overlaps only while the chain CTAs are at
+    most half the grid (8 per tile): 10 tiles run the split layout with the chain step on its own, and a later call with
+    few replicas on the same handle overlaps again.  Both must match the oracle."""
+    wl = W.config5(n=70000, sweeps=4, replicas=300)
+    g = gpu_anneal(wl, want_best_spins=False)
+    assert g["problem"].engine == P.ENGINE_GRID_TAIL_CHAIN and g["problem"].info(19) > 0
+    o = oracle_anneal(wl, n_threads=16)
+    assert_same(g, o, best_spins=False)
+    g2 = gpu_anneal(wl, n_replicas=40, problem=g["problem"])
+    o2 = oracle_anneal(wl, n_replicas=40, n_threads=16)
+    assert_same(g2, o2)
+
+
 @pytest.mark.parametrize("flags", [0, P.ISING_LOAD_NO_CLUSTER])
 def test_small_graph_flip_producer_with_zero_threshold_sweeps(flags):
     """Small-graph engine as a cluster of two CTAs per word (levels + flip producer) and as one CTA per word: sweeps
