@@ -290,6 +290,97 @@ __device__ __forceinline__ void chain_segment(const ChainSeg sg, const ChainChun
     if (N32) { dE[0] += e0s; dE[1] += e1s; dE[2] += e2s; dE[3] += e3s; }
 }
 
+// chain_segment<false, PREMUL, true> for segments in which a thread walks SEVERAL rows (throughput-bound levels: config
+// 3's checkerboard classes, the big classes of config 2): two rows per trip.  The rows of a level are independent, so
+// the two dependent chains (cell pointers -> neighbour offsets -> spin words -> dp4a -> butterfly -> update) interleave.
+// A row that has run out of cells rides along on cell 0 of the chunk with weight 0.
+template <bool PREMUL>
+__device__ __forceinline__ void chain_segment_rows2(const ChainSeg sg, const ChainChunk& ck, uint32_t buf, uint32_t val,
+                                                    uint32_t flip, const ChainRt& rt, long long (&dE)[4], uint32_t tid,
+                                                    uint32_t nthr) {
+    const uint32_t logL = sg.info & 0xffu, L = 1u << logL, q = tid & (L - 1u);
+    const uint32_t rpi = nthr >> logL;
+    const ChunkLayout l = chunk_layout(ck.r1 - ck.r0, ck.c1 - ck.c0, false);
+    const uint32_t s_lo = sg.r0, s_hi = sg.r1;
+    const uint32_t fmask = rt.thr != 0u ? 15u : 0u;
+    int es0 = 0, es1 = 0, es2 = 0, es3 = 0;
+    uint32_t r = s_lo + (tid >> logL);
+    for (uint32_t rw = s_lo + ((tid & ~31u) >> logL); rw < s_hi; rw += 2u * rpi, r += 2u * rpi) {   // warp-uniform trip count
+        const uint32_t rB = r + rpi;
+        const bool stA = r < s_hi && q == 0u, stB = rB < s_hi && q == 0u;
+        const uint32_t rowA = min(r, s_hi - 1u), rowB = min(rB, s_hi - 1u);
+        const uint32_t lrA = rowA - ck.r0, lrB = rowB - ck.r0;
+        const uint32_t p0A = lds16(buf + l.ptr + 2u * lrA), p1A = lds16(buf + l.ptr + 2u * lrA + 2u);
+        const uint32_t p0B = lds16(buf + l.ptr + 2u * lrB), p1B = lds16(buf + l.ptr + 2u * lrB + 2u);
+        const uint32_t fA = lds8(flip + rowA) & fmask, fB = lds8(flip + rowB) & fmask;
+        const uint32_t oldA = lds32(val + 4u * rowA), oldB = lds32(val + 4u * rowB);
+        int a0 = 0, a1 = 0, a2 = 0, a3 = 0, b0 = 0, b1 = 0, b2 = 0, b3 = 0;
+        uint32_t kA = p0A + q, kB = p0B + q;
+        while (kA < p1A || kB < p1B) {
+            const bool ha = kA < p1A, hb = kB < p1B;
+            const uint32_t ka = ha ? kA : 0u, kb = hb ? kB : 0u;
+            const uint2 ix = lds64(buf + l.idx + 8u * ka), jx = lds64(buf + l.idx + 8u * kb);
+            uint32_t wa = lds32(buf + l.w + 4u * ka), wb = lds32(buf + l.w + 4u * kb);
+            wa = ha ? wa : 0u;
+            wb = hb ? wb : 0u;
+            uint32_t e0, e1, e2, e3, f0, f1, f2, f3;
+            if (PREMUL) {
+                e0 = lds32(val + (ix.x & 0xffffu)); e1 = lds32(val + (ix.x >> 16));
+                e2 = lds32(val + (ix.y & 0xffffu)); e3 = lds32(val + (ix.y >> 16));
+                f0 = lds32(val + (jx.x & 0xffffu)); f1 = lds32(val + (jx.x >> 16));
+                f2 = lds32(val + (jx.y & 0xffffu)); f3 = lds32(val + (jx.y >> 16));
+            } else {
+                e0 = lds32(val + 4u * (ix.x & 0xffffu)); e1 = lds32(val + 4u * (ix.x >> 16));
+                e2 = lds32(val + 4u * (ix.y & 0xffffu)); e3 = lds32(val + 4u * (ix.y >> 16));
+                f0 = lds32(val + 4u * (jx.x & 0xffffu)); f1 = lds32(val + 4u * (jx.x >> 16));
+                f2 = lds32(val + 4u * (jx.y & 0xffffu)); f3 = lds32(val + 4u * (jx.y >> 16));
+            }
+            uint32_t t0, t1, t2, t3, u0, u1, u2, u3;
+            transpose4x4(e0, e1, e2, e3, t0, t1, t2, t3);
+            transpose4x4(f0, f1, f2, f3, u0, u1, u2, u3);
+            a0 = __dp4a((int)t0, (int)wa, a0); a1 = __dp4a((int)t1, (int)wa, a1);
+            a2 = __dp4a((int)t2, (int)wa, a2); a3 = __dp4a((int)t3, (int)wa, a3);
+            b0 = __dp4a((int)u0, (int)wb, b0); b1 = __dp4a((int)u1, (int)wb, b1);
+            b2 = __dp4a((int)u2, (int)wb, b2); b3 = __dp4a((int)u3, (int)wb, b3);
+            kA += L;
+            kB += L;
+        }
+#define ISING_BFLY2(o) a0 += __shfl_xor_sync(0xffffffffu, a0, o); a1 += __shfl_xor_sync(0xffffffffu, a1, o); \
+                       a2 += __shfl_xor_sync(0xffffffffu, a2, o); a3 += __shfl_xor_sync(0xffffffffu, a3, o); \
+                       b0 += __shfl_xor_sync(0xffffffffu, b0, o); b1 += __shfl_xor_sync(0xffffffffu, b1, o); \
+                       b2 += __shfl_xor_sync(0xffffffffu, b2, o); b3 += __shfl_xor_sync(0xffffffffu, b3, o);
+        if (L > 1u) switch (logL) {
+            case 5: ISING_BFLY2(16)   // fall through
+            case 4: ISING_BFLY2(8)    // fall through
+            case 3: ISING_BFLY2(4)    // fall through
+            case 2: ISING_BFLY2(2)    // fall through
+            case 1: ISING_BFLY2(1)    // fall through
+            default: break;
+        }
+#undef ISING_BFLY2
+        uint32_t xa = ~sign_bytes(a0, a1, a2, a3) | 0x01010101u;   // +1 where h < 0, else -1
+        uint32_t xb = ~sign_bytes(b0, b1, b2, b3) | 0x01010101u;
+        if (rt.tie_rule == 1) {                                    // KEEP: h == 0 leaves the spin
+            const uint32_t za = (a0 == 0 ? 0xffu : 0u) | (a1 == 0 ? 0xff00u : 0u) | (a2 == 0 ? 0xff0000u : 0u) |
+                                (a3 == 0 ? 0xff000000u : 0u);
+            const uint32_t zb = (b0 == 0 ? 0xffu : 0u) | (b1 == 0 ? 0xff00u : 0u) | (b2 == 0 ? 0xff0000u : 0u) |
+                                (b3 == 0 ? 0xff000000u : 0u);
+            xa = (xa & ~za) | (oldA & za);
+            xb = (xb & ~zb) | (oldB & zb);
+        }
+        xa ^= ((fA * 0x00204081u) & 0x01010101u) * 0xfeu;
+        xb ^= ((fB * 0x00204081u) & 0x01010101u) * 0xfeu;
+        const uint32_t dA = stA ? (xa << 1) & (xa ^ oldA) : 0u, dB = stB ? (xb << 1) & (xb ^ oldB) : 0u;
+        es0 += sbyte(dA, 0) * a0 + sbyte(dB, 0) * b0;
+        es1 += sbyte(dA, 1) * a1 + sbyte(dB, 1) * b1;
+        es2 += sbyte(dA, 2) * a2 + sbyte(dB, 2) * b2;
+        es3 += sbyte(dA, 3) * a3 + sbyte(dB, 3) * b3;
+        if (stA) sts32(val + 4u * rowA, xa);
+        if (stB) sts32(val + 4u * rowB, xb);
+    }
+    dE[0] += es0; dE[1] += es1; dE[2] += es2; dE[3] += es3;
+}
+
 // One pass over all chain levels (one sweep of the chain rows), chunks streamed through two buffers.
 // s_chunks / s_segs: the tables in shared memory.  DELTA: h0 of a chunk is cleared once it has landed.
 template <bool DELTA, bool PREMUL>
@@ -495,7 +586,7 @@ __global__ void __launch_bounds__(kSmallThreadsMax, 1) k_anneal_small(const Smal
             for (uint32_t s = 0; s < n_segs; ++s) {
                 const ChainSeg sg = s_segs[s];
                 if (sg.info & n32_bit)   // several rows per thread and all sums fit 32 bits
-                    chain_segment<false, PREMUL, true>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
+                    chain_segment_rows2<PREMUL>(sg, ck, buf0, val, flip, rt, dE, tid, nthr);
                 else
                     chain_segment<false, PREMUL, false>(sg, ck, buf0, val, flip, rt, p.keys, dE, cg, tid, nthr);
                 if (sg.info & 0x100u) __syncthreads();
